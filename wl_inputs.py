@@ -1,0 +1,155 @@
+"""Seeded synthetic inputs and the workload catalogue, shared by the oracle tests, the GPU
+parity tests and bench.py.
+
+This module holds NONE of the method's arithmetic (no stencils, kernels, SDFs, solvers):
+only plain parameter dictionaries (the five BASELINE.json configs in grid units, see
+DESIGN.md section 4) and a seeded random-field generator.  Both the oracle binding
+(oracle/wl_oracle.py) and the CUDA binding (paper_2407_16032_b200/wl.py) turn these
+dictionaries into their own config structs.
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+
+SEED = 20240716  # per-kernel parity inputs
+
+BODY_NONE, BODY_SPHERE, BODY_TORUS = 0, 1, 2
+MOTION_STATIC, MOTION_HEAVE_SIN = 0, 1
+
+CONFIG_DEFAULTS = dict(
+    ndim=3, dims=(32, 32, 32), L=1.0, U=(1.0, 0.0, 0.0), nu=0.01,
+    periodic=(0, 0, 0), exit_bc=0, eps=1.0,
+    dt0=0.25, dt_max=10.0, cfl_c=1.0, cfl_cnu=5.0,
+    body_kind=BODY_NONE, centre=(0.0, 0.0, 0.0), R=0.0, r=0.0, axis=0,
+    motion=MOTION_STATIC, heave_dir=1, amp=0.0, freq=0.0, phase=0.0,
+    max_levels=0, smooth_iters=6, max_vcycles=32, fixed_vcycles=2, tol=1e-4,
+)
+
+
+def make(**kw) -> dict:
+    cfg = dict(CONFIG_DEFAULTS)
+    for k, v in kw.items():
+        if k not in cfg:
+            raise KeyError(k)
+        cfg[k] = v
+    return cfg
+
+
+def tgv2d(n=64, nu_phys=0.01, **kw) -> dict:
+    """C1: 2-D Taylor-Green vortex on [0,2pi)^2, n x n periodic; grid units h = 2pi/n."""
+    h = 2 * math.pi / n
+    base = dict(ndim=2, dims=(n, n), L=n / (2 * math.pi), U=(0.0, 0.0, 0.0), nu=nu_phys / h,
+                periodic=(1, 1), max_levels=4)
+    base.update(kw)
+    return make(**base)
+
+
+def tgv3d(n=128, Re=1600.0, **kw) -> dict:
+    """C2: 3-D Taylor-Green vortex, n^3 periodic, Re = U L_ref / nu with L_ref = 1/kappa."""
+    Lref = n / (2 * math.pi)
+    base = dict(ndim=3, dims=(n, n, n), L=Lref, U=(0.0, 0.0, 0.0), nu=Lref / Re, periodic=(1, 1, 1))
+    base.update(kw)
+    return make(**base)
+
+
+def sphere(dims=(256, 128, 128), D=32.0, Re=3700.0, centre=None, **kw) -> dict:
+    """C3: static sphere, inflow +x, convective exit, slip side walls."""
+    centre = centre or (dims[0] / 4.0, dims[1] / 2.0, dims[2] / 2.0)
+    base = dict(ndim=3, dims=tuple(dims), L=D, U=(1.0, 0.0, 0.0), nu=D / Re, exit_bc=1,
+                body_kind=BODY_SPHERE, centre=tuple(centre), R=D / 2.0)
+    base.update(kw)
+    return make(**base)
+
+
+def torus(dims=(512, 256, 256), R=32.0, r=8.0, Re=1000.0, centre=None, **kw) -> dict:
+    """C4: static torus, axis along the inflow, Re on the minor diameter 2r."""
+    centre = centre or (dims[0] / 4.0, dims[1] / 2.0, dims[2] / 2.0)
+    base = dict(ndim=3, dims=tuple(dims), L=2 * r, U=(1.0, 0.0, 0.0), nu=2 * r / Re, exit_bc=1,
+                body_kind=BODY_TORUS, centre=tuple(centre), R=R, r=r, axis=0)
+    base.update(kw)
+    return make(**base)
+
+
+def heaving_sphere(dims=(384, 256, 256), D=48.0, Re=1000.0, St=0.2, amp_over_D=0.25, centre=None, **kw) -> dict:
+    """C5: sphere heaving in y, y(t) = amp sin(2 pi f t), St = f D / U."""
+    centre = centre or (dims[0] / 3.0, dims[1] / 2.0, dims[2] / 2.0)
+    base = dict(ndim=3, dims=tuple(dims), L=D, U=(1.0, 0.0, 0.0), nu=D / Re, exit_bc=1,
+                body_kind=BODY_SPHERE, centre=tuple(centre), R=D / 2.0,
+                motion=MOTION_HEAVE_SIN, heave_dir=1, amp=amp_over_D * D, freq=St / D)
+    base.update(kw)
+    return make(**base)
+
+
+def baseline_config(k: int, scale: int = 1) -> dict:
+    """BASELINE.json configs[k]; scale > 1 divides every length by `scale` (same shape,
+    same Reynolds number) for tests the oracle must finish in seconds."""
+    s = scale
+    if k == 0:
+        return tgv2d(64 // s)
+    if k == 1:
+        return tgv3d(128 // s)
+    if k == 2:
+        return sphere((256 // s, 128 // s, 128 // s), D=32.0 / s, centre=(64.0 / s, 64.0 / s, 64.0 / s))
+    if k == 3:
+        return torus((512 // s, 256 // s, 256 // s), R=32.0 / s, r=8.0 / s,
+                     centre=(128.0 / s, 128.0 / s, 128.0 / s))
+    if k == 4:
+        return heaving_sphere((384 // s, 256 // s, 256 // s), D=48.0 / s,
+                              centre=(128.0 / s, 128.0 / s, 128.0 / s))
+    raise IndexError(k)
+
+
+WORKLOAD_NAMES = ["C1_tgv2d_64", "C2_tgv3d_128", "C3_sphere_256x128x128",
+                  "C4_torus_512x256x256", "C5_heaving_sphere_384x256x256"]
+
+
+def rng(seed: int = SEED) -> np.random.Generator:
+    return np.random.Generator(np.random.MT19937(seed))
+
+
+def random_velocity(dims, seed: int = SEED, nmodes: int = 8, kmax: int = 4, step: float = 0.5,
+                    mean=(1.0, 0.0, 0.0)) -> np.ndarray:
+    """Interior-sized velocity (ndim, [Nz,] Ny, Nx), float64: a sum of `nmodes` random
+    Fourier modes (|k| <= kmax, amplitudes U(-0.5,0.5)) + a uniform stream + a planar step
+    of height `step` at x = N/3 (exercises both limiter branches and both flux signs)."""
+    g = rng(seed)
+    nd = len(dims)
+    shape = tuple(reversed(dims))
+    axes = [np.arange(n, dtype=np.float64) for n in dims]           # x, y[, z]
+    grids = np.meshgrid(*reversed(axes), indexing="ij")               # z, y, x order
+    grids = list(reversed(grids))                                     # -> x, y[, z]
+    u = np.zeros((nd,) + shape)
+    for c in range(nd):
+        for _ in range(nmodes):
+            k = g.integers(-kmax, kmax + 1, size=nd)
+            amp = g.uniform(-0.5, 0.5)
+            ph = g.uniform(0, 2 * math.pi)
+            arg = ph
+            for d in range(nd):
+                arg = arg + 2 * math.pi * k[d] * grids[d] / dims[d]
+            u[c] += amp * np.sin(arg)
+        u[c] += mean[c] if c < len(mean) else 0.0
+    u[0] += step * (grids[0] >= dims[0] / 3.0)
+    return u
+
+
+def random_scalar(dims, seed: int = SEED + 1, nmodes: int = 8, kmax: int = 4) -> np.ndarray:
+    """Interior-sized scalar ([Nz,] Ny, Nx), float64, random Fourier modes + white noise."""
+    g = rng(seed)
+    nd = len(dims)
+    shape = tuple(reversed(dims))
+    axes = [np.arange(n, dtype=np.float64) for n in dims]
+    grids = list(reversed(np.meshgrid(*reversed(axes), indexing="ij")))
+    a = np.zeros(shape)
+    for _ in range(nmodes):
+        k = g.integers(-kmax, kmax + 1, size=nd)
+        amp = g.uniform(-0.5, 0.5)
+        ph = g.uniform(0, 2 * math.pi)
+        arg = ph
+        for d in range(nd):
+            arg = arg + 2 * math.pi * k[d] * grids[d] / dims[d]
+        a += amp * np.sin(arg)
+    a += 0.1 * g.standard_normal(shape)
+    return a
