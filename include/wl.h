@@ -1,0 +1,167 @@
+/*
+ * wl.h -- C ABI of libwl: one incompressible BDIM time step (mom_step) on a B200.
+ *
+ * The operations are the routines the paper names for one time step of its solver
+ * (/root/reference/PAPER.md, cited "P:<line>"; Fig. 2 caption P:139 lists them:
+ * measure!, conv_diff!, BDIM!, BC!, exitBC!, scale_u!, project!, CFL!), on the uniform
+ * staggered Cartesian grid of P:74 with the boundary-data-immersion treatment of P:58-72
+ * (Eq. 1-2).  The paper defers every formula to cited works; the readings this library
+ * implements are written out in DESIGN.md section 3 ("R-<x>") and restate SURVEY.md 8(c).
+ *
+ * Conventions
+ *   - plain C, no exceptions, no global state; every call returns an int status
+ *     (WL_OK = 0, negative = error) unless stated otherwise.
+ *   - one handle = one CUDA stream; calls on one handle are not thread-safe.
+ *   - DEVICE memory is owned by the caller: the workspace passed to wl_sim_create is
+ *     allocated by the caller (through PyTorch in this repo), must be 256-byte aligned,
+ *     must outlive the handle, and is never freed by the library.
+ *   - grid units: spacing h = 1, density 1 ("no grid information is stored");
+ *     cell c (1-based interior index I_d = 2..N_d+1 in the paper) has centre
+ *     x = I_d - 3/2; u_i[I] lives on the LOWER i-face of cell I (forced by the stencil of
+ *     the pressure-gradient kernel u[I,i] -= c[I,i]*(p[I]-p[I-d(i)])).
+ *   - user-visible field buffers are INTERIOR-sized, x fastest: a scalar is
+ *     dims[2]*dims[1]*dims[0] floats (2-D: dims[1]*dims[0]); a vector field is ndim such
+ *     arrays back to back (component-major).  `on_device` says whether the pointer is a
+ *     device (1) or host (0) pointer.
+ *   - all arithmetic is fp32 on the device; reductions accumulate in fp64.
+ *   - there is no CPU fallback: every entry point that computes runs CUDA kernels.
+ */
+#ifndef WL_H
+#define WL_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* status codes */
+#define WL_OK        0
+#define WL_EINVAL   -1   /* bad argument / config (ndim not 2 or 3, a dim < 4, nu < 0, eps <= 0, unknown body) */
+#define WL_ENOMEM   -2   /* workspace too small or misaligned */
+#define WL_ECUDA    -3   /* CUDA error (sticky); text through wl_last_error */
+#define WL_ENOCONV  -4   /* tolerance-mode Poisson solve hit max_vcycles (result still written) */
+
+/* body kinds and motions: SDF + coordinate map of the paper's AutoBody */
+enum { WL_BODY_NONE = 0, WL_BODY_SPHERE = 1 /* circle in 2-D */, WL_BODY_TORUS = 2 };
+enum { WL_MOTION_STATIC = 0, WL_MOTION_HEAVE_SIN = 1 /* c(t) = c0 + amp sin(2 pi freq t + phase) e_heave */ };
+
+typedef struct {
+    int   kind;          /* WL_BODY_* */
+    float centre[3];     /* c0, grid units */
+    float R, r;          /* sphere radius R; torus major R, minor r */
+    int   axis;          /* torus axis 0..2 */
+    int   motion;        /* WL_MOTION_* */
+    int   heave_dir;     /* 0..2 */
+    float amp, freq, phase;
+} wl_body;
+
+typedef struct {
+    int   max_levels;    /* <= 0: coarsen while every N_d is even and > 4 */
+    int   smooth_iters;  /* Jacobi-PCG iterations per smoother call */
+    int   max_vcycles;   /* tolerance mode cap */
+    int   fixed_vcycles; /* > 0: exactly this many {V-cycle; smooth} per solve, no tolerance test */
+    float tol;           /* tolerance mode: stop when max|r| <= tol */
+} wl_mg;
+
+/* Problem statement (grid size, boundary velocity, length scale, viscosity, BC type,
+ * body).  POD, caller-owned, copied at create. */
+typedef struct {
+    int   ndim;          /* 2 or 3 */
+    int   dims[3];       /* interior cells N_d (dims[2] ignored in 2-D) */
+    float L;             /* length scale; only scales reported quantities */
+    float U[3];          /* boundary / inflow velocity */
+    float nu;            /* kinematic viscosity in grid units */
+    int   periodic[3];   /* per direction */
+    int   exit_bc;       /* convective exit on the +x plane */
+    float eps;           /* BDIM kernel half-width in cells */
+    float dt0, dt_max, cfl_c, cfl_cnu;   /* CFL rule, DESIGN.md R-U */
+    wl_body body;
+    wl_mg   mg;
+} wl_config;
+
+typedef struct wl_sim wl_sim;
+
+typedef struct {
+    int    vcycles[2];   /* V-cycles used by the predictor / corrector solve of the last step */
+    double res[2];       /* max|r| after each (tolerance mode only; -1 in fixed mode) */
+    int    nlevels;
+    int    kernel_launches;   /* kernels launched by this handle since create */
+    int    nan_flag;          /* 1 if the last CFL reduction saw a non-finite velocity */
+} wl_stats_t;
+
+/* Pure function: bytes of device workspace wl_sim_create needs; 0 on invalid config. */
+size_t wl_workspace_bytes(const wl_config* cfg);
+
+/* Create a simulation in caller-owned DEVICE memory `dev_ws` (>= wl_workspace_bytes,
+ * 256-B aligned).  `cuda_stream` is a cudaStream_t (NULL = default stream).  Initial state
+ * (R-V): u = U everywhere, p = 0, measure(0), multigrid hierarchy built, BC filled. */
+int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes, void* cuda_stream, wl_sim** out);
+
+/* Frees the host-side handle only (never the workspace).  Synchronises the stream. */
+int wl_sim_destroy(wl_sim* s);
+
+/* Set state from interior-sized buffers (NULL leaves a field untouched); u: ndim arrays,
+ * p: one.  Ghost cells are then filled by the BC rule.  Synchronises when host. */
+int wl_set_fields(wl_sim* s, const float* u, const float* p, int on_device);
+
+/* Taylor-Green initial condition of P:112-116 (Eq. 3-5) on the periodic box, staggered
+ * sampling; sign = +1 gives BASELINE.json's u = sin x cos y [cos z], v = -cos x sin y [cos z];
+ * sign = -1 gives the paper's.  p = 0. */
+int wl_init_tgv(wl_sim* s, int sign);
+
+/* measure!: evaluate the SDF and motion map at every face at time t (solver
+ * time units h/U), write mu0, mu1, body velocity V, then the Poisson diagonal and the
+ * coarse-level coefficients.  Call before wl_mom_step when the body moves (R-R:
+ * with t = t_n + dt).  Asynchronous. */
+int wl_measure(wl_sim* s, double t);
+
+/* mom_step ("explicit predictor-corrector", routine list P:139; reading R-K):
+ * one full Heun step with two pressure projections.  Asynchronous on the stream. */
+int wl_mom_step(wl_sim* s, float dt);
+
+/* CFL! ("time step is adapted automatically"): dt for the next step from the current
+ * velocity (reading R-U).  Synchronises. */
+int wl_cfl(wl_sim* s, float* dt_out);
+
+/* Pressure force ON THE BODY, grid units (rho = 1, h = 1), reading R-Z:
+ * F = -sum_cells p n K(d) at cell centres, body placed at time t.  Synchronises. */
+int wl_pressure_force(wl_sim* s, double t, float F_out[3]);
+
+/* Copy interior fields out; any pointer may be NULL.  u: ndim arrays; p, mu0 likewise
+ * (mu0: ndim arrays).  Synchronises when host. */
+int wl_get_fields(wl_sim* s, float* u, float* p, float* mu0, int on_device);
+
+/* Fused benchmark step: wl_measure(t) (only if the body moves) + wl_mom_step(dt) +
+ * the CFL reduction, all asynchronous; the new dt stays on the device and is read by
+ * wl_cfl_result.  With `adaptive` != 0 the NEXT call ignores `dt` and uses the device-
+ * resident dt (no host round trip).  */
+int wl_step(wl_sim* s, double t, float dt, int adaptive);
+
+/* ---- stage hooks: each applies one stage once to the current state (parity tests) ---- */
+int wl_dbg_conv_diff_bdim(wl_sim* s, float dt, int corrector); /* u0 must hold the step's start state: see wl_dbg_save_u0 */
+int wl_dbg_save_u0(wl_sim* s);                                 /* u0 <- u */
+int wl_dbg_bc(wl_sim* s);
+int wl_dbg_exit_bc(wl_sim* s, float dt);
+int wl_dbg_project(wl_sim* s, float w, float dt);
+int wl_dbg_residual(wl_sim* s);                                /* sigma = div u; r = sigma - A x on level 0 */
+int wl_dbg_restrict(wl_sim* s, int level);
+int wl_dbg_prolong(wl_sim* s, int level);
+int wl_dbg_smooth(wl_sim* s, int level, int iters);
+int wl_dbg_vcycle(wl_sim* s, int level);
+/* Raw access to a solver array for tests: name in {"u","u0","p","mu0","mu1","L","iD","x","r"};
+ * interior-sized copy into `out` (host), ncomp arrays; returns ncomp or a negative status. */
+int wl_dbg_get(wl_sim* s, const char* name, int level, float* out, size_t out_floats);
+int wl_dbg_set(wl_sim* s, const char* name, int level, const float* in, size_t in_floats);
+/* same as wl_dbg_get but the whole padded array (ghost cells included): (N_d + 2) per direction */
+int wl_dbg_get_padded(wl_sim* s, const char* name, int level, float* out, size_t out_floats);
+int wl_level_dims(const wl_sim* s, int level, int dims_out[3]);
+
+const char* wl_last_error(const wl_sim* s);
+int wl_stats(wl_sim* s, wl_stats_t* out);
+int wl_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WL_H */

@@ -194,8 +194,13 @@ double wlo_body_eval(const wlo_config *cf, const double *xpt, double t, double *
 }
 
 /* -------------------------------------------------- O7: Poisson diagonal
- * D_I = -sum_i (L[I,i] + L[I+d_i,i]);  iD = 1/D if D != 0 else 0 (reading R-O/S).
+ * D_I = -sum_i (L[I,i] + L[I+d_i,i]);  iD = 1/D if |D| > 2n*1e-6 else 0 (reading R-O/S:
+ * cells buried in the body decouple).  The threshold (WLO_DMIN per face) instead of an exact
+ * test for zero keeps cells whose faces all sit within ~1e-2 eps of the d = -eps shell out
+ * of the solve: their mu0 ~ 1e-6 or less, so 1/D would multiply fp32 round-off in div u by
+ * 1e6 or more and dominate the CG dot products.
  */
+#define WLO_DMIN 1e-6
 static void level_diag(wlo_level *g, int nd)
 {
 #pragma omp parallel for collapse(2)
@@ -206,7 +211,7 @@ static void level_diag(wlo_level *g, int nd)
                 double D = 0;
                 for (int i = 0; i < nd; ++i)
                     D -= g->L[i * g->ncell + id] + g->L[i * g->ncell + id + g->st[i]];
-                g->iD[id] = D != 0.0 ? 1.0 / D : 0.0;
+                g->iD[id] = fabs(D) > 2.0 * nd * WLO_DMIN ? 1.0 / D : 0.0;
             }
 }
 
@@ -567,15 +572,27 @@ static double level_maxabs_r(const wlo_sim *s, const wlo_level *g)
 /* -------------------------------------------------- O8: smoother
  * P:149 "a preconditioned conjugate gradient smoother (PCG) is employed in the geometric
  * multi-grid solver ... contains several reduction operations".  Reading R-S/T: Jacobi-
- * preconditioned CG, `its` iterations, restarted at every call; guard tau = 1e-30 on
- * |rho|; gamma = 0 or non-finite => return.  `q` doubles as the z work array.
+ * preconditioned CG, `its` iterations, restarted at every call:
+ *   z = e = iD r; rho0 = rho = r.z; if |rho| < tau return
+ *   loop k = 1..its: q = A e; gamma = q.e; (gamma = 0 or non-finite => return)
+ *                    alpha = rho/gamma; x += alpha e; r -= alpha q; if k == its break;
+ *                    z = iD r; rho' = r.z; if |rho'| < tau or |rho'| < theta |rho0| break;
+ *                    beta = rho'/rho; e = beta e + z; rho = rho'
+ * tau = 1e-30 only protects 0/0.  theta = 1e-8 stops the iteration once this call has reduced
+ * the residual by 1e-4 in the iD norm: continuing CG on a converged residual divides round-off
+ * by round-off (alpha = rho/gamma) and blows up -- in fp32 already on the 8x8 level of the
+ * 2-D Taylor-Green case, whose residual is a single eigenmode (converged after two iterations).
+ * A relative test makes the fp64 oracle and an fp32 implementation take the same branch.
+ * `q` doubles as the z work array.
  */
 #define WLO_TAU 1e-30
+#define WLO_THETA 1e-8
 void wlo_smooth(wlo_sim *s, int l, int its)
 {
     wlo_level *g = &s->lev[l];
     int nd = s->nd;
     double rho = level_dot_riDr(s, g, g->e);    /* z = e = iD r ; rho = r.z */
+    double rho0 = rho;
     if (fabs(rho) < WLO_TAU) return;
     for (int k = 1; k <= its; ++k) {
         double gamma = level_matvec(s, g, g->e, g->q);  /* q = A e ; gamma = q.e */
@@ -591,7 +608,7 @@ void wlo_smooth(wlo_sim *s, int l, int its)
                 }
         if (k == its) break;
         double rho2 = level_dot_riDr(s, g, g->q);   /* z (in q) = iD r ; rho' = r.z */
-        if (fabs(rho2) < WLO_TAU) break;
+        if (fabs(rho2) < WLO_TAU || fabs(rho2) < WLO_THETA * fabs(rho0)) break;
         double beta = rho2 / rho;
 #pragma omp parallel for collapse(2)
         for (int c2 = ZLO(g, nd); c2 <= ZHI(g, nd); ++c2)

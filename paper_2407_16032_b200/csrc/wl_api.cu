@@ -1,0 +1,518 @@
+// wl_api.cu -- host side of libwl: workspace layout, the mom_step sequence, and the C ABI of
+// include/wl.h.  No torch types; plain pointers and sizes only.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <cmath>
+#include "wl_internal.h"
+
+// ------------------------------------------------------------------ launch geometry
+dim3 wl_block(int nd) { return nd == 3 ? dim3(32, 4, 4) : dim3(32, 16, 1); }
+
+Tiling wl_tiling(int nd, const int o[3], const int e[3])
+{
+    dim3 b = wl_block(nd);
+    Tiling T;
+    for (int d = 0; d < 3; ++d) { T.o[d] = o[d]; T.e[d] = e[d]; }
+    T.ntx = (e[0] + b.x - 1) / b.x;
+    T.nty = (e[1] + b.y - 1) / b.y;
+    T.ntz = (e[2] + b.z - 1) / b.z;
+    T.ntiles = T.ntx * T.nty * T.ntz;
+    return T;
+}
+Tiling wl_tiles_interior(const wl_sim* s, const Grid& g)
+{
+    int o[3] = { 1, 1, s->nd == 3 ? 1 : 0 };
+    int e[3] = { g.n[0], g.n[1], s->nd == 3 ? g.n[2] : 1 };
+    return wl_tiling(s->nd, o, e);
+}
+Tiling wl_tiles_padded(const wl_sim* s, const Grid& g)
+{
+    int o[3] = { 0, 0, 0 };
+    int e[3] = { g.S[0], g.S[1], g.S[2] };
+    return wl_tiling(s->nd, o, e);
+}
+int wl_grid(const wl_sim* s, const Tiling& T)
+{
+    int cap = s->sm_count * 4;
+    if (cap > WL_MAX_PARTIALS) cap = WL_MAX_PARTIALS;
+    return T.ntiles < cap ? (T.ntiles > 0 ? T.ntiles : 1) : cap;
+}
+FlowP wl_flowp(const wl_sim* s)
+{
+    FlowP P;
+    P.g = s->lev[0].g;
+    P.nu = s->cfg.nu;
+    for (int k = 0; k < 3; ++k) P.U[k] = s->cfg.U[k];
+    P.exit_bc = s->cfg.exit_bc;
+    return P;
+}
+
+// ------------------------------------------------------------------ config / layout
+static int config_ok(const wl_config* c)
+{
+    if (!c) return 0;
+    if (c->ndim != 2 && c->ndim != 3) return 0;
+    for (int d = 0; d < c->ndim; ++d) if (c->dims[d] < 4 || c->dims[d] > 16384) return 0;
+    if (!(c->nu >= 0.0f) || !(c->eps > 0.0f)) return 0;
+    if (c->body.kind < 0 || c->body.kind > 2) return 0;
+    if (c->body.kind == WL_BODY_TORUS && (c->ndim != 3 || c->body.axis < 0 || c->body.axis > 2)) return 0;
+    if (c->body.motion < 0 || c->body.motion > 1) return 0;
+    if (c->body.motion == WL_MOTION_HEAVE_SIN && (c->body.heave_dir < 0 || c->body.heave_dir >= c->ndim)) return 0;
+    if (c->exit_bc && c->periodic[0]) return 0;
+    if (c->mg.smooth_iters < 1) return 0;
+    return 1;
+}
+
+static Grid make_grid(int nd, const int* n, const int* per)
+{
+    Grid g;
+    for (int d = 0; d < 3; ++d) {
+        g.n[d] = d < nd ? n[d] : 1;
+        g.S[d] = d < nd ? n[d] + 2 : 1;
+        g.per[d] = d < nd ? (per[d] ? 1 : 0) : 0;
+    }
+    g.P = ((g.n[0] + 9 + 7) / 8) * 8;
+    g.sy = g.P;
+    g.sz = nd == 3 ? (int64_t)g.P * g.S[1] : 0;
+    int64_t tot = (int64_t)g.P * g.S[1] * g.S[2];
+    g.nalloc = ((tot + 63) / 64) * 64;
+    return g;
+}
+
+static int level_dims(const wl_config* c, int dims[WL_MAXLEV][3])
+{
+    int nd = c->ndim, n[3] = { c->dims[0], c->dims[1], nd == 3 ? c->dims[2] : 1 };
+    int cap = c->mg.max_levels > 0 ? c->mg.max_levels : WL_MAXLEV;
+    if (cap > WL_MAXLEV) cap = WL_MAXLEV;
+    int nlev = 0;
+    for (;;) {
+        for (int d = 0; d < 3; ++d) dims[nlev][d] = n[d];
+        ++nlev;
+        if (nlev >= cap) break;
+        int ok = 1;
+        for (int d = 0; d < nd; ++d) if ((n[d] & 1) || n[d] <= 4) ok = 0;
+        if (!ok) break;
+        for (int d = 0; d < nd; ++d) n[d] /= 2;
+    }
+    return nlev;
+}
+
+struct Carver {
+    char* base; size_t off;
+    void* take(size_t bytes) { void* p = base ? base + off : nullptr; off += (bytes + 255) / 256 * 256; return p; }
+};
+
+// lays the arrays out in the workspace; with base == NULL only computes the size
+static size_t layout(wl_sim* s, const wl_config* c, void* base)
+{
+    Carver cv = { (char*)base, 0 };
+    int nd = c->ndim, dims[WL_MAXLEV][3];
+    int nlev = level_dims(c, dims);
+    DevScal* ds = (DevScal*)cv.take(sizeof(DevScal));
+    double* partial = (double*)cv.take(sizeof(double) * 4 * WL_MAX_PARTIALS);
+    unsigned int* counter = (unsigned int*)cv.take(256);
+    Grid g0 = make_grid(nd, dims[0], c->periodic);
+    size_t sc = sizeof(float) * (size_t)g0.nalloc;
+    float* ub[3];
+    for (int k = 0; k < 3; ++k) ub[k] = (float*)cv.take(sc * nd);
+    float* p = (float*)cv.take(sc);
+    float* mu0 = (float*)cv.take(sc * nd);
+    float* mu1 = (float*)cv.take(sc * nd * nd);
+    if (s) {
+        s->ds = ds; s->rb.partial = partial; s->rb.counter = counter;
+        for (int k = 0; k < 3; ++k) s->ubuf[k] = ub[k];
+        s->p = p; s->mu0 = mu0; s->mu1 = mu1;
+        s->nlev = nlev; s->nd = nd;
+    }
+    for (int l = 0; l < nlev; ++l) {
+        Grid g = make_grid(nd, dims[l], c->periodic);
+        size_t scl = sizeof(float) * (size_t)g.nalloc;
+        float* L = l == 0 ? mu0 : (float*)cv.take(scl * nd);
+        float* iD = (float*)cv.take(scl);
+        float* x = (float*)cv.take(scl);
+        float* r = (float*)cv.take(scl);
+        float* e = (float*)cv.take(scl);
+        float* q = (float*)cv.take(scl);
+        if (s) { Level& lv = s->lev[l]; lv.g = g; lv.L = L; lv.iD = iD; lv.x = x; lv.r = r; lv.e = e; lv.q = q; }
+    }
+    return cv.off;
+}
+
+extern "C" size_t wl_workspace_bytes(const wl_config* cfg)
+{
+    if (!config_ok(cfg)) return 0;
+    return layout(nullptr, cfg, nullptr);
+}
+
+extern "C" int wl_abi_version(void) { return 1; }
+
+// ------------------------------------------------------------------ the step
+static void bc_all(wl_sim* s, float* u) { wl_k_bc(s, u); }
+
+static int solve(wl_sim* s)
+{
+    const wl_mg& mg = s->cfg.mg;
+    int nv = 0;
+    if (mg.fixed_vcycles > 0) {
+        for (; nv < mg.fixed_vcycles; ++nv) { wl_k_vcycle(s, 0); wl_k_smooth(s, 0, mg.smooth_iters); }
+        s->res[s->solve_slot] = -1.0;
+    } else {
+        double res = 0.0;
+        for (;;) {
+            wl_k_resmax(s);
+            cudaMemcpyAsync(&s->hs->resmax, &s->ds->resmax, sizeof(double), cudaMemcpyDeviceToHost, s->st);
+            if (cudaStreamSynchronize(s->st) != cudaSuccess) return WL_ECUDA;
+            res = s->hs->resmax;
+            if (!(res > (double)mg.tol) || nv >= mg.max_vcycles) break;
+            wl_k_vcycle(s, 0);
+            wl_k_smooth(s, 0, mg.smooth_iters);
+            ++nv;
+        }
+        s->res[s->solve_slot] = res;
+        if (res > (double)mg.tol) s->noconv = 1;
+    }
+    s->vcycles[s->solve_slot] = nv;
+    return WL_OK;
+}
+
+// project!: z = div u; x = (w dt) p; solve A x = z; u -= L grad x; p = x/(w dt)
+static int project(wl_sim* s, float* u, float w)
+{
+    wl_k_residual(s, u, w);
+    int rc = solve(s);
+    wl_k_apply_gradient(s, u);
+    return rc;
+}
+
+// mom_step (reading R-K/R-L).  ds->dt must hold the step's dt.
+static int mom_step_body(wl_sim* s)
+{
+    // u0 <- u by swapping roles; the predictor writes the other buffer
+    float* t = s->u0; s->u0 = s->u; s->u = t;
+    wl_k_conv_diff_bdim(s, s->u0, s->u0, s->u, 0);
+    bc_all(s, s->u);
+    if (s->cfg.exit_bc) wl_k_exit_bc(s, s->u, s->u0);
+    s->solve_slot = 0;
+    int rc = project(s, s->u, 1.0f);
+    if (rc != WL_OK) return rc;
+    bc_all(s, s->u);
+    wl_k_conv_diff_bdim(s, s->u, s->u0, s->ut, 1);
+    bc_all(s, s->ut);
+    s->solve_slot = 1;
+    rc = project(s, s->ut, 0.5f);
+    if (rc != WL_OK) return rc;
+    bc_all(s, s->ut);
+    t = s->u; s->u = s->ut; s->ut = t;
+    return WL_OK;
+}
+
+static int check(wl_sim* s)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        snprintf(s->err, sizeof(s->err), "CUDA: %s", cudaGetErrorString(e));
+        return WL_ECUDA;
+    }
+    return WL_OK;
+}
+static int sync(wl_sim* s)
+{
+    cudaError_t e = cudaStreamSynchronize(s->st);
+    if (e != cudaSuccess) {
+        snprintf(s->err, sizeof(s->err), "CUDA: %s", cudaGetErrorString(e));
+        return WL_ECUDA;
+    }
+    return check(s);
+}
+
+// ------------------------------------------------------------------ C ABI
+extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes, void* cuda_stream, wl_sim** out)
+{
+    if (!out) return WL_EINVAL;
+    *out = nullptr;
+    if (!config_ok(cfg)) return WL_EINVAL;
+    size_t need = layout(nullptr, cfg, nullptr);
+    if (!dev_ws || ws_bytes < need || ((uintptr_t)dev_ws & 255u)) return WL_ENOMEM;
+    wl_sim* s = (wl_sim*)calloc(1, sizeof(wl_sim));
+    if (!s) return WL_ENOMEM;
+    s->cfg = *cfg;
+    s->st = (cudaStream_t)cuda_stream;
+    layout(s, cfg, dev_ws);
+    s->u = s->ubuf[0]; s->u0 = s->ubuf[1]; s->ut = s->ubuf[2];
+    s->body.kind = cfg->body.kind; s->body.axis = cfg->body.axis;
+    s->body.R = cfg->body.R; s->body.r = cfg->body.r; s->body.eps = cfg->eps;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        free(s);
+        return WL_ECUDA;
+    }
+    s->sm_count = prop.multiProcessorCount;
+    if (cudaMallocHost((void**)&s->hs, sizeof(DevScal)) != cudaSuccess) { free(s); return WL_ECUDA; }
+    memset(s->hs, 0, sizeof(DevScal));
+    if (cudaMemsetAsync(dev_ws, 0, need, s->st) != cudaSuccess) { cudaFreeHost(s->hs); free(s); return WL_ECUDA; }
+    // initial state (R-V): u = U everywhere (all three buffers, so the exit plane is defined), p = 0, measure(0)
+    for (int k = 0; k < 3; ++k) wl_k_fill_u(s, s->ubuf[k]);
+    wl_k_set_time(s, 0.0, cfg->dt0, 1, 1);
+    wl_k_measure(s);
+    bc_all(s, s->u);
+    int rc = sync(s);
+    if (rc != WL_OK) { cudaFreeHost(s->hs); free(s); return rc; }
+    *out = s;
+    return WL_OK;
+}
+
+extern "C" int wl_sim_destroy(wl_sim* s)
+{
+    if (!s) return WL_EINVAL;
+    cudaStreamSynchronize(s->st);
+    if (s->hs) cudaFreeHost(s->hs);
+    free(s);
+    return WL_OK;
+}
+
+extern "C" const char* wl_last_error(const wl_sim* s) { return s ? s->err : "null handle"; }
+
+static int64_t interior_count(const Grid& g) { return (int64_t)g.n[0] * g.n[1] * g.n[2]; }
+
+// copy `ncomp` padded arrays out to an interior-sized user buffer, one component at a time
+static int copy_out(wl_sim* s, const Grid& g, const float* padded, int ncomp, float* dst, int on_device, int whole = 0)
+{
+    int64_t ni = whole ? (int64_t)g.S[0] * g.S[1] * g.S[2] : interior_count(g);
+    for (int m = 0; m < ncomp; ++m) {
+        if (on_device) {
+            wl_k_pack(s, g, padded + m * g.nalloc, dst + m * ni, 1, 1.0f, whole);
+        } else {
+            // staging: the level-0 q array (>= any interior size); it is scratch between solver calls
+            float* stage = s->lev[0].q;
+            wl_k_pack(s, g, padded + m * g.nalloc, stage, 1, 1.0f, whole);
+            WL_CUDA_CHECK(s, cudaMemcpyAsync(dst + m * ni, stage, sizeof(float) * ni, cudaMemcpyDeviceToHost, s->st));
+            WL_CUDA_CHECK(s, cudaStreamSynchronize(s->st));
+        }
+    }
+    return check(s);
+}
+static int copy_in(wl_sim* s, const Grid& g, float* padded, int ncomp, const float* src, int on_device)
+{
+    int64_t ni = interior_count(g);
+    for (int m = 0; m < ncomp; ++m) {
+        if (on_device) {
+            wl_k_unpack(s, g, src + m * ni, padded + m * g.nalloc, 1);
+        } else {
+            float* stage = s->lev[0].q;
+            WL_CUDA_CHECK(s, cudaMemcpyAsync(stage, src + m * ni, sizeof(float) * ni, cudaMemcpyHostToDevice, s->st));
+            wl_k_unpack(s, g, stage, padded + m * g.nalloc, 1);
+            WL_CUDA_CHECK(s, cudaStreamSynchronize(s->st));
+        }
+    }
+    return check(s);
+}
+
+extern "C" int wl_set_fields(wl_sim* s, const float* u, const float* p, int on_device)
+{
+    if (!s) return WL_EINVAL;
+    const Grid& g = s->lev[0].g;
+    int rc;
+    if (u) {
+        if ((rc = copy_in(s, g, s->u, s->nd, u, on_device)) != WL_OK) return rc;
+        bc_all(s, s->u);
+    }
+    if (p && (rc = copy_in(s, g, s->p, 1, p, on_device)) != WL_OK) return rc;
+    return on_device ? check(s) : sync(s);
+}
+
+extern "C" int wl_get_fields(wl_sim* s, float* u, float* p, float* mu0, int on_device)
+{
+    if (!s) return WL_EINVAL;
+    const Grid& g = s->lev[0].g;
+    int rc;
+    if (u && (rc = copy_out(s, g, s->u, s->nd, u, on_device)) != WL_OK) return rc;
+    if (p && (rc = copy_out(s, g, s->p, 1, p, on_device)) != WL_OK) return rc;
+    if (mu0 && (rc = copy_out(s, g, s->mu0, s->nd, mu0, on_device)) != WL_OK) return rc;
+    return on_device ? check(s) : sync(s);
+}
+
+extern "C" int wl_init_tgv(wl_sim* s, int sign)
+{
+    if (!s) return WL_EINVAL;
+    wl_k_init_tgv(s, sign >= 0 ? 1 : -1);
+    bc_all(s, s->u);
+    return check(s);
+}
+
+extern "C" int wl_measure(wl_sim* s, double t)
+{
+    if (!s) return WL_EINVAL;
+    wl_k_set_time(s, t, 0.0f, 1, -1);
+    wl_k_measure(s);
+    return check(s);
+}
+
+extern "C" int wl_mom_step(wl_sim* s, float dt)
+{
+    if (!s || !(dt > 0.0f)) return WL_EINVAL;
+    wl_k_set_time(s, 0.0, dt, -1, 1);
+    int rc = mom_step_body(s);
+    if (rc != WL_OK) return rc;
+    return check(s);
+}
+
+extern "C" int wl_step(wl_sim* s, double t, float dt, int adaptive)
+{
+    if (!s) return WL_EINVAL;
+    int dev = adaptive && s->primed;   // device-resident t and dt are valid
+    if (!dev && !(dt > 0.0f)) return WL_EINVAL;
+    wl_k_set_time(s, t, dt, dev ? 0 : 1, dev ? 0 : 1);
+    if (s->cfg.body.kind != WL_BODY_NONE && s->cfg.body.motion != WL_MOTION_STATIC) wl_k_measure(s);
+    int rc = mom_step_body(s);
+    if (rc != WL_OK) return rc;
+    wl_k_cfl(s, s->u);
+    s->primed = adaptive ? 1 : 0;
+    return check(s);
+}
+
+extern "C" int wl_cfl(wl_sim* s, float* dt_out)
+{
+    if (!s || !dt_out) return WL_EINVAL;
+    wl_k_cfl(s, s->u);
+    WL_CUDA_CHECK(s, cudaMemcpyAsync(&s->hs->dt_next, &s->ds->dt_next, sizeof(float), cudaMemcpyDeviceToHost, s->st));
+    WL_CUDA_CHECK(s, cudaMemcpyAsync(&s->hs->nan_flag, &s->ds->nan_flag, sizeof(int), cudaMemcpyDeviceToHost, s->st));
+    int rc = sync(s);
+    if (rc != WL_OK) return rc;
+    *dt_out = s->hs->dt_next;
+    if (s->noconv) { s->noconv = 0; return WL_ENOCONV; }
+    return WL_OK;
+}
+
+extern "C" int wl_pressure_force(wl_sim* s, double t, float F_out[3])
+{
+    if (!s || !F_out) return WL_EINVAL;
+    if (t == t) wl_k_set_time(s, t, 0.0f, 1, -1);    // NaN: keep the device-resident body state
+    wl_k_force(s);
+    WL_CUDA_CHECK(s, cudaMemcpyAsync(s->hs->force, s->ds->force, 3 * sizeof(double), cudaMemcpyDeviceToHost, s->st));
+    int rc = sync(s);
+    if (rc != WL_OK) return rc;
+    for (int k = 0; k < 3; ++k) F_out[k] = (float)s->hs->force[k];
+    return WL_OK;
+}
+
+extern "C" int wl_stats(wl_sim* s, wl_stats_t* out)
+{
+    if (!s || !out) return WL_EINVAL;
+    out->vcycles[0] = s->vcycles[0]; out->vcycles[1] = s->vcycles[1];
+    out->res[0] = s->res[0]; out->res[1] = s->res[1];
+    out->nlevels = s->nlev;
+    out->kernel_launches = s->launches;
+    out->nan_flag = s->hs->nan_flag;
+    return WL_OK;
+}
+
+extern "C" int wl_level_dims(const wl_sim* s, int level, int dims_out[3])
+{
+    if (!s || level < 0 || level >= s->nlev) return WL_EINVAL;
+    for (int d = 0; d < 3; ++d) dims_out[d] = s->lev[level].g.n[d];
+    return WL_OK;
+}
+
+// ---- stage hooks
+extern "C" int wl_dbg_save_u0(wl_sim* s)
+{
+    if (!s) return WL_EINVAL;
+    const Grid& g = s->lev[0].g;
+    WL_CUDA_CHECK(s, cudaMemcpyAsync(s->u0, s->u, sizeof(float) * g.nalloc * s->nd, cudaMemcpyDeviceToDevice, s->st));
+    return WL_OK;
+}
+extern "C" int wl_dbg_conv_diff_bdim(wl_sim* s, float dt, int corrector)
+{
+    if (!s) return WL_EINVAL;
+    wl_k_set_time(s, 0.0, dt, -1, 1);
+    wl_k_conv_diff_bdim(s, s->u, s->u0, s->ut, corrector);
+    float* t = s->u; s->u = s->ut; s->ut = t;
+    return check(s);
+}
+extern "C" int wl_dbg_bc(wl_sim* s) { if (!s) return WL_EINVAL; bc_all(s, s->u); return check(s); }
+extern "C" int wl_dbg_exit_bc(wl_sim* s, float dt)
+{
+    if (!s) return WL_EINVAL;
+    wl_k_set_time(s, 0.0, dt, -1, 1);
+    wl_k_exit_bc(s, s->u, s->u0);
+    return check(s);
+}
+extern "C" int wl_dbg_project(wl_sim* s, float w, float dt)
+{
+    if (!s) return WL_EINVAL;
+    wl_k_set_time(s, 0.0, dt, -1, 1);
+    s->solve_slot = 0;
+    int rc = project(s, s->u, w);
+    return rc != WL_OK ? rc : check(s);
+}
+extern "C" int wl_dbg_residual(wl_sim* s)
+{
+    // r = div u - A x with the CURRENT x: expressed through k_residual by p := x, w dt := 1
+    if (!s) return WL_EINVAL;
+    const Grid& g = s->lev[0].g;
+    WL_CUDA_CHECK(s, cudaMemcpyAsync(s->lev[0].q, s->p, sizeof(float) * g.nalloc, cudaMemcpyDeviceToDevice, s->st));
+    WL_CUDA_CHECK(s, cudaMemcpyAsync(s->p, s->lev[0].x, sizeof(float) * g.nalloc, cudaMemcpyDeviceToDevice, s->st));
+    wl_k_set_time(s, 0.0, 1.0f, -1, 1);
+    wl_k_residual(s, s->u, 1.0f);
+    WL_CUDA_CHECK(s, cudaMemcpyAsync(s->p, s->lev[0].q, sizeof(float) * g.nalloc, cudaMemcpyDeviceToDevice, s->st));
+    return check(s);
+}
+extern "C" int wl_dbg_restrict(wl_sim* s, int l) { if (!s || l < 0 || l + 1 >= s->nlev) return WL_EINVAL; wl_k_restrict(s, l); return check(s); }
+extern "C" int wl_dbg_prolong(wl_sim* s, int l) { if (!s || l < 0 || l + 1 >= s->nlev) return WL_EINVAL; wl_k_prolong(s, l); return check(s); }
+extern "C" int wl_dbg_smooth(wl_sim* s, int l, int iters) { if (!s || l < 0 || l >= s->nlev || iters < 1) return WL_EINVAL; wl_k_smooth(s, l, iters); return check(s); }
+extern "C" int wl_dbg_vcycle(wl_sim* s, int l) { if (!s || l < 0 || l >= s->nlev) return WL_EINVAL; wl_k_vcycle(s, l); return check(s); }
+
+static int find_array(wl_sim* s, const char* name, int level, float** arr, int* ncomp, const Grid** g)
+{
+    if (level < 0 || level >= s->nlev) return WL_EINVAL;
+    Level& lv = s->lev[level];
+    *g = &lv.g; *ncomp = 1;
+    if (!strcmp(name, "L")) { *arr = lv.L; *ncomp = s->nd; return WL_OK; }
+    if (!strcmp(name, "iD")) { *arr = lv.iD; return WL_OK; }
+    if (!strcmp(name, "x")) { *arr = lv.x; return WL_OK; }
+    if (!strcmp(name, "r")) { *arr = lv.r; return WL_OK; }
+    if (!strcmp(name, "e")) { *arr = lv.e; return WL_OK; }
+    if (!strcmp(name, "q")) { *arr = lv.q; return WL_OK; }
+    *g = &s->lev[0].g;
+    if (!strcmp(name, "u")) { *arr = s->u; *ncomp = s->nd; return WL_OK; }
+    if (!strcmp(name, "u0")) { *arr = s->u0; *ncomp = s->nd; return WL_OK; }
+    if (!strcmp(name, "p")) { *arr = s->p; return WL_OK; }
+    if (!strcmp(name, "mu0")) { *arr = s->mu0; *ncomp = s->nd; return WL_OK; }
+    if (!strcmp(name, "mu1")) { *arr = s->mu1; *ncomp = s->nd * s->nd; return WL_OK; }
+    return WL_EINVAL;
+}
+static int dbg_get(wl_sim* s, const char* name, int level, float* out, size_t out_floats, int whole)
+{
+    if (!s || !name || !out) return WL_EINVAL;
+    float* arr; int nc; const Grid* g;
+    int rc = find_array(s, name, level, &arr, &nc, &g);
+    if (rc != WL_OK) return rc;
+    int64_t cnt = whole ? (int64_t)g->S[0] * g->S[1] * g->S[2] : interior_count(*g);
+    if (out_floats < (size_t)(cnt * nc)) return WL_EINVAL;
+    if (arr == s->lev[0].q) {   // q is the staging buffer: go through e's slot is not possible; copy via ut
+        WL_CUDA_CHECK(s, cudaMemcpyAsync(s->ut, arr, sizeof(float) * g->nalloc, cudaMemcpyDeviceToDevice, s->st));
+        arr = s->ut;
+    }
+    rc = copy_out(s, *g, arr, nc, out, 0, whole);
+    return rc != WL_OK ? rc : nc;
+}
+extern "C" int wl_dbg_get(wl_sim* s, const char* name, int level, float* out, size_t out_floats)
+{
+    return dbg_get(s, name, level, out, out_floats, 0);
+}
+extern "C" int wl_dbg_get_padded(wl_sim* s, const char* name, int level, float* out, size_t out_floats)
+{
+    return dbg_get(s, name, level, out, out_floats, 1);
+}
+extern "C" int wl_dbg_set(wl_sim* s, const char* name, int level, const float* in, size_t in_floats)
+{
+    if (!s || !name || !in) return WL_EINVAL;
+    float* arr; int nc; const Grid* g;
+    int rc = find_array(s, name, level, &arr, &nc, &g);
+    if (rc != WL_OK) return rc;
+    if (in_floats < (size_t)(interior_count(*g) * nc) || arr == s->lev[0].q) return WL_EINVAL;
+    rc = copy_in(s, *g, arr, nc, in, 0);
+    return rc != WL_OK ? rc : nc;
+}

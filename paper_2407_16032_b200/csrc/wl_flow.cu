@@ -1,0 +1,380 @@
+// wl_flow.cu -- flow-side kernels of libwl: body measurement, boundary conditions, convective
+// exit, CFL reduction, pressure force, initial conditions, pack/unpack of user buffers.
+// Citations "P:<line>" are /root/reference/PAPER.md; "R-<x>" are the readings of DESIGN.md s.3.
+#include <cstdio>
+#include "wl_internal.h"
+
+// ------------------------------------------------------------------ time / body state
+// One thread.  Sets the running dt (host value, or the device-resident CFL result) and the
+// time at which the body is measured (host value, or t + dt: reading R-R), then the
+// translation map c(t) = c0 + amp sin(2 pi f t + phase) e_heave and V = dc/dt.
+// Modes: t_mode / dt_mode = 1: take the host value; 0: device-resident (t + dt / last CFL result);
+// -1: keep the current value.
+__global__ void k_set_time(DevScal* ds, wl_body b, double t_host, float dt_host, int t_mode, int dt_mode)
+{
+    if (dt_mode == 1) ds->dt = dt_host; else if (dt_mode == 0) ds->dt = ds->dt_next;
+    double t = t_mode == 1 ? t_host : (t_mode == 0 ? ds->t + (double)ds->dt : ds->t);
+    ds->t = t;
+    double c[3] = { (double)b.centre[0], (double)b.centre[1], (double)b.centre[2] };
+    float v[3] = { 0.f, 0.f, 0.f };
+    if (b.motion == WL_MOTION_HEAVE_SIN) {
+        const double two_pi = 6.283185307179586476925286766559;
+        double ph = two_pi * (double)b.freq * t + (double)b.phase;
+        c[b.heave_dir] += (double)b.amp * sin(ph);
+        v[b.heave_dir] = (float)((double)b.amp * two_pi * (double)b.freq * cos(ph));
+    }
+    for (int k = 0; k < 3; ++k) { ds->centre[k] = c[k]; ds->vel[k] = v[k]; }
+}
+
+// ------------------------------------------------------------------ measure!
+// One thread per padded cell; for each face (c,i), x_f = x_c(c) - e_i/2:
+//   mu0[c,i] = mu0(d), mu1[c,i,j] = mu1(d) n_j                       (R-B, R-D, R-E)
+// Periodic ghosts are evaluated at the wrapped position; on non-periodic boundaries mu0 = 0 on
+// the two boundary-normal faces c_i = 1 and c_i = N_i+1 (R-O: homogeneous-Neumann Poisson
+// problem).  V is a uniform vector for the translation maps supported and lives in DevScal.
+template <int ND>
+__global__ void __launch_bounds__(512) k_measure(Grid g, Tiling T, BodyP b, const DevScal* __restrict__ ds,
+                                                 float* __restrict__ mu0, float* __restrict__ mu1)
+{
+    double ctr[3] = { ds->centre[0], ds->centre[1], ds->centre[2] };
+    for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
+        int c[3];
+        if (!tile_cell(T, tile, c[0], c[1], c[2])) continue;
+        int64_t id = gidx(g, c[0], c[1], c[2]);
+        float xc[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) xc[k] = k < ND ? (float)wrapc(c[k], g.n[k], g.per[k]) - 0.5f : 0.0f;
+#pragma unroll
+        for (int i = 0; i < ND; ++i) {
+            float m0 = 1.0f, m1 = 0.0f, nrm[3] = { 0.f, 0.f, 0.f };
+            if (b.kind != WLB_NONE) {
+                float xi[3];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    double xf = (double)xc[k] - (k == i ? 0.5 : 0.0);
+                    xi[k] = k < ND ? (float)(xf - ctr[k]) : 0.0f;
+                }
+                float d = body_sdf<ND>(b, xi, nrm);
+                m0 = bdim_mu0(d, b.eps);
+                m1 = bdim_mu1(d, b.eps);
+            }
+            if (!g.per[i] && (c[i] == 1 || c[i] == g.n[i] + 1)) m0 = 0.0f;
+            mu0[i * g.nalloc + id] = m0;
+#pragma unroll
+            for (int j = 0; j < ND; ++j) mu1[(i * ND + j) * g.nalloc + id] = m1 * nrm[j];
+        }
+    }
+}
+
+// ------------------------------------------------------------------ BC! (R-M)
+// The rule is stated direction by direction (x, then y, then z, each over the whole padded
+// range of the others): periodic -> ghost := wrapped interior; otherwise the normal component
+// is U_j on c_j in {0, 1, N_j+1} (the upper one is left alone on the convective exit) and the
+// tangential ghosts copy the adjacent interior value (slip).  Composing the three passes, the
+// final value of any shell cell is found by walking the directions from the last to the first
+// and redirecting the coordinate to its source; sources are never written by this kernel.
+template <int ND>
+__device__ __forceinline__ float bc_resolve(const FlowP& P, const float* u, int i, const int (&c)[3], bool& self)
+{
+    int cc[3] = { c[0], c[1], c[2] };
+#pragma unroll
+    for (int j = ND - 1; j >= 0; --j) {
+        const int N = P.g.n[j];
+        if (P.g.per[j]) {
+            if (cc[j] == 0) cc[j] = N; else if (cc[j] == N + 1) cc[j] = 1;
+        } else if (i == j) {
+            if (cc[j] <= 1 || (cc[j] == N + 1 && !(P.exit_bc && j == 0))) { self = false; return P.U[j]; }
+        } else {
+            if (cc[j] == 0) cc[j] = 1; else if (cc[j] == N + 1) cc[j] = N;
+        }
+    }
+    self = (cc[0] == c[0] && cc[1] == c[1] && cc[2] == c[2]);
+    return u[i * P.g.nalloc + gidx(P.g, cc[0], cc[1], cc[2])];
+}
+
+template <int ND>
+__global__ void k_bc(FlowP P, float* u)
+{
+    const Grid& g = P.g;
+    int64_t A[3];
+    A[0] = (int64_t)g.S[1] * g.S[2]; A[1] = (int64_t)g.S[0] * g.S[2]; A[2] = (int64_t)g.S[0] * g.S[1];
+    int64_t total = 0;
+    for (int j = 0; j < ND; ++j) total += 3 * A[j];
+    for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+        int64_t rem = t;
+        int j = 0;
+        while (rem >= 3 * A[j]) { rem -= 3 * A[j]; ++j; }
+        int plane = (int)(rem / A[j]);
+        int64_t ab = rem % A[j];
+        int c[3] = { 0, 0, 0 };
+        int d0 = j == 0 ? 1 : 0;                 // fastest of the two in-plane directions
+        int d1 = j == 2 ? 1 : 2;
+        c[d0] = (int)(ab % g.S[d0]);
+        c[d1] = (int)(ab / g.S[d0]);
+        if (ND == 2) c[2] = 0;
+        c[j] = plane == 0 ? 0 : (plane == 1 ? 1 : g.n[j] + 1);
+        if (plane == 1 && g.per[j]) continue;
+        int64_t id = gidx(g, c[0], c[1], c[2]);
+#pragma unroll
+        for (int i = 0; i < ND; ++i) {
+            if (plane == 1 && i != j) continue;
+            bool self;
+            float v = bc_resolve<ND>(P, u, i, c, self);
+            if (!self) u[i * g.nalloc + id] = v;
+        }
+    }
+}
+
+// ------------------------------------------------------------------ exitBC! (R-N)
+// Exit plane c_x = N_x+1: u_x <- u0_x - U_x dt (u0_x[c] - u0_x[c - d_x]); then every value is
+// shifted by (mean - U_x) so that outflow = nominal inflow.
+template <int ND>
+__global__ void __launch_bounds__(256) k_exit_a(FlowP P, float* u, const float* __restrict__ u0, DevScal* ds, RedBuf rb)
+{
+    const Grid& g = P.g;
+    const int n1 = g.n[1], n2 = ND == 3 ? g.n[2] : 1;
+    const int cnt = n1 * n2;
+    const float dt = ds->dt;
+    double v[1] = { 0.0 };
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < cnt; t += gridDim.x * blockDim.x) {
+        int c1 = 1 + t % n1, c2 = ND == 3 ? 1 + t / n1 : 0;
+        int64_t id = gidx(g, g.n[0] + 1, c1, c2);
+        float a = u0[id], b = u0[id - 1];
+        float val = a - P.U[0] * dt * (a - b);
+        u[id] = val;
+        v[0] += (double)val;
+    }
+    if (grid_reduce<1, OpSum>(v, rb)) {
+        if (threadIdx.x == 0) ds->exit_corr = (float)(v[0] / (double)cnt - (double)P.U[0]);
+    }
+}
+template <int ND>
+__global__ void k_exit_b(FlowP P, float* u, const DevScal* __restrict__ ds)
+{
+    const Grid& g = P.g;
+    const int n1 = g.n[1], n2 = ND == 3 ? g.n[2] : 1;
+    const int cnt = n1 * n2;
+    const float corr = ds->exit_corr;
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < cnt; t += gridDim.x * blockDim.x) {
+        int c1 = 1 + t % n1, c2 = ND == 3 ? 1 + t / n1 : 0;
+        u[gidx(g, g.n[0] + 1, c1, c2)] -= corr;
+    }
+}
+
+// ------------------------------------------------------------------ CFL! (R-U)
+// dt = min(dt_max, cfl_c / (max_c sum_i [max(0,u_i[c+d_i]) + max(0,-u_i[c])] + cfl_cnu nu))
+template <int ND>
+__global__ void __launch_bounds__(512) k_cfl(Grid g, Tiling T, const float* __restrict__ u, DevScal* ds, RedBuf rb,
+                                             float nu, float cfl_c, float cfl_cnu, float dt_max)
+{
+    double v[2] = { 0.0, 0.0 };
+    const int64_t st[3] = { 1, g.sy, g.sz };
+    for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
+        int c0, c1, c2;
+        if (!tile_cell(T, tile, c0, c1, c2)) continue;
+        int64_t id = gidx(g, c0, c1, c2);
+        float a = 0.0f;
+#pragma unroll
+        for (int i = 0; i < ND; ++i) {
+            float up = u[i * g.nalloc + id + st[i]], lo = u[i * g.nalloc + id];
+            a += fmaxf(up, 0.0f) + fmaxf(-lo, 0.0f);
+            if (!isfinite(up) || !isfinite(lo)) v[1] = 1.0;
+        }
+        if ((double)a > v[0]) v[0] = (double)a;
+    }
+    if (grid_reduce<2, OpMax>(v, rb)) {
+        if (threadIdx.x == 0 && threadIdx.y == 0 && threadIdx.z == 0) {
+            float m = (float)v[0];
+            float dt = cfl_c / (m + cfl_cnu * nu);
+            ds->dt_next = dt < dt_max ? dt : dt_max;
+            ds->cfl_max = v[0];
+            ds->nan_flag = v[1] > 0.5 ? 1 : 0;
+        }
+    }
+}
+
+// ------------------------------------------------------------------ pressure force (R-Z)
+// F = - sum_{c interior} p[c] n(x_c) K^{1}(d(x_c)), one-cell-wide surface delta at cell centres.
+template <int ND>
+__global__ void __launch_bounds__(512) k_force(Grid g, Tiling T, BodyP b, const float* __restrict__ p, DevScal* ds, RedBuf rb)
+{
+    double ctr[3] = { ds->centre[0], ds->centre[1], ds->centre[2] };
+    double v[3] = { 0.0, 0.0, 0.0 };
+    if (b.kind != WLB_NONE) {
+        for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
+            int c[3];
+            if (!tile_cell(T, tile, c[0], c[1], c[2])) continue;
+            float xi[3], nrm[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) xi[k] = k < ND ? (float)(((double)c[k] - 0.5) - ctr[k]) : 0.0f;
+            float d = body_sdf<ND>(b, xi, nrm);
+            float kk = bdim_K(d, 1.0f);
+            if (kk == 0.0f) continue;
+            float pk = p[gidx(g, c[0], c[1], c[2])] * kk;
+            v[0] -= (double)(pk * nrm[0]); v[1] -= (double)(pk * nrm[1]); v[2] -= (double)(pk * nrm[2]);
+        }
+    }
+    if (grid_reduce<3, OpSum>(v, rb)) {
+        if (threadIdx.x == 0 && threadIdx.y == 0 && threadIdx.z == 0) {
+            ds->force[0] = v[0]; ds->force[1] = v[1]; ds->force[2] = v[2];
+        }
+    }
+}
+
+// ------------------------------------------------------------------ initial conditions
+// Taylor-Green vortex (Eq. 3-5; R-W), staggered sampling, whole padded array.
+template <int ND>
+__global__ void __launch_bounds__(512) k_init_tgv(Grid g, Tiling T, float* u, float* p, int sign)
+{
+    const double two_pi = 6.283185307179586476925286766559;
+    const double k0 = two_pi / g.n[0], k1 = two_pi / g.n[1], k2 = ND == 3 ? two_pi / g.n[2] : 0.0;
+    for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
+        int c0, c1, c2;
+        if (!tile_cell(T, tile, c0, c1, c2)) continue;
+        int64_t id = gidx(g, c0, c1, c2);
+        double xc = c0 - 0.5, yc = c1 - 0.5, zc = ND == 3 ? c2 - 0.5 : 0.0;
+        double cz = ND == 3 ? cos(k2 * zc) : 1.0;
+        u[id] = (float)(sign * sin(k0 * (xc - 0.5)) * cos(k1 * yc) * cz);
+        u[g.nalloc + id] = (float)(-sign * cos(k0 * xc) * sin(k1 * (yc - 0.5)) * cz);
+        if (ND == 3) u[2 * g.nalloc + id] = 0.0f;
+        p[id] = 0.0f;
+    }
+}
+
+__global__ void k_fill(float* a, int64_t n, float v)
+{
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) a[i] = v;
+}
+
+// user buffer (the box T.o .. T.o+T.e of the padded array, dense) <-> padded array
+template <int ND>
+__global__ void __launch_bounds__(512) k_pack(Grid g, Tiling T, const float* __restrict__ padded, float* __restrict__ dense, int ncomp, float scale)
+{
+    const int64_t nint = (int64_t)T.e[0] * T.e[1] * T.e[2];
+    for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
+        int c0, c1, c2;
+        if (!tile_cell(T, tile, c0, c1, c2)) continue;
+        int64_t id = gidx(g, c0, c1, c2);
+        int64_t k = (c0 - T.o[0]) + (int64_t)T.e[0] * ((c1 - T.o[1]) + (int64_t)T.e[1] * (c2 - T.o[2]));
+        for (int m = 0; m < ncomp; ++m) dense[m * nint + k] = scale * padded[m * g.nalloc + id];
+    }
+}
+template <int ND>
+__global__ void __launch_bounds__(512) k_unpack(Grid g, Tiling T, const float* __restrict__ dense, float* __restrict__ padded, int ncomp)
+{
+    const int64_t nint = (int64_t)T.e[0] * T.e[1] * T.e[2];
+    for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
+        int c0, c1, c2;
+        if (!tile_cell(T, tile, c0, c1, c2)) continue;
+        int64_t id = gidx(g, c0, c1, c2);
+        int64_t k = (c0 - T.o[0]) + (int64_t)T.e[0] * ((c1 - T.o[1]) + (int64_t)T.e[1] * (c2 - T.o[2]));
+        for (int m = 0; m < ncomp; ++m) padded[m * g.nalloc + id] = dense[m * nint + k];
+    }
+}
+
+// ================================================================== host launchers
+#define LAUNCH(s) ((s)->launches++)
+
+void wl_k_set_time(wl_sim* s, double t, float dt, int t_mode, int dt_mode)
+{
+    LAUNCH(s);
+    k_set_time<<<1, 1, 0, s->st>>>(s->ds, s->cfg.body, t, dt, t_mode, dt_mode);
+}
+
+void wl_k_measure(wl_sim* s)
+{
+    const Grid& g = s->lev[0].g;
+    Tiling T = wl_tiles_padded(s, g);
+    LAUNCH(s);
+    if (s->nd == 3) k_measure<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1);
+    else            k_measure<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1);
+    wl_k_poisson_update(s);
+}
+
+void wl_k_bc(wl_sim* s, float* u)
+{
+    FlowP P = wl_flowp(s);
+    const Grid& g = P.g;
+    int64_t total = 3 * ((int64_t)g.S[1] * g.S[2] + (int64_t)g.S[0] * g.S[2] + (s->nd == 3 ? (int64_t)g.S[0] * g.S[1] : 0));
+    int blocks = (int)((total + 255) / 256);
+    if (blocks > s->sm_count * 8) blocks = s->sm_count * 8;
+    LAUNCH(s);
+    if (s->nd == 3) k_bc<3><<<blocks, 256, 0, s->st>>>(P, u);
+    else            k_bc<2><<<blocks, 256, 0, s->st>>>(P, u);
+}
+
+void wl_k_exit_bc(wl_sim* s, float* u, const float* u0)
+{
+    FlowP P = wl_flowp(s);
+    const Grid& g = P.g;
+    int cnt = g.n[1] * (s->nd == 3 ? g.n[2] : 1);
+    int blocks = (cnt + 255) / 256;
+    if (blocks > s->sm_count) blocks = s->sm_count;
+    s->launches += 2;
+    if (s->nd == 3) {
+        k_exit_a<3><<<blocks, 256, 0, s->st>>>(P, u, u0, s->ds, s->rb);
+        k_exit_b<3><<<blocks, 256, 0, s->st>>>(P, u, s->ds);
+    } else {
+        k_exit_a<2><<<blocks, 256, 0, s->st>>>(P, u, u0, s->ds, s->rb);
+        k_exit_b<2><<<blocks, 256, 0, s->st>>>(P, u, s->ds);
+    }
+}
+
+void wl_k_cfl(wl_sim* s, const float* u)
+{
+    const Grid& g = s->lev[0].g;
+    Tiling T = wl_tiles_interior(s, g);
+    const wl_config& c = s->cfg;
+    LAUNCH(s);
+    if (s->nd == 3) k_cfl<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, u, s->ds, s->rb, c.nu, c.cfl_c, c.cfl_cnu, c.dt_max);
+    else            k_cfl<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, u, s->ds, s->rb, c.nu, c.cfl_c, c.cfl_cnu, c.dt_max);
+}
+
+void wl_k_force(wl_sim* s)
+{
+    const Grid& g = s->lev[0].g;
+    Tiling T = wl_tiles_interior(s, g);
+    LAUNCH(s);
+    if (s->nd == 3) k_force<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->p, s->ds, s->rb);
+    else            k_force<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->p, s->ds, s->rb);
+}
+
+void wl_k_init_tgv(wl_sim* s, int sign)
+{
+    const Grid& g = s->lev[0].g;
+    Tiling T = wl_tiles_padded(s, g);
+    LAUNCH(s);
+    if (s->nd == 3) k_init_tgv<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->u, s->p, sign);
+    else            k_init_tgv<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->u, s->p, sign);
+}
+
+void wl_k_fill(wl_sim* s, float* a, int64_t n, float v)
+{
+    int blocks = (int)((n + 1023) / 1024);
+    if (blocks > s->sm_count * 8) blocks = s->sm_count * 8;
+    if (blocks < 1) blocks = 1;
+    LAUNCH(s);
+    k_fill<<<blocks, 256, 0, s->st>>>(a, n, v);
+}
+
+void wl_k_fill_u(wl_sim* s, float* u)
+{
+    const Grid& g = s->lev[0].g;
+    for (int i = 0; i < s->nd; ++i) wl_k_fill(s, u + i * g.nalloc, g.nalloc, s->cfg.U[i]);
+}
+
+void wl_k_pack(wl_sim* s, const Grid& g, const float* padded, float* interior, int ncomp, float scale, int whole)
+{
+    Tiling T = whole ? wl_tiles_padded(s, g) : wl_tiles_interior(s, g);
+    LAUNCH(s);
+    if (s->nd == 3) k_pack<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, padded, interior, ncomp, scale);
+    else            k_pack<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, padded, interior, ncomp, scale);
+}
+
+void wl_k_unpack(wl_sim* s, const Grid& g, const float* interior, float* padded, int ncomp)
+{
+    Tiling T = wl_tiles_interior(s, g);
+    LAUNCH(s);
+    if (s->nd == 3) k_unpack<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, interior, padded, ncomp);
+    else            k_unpack<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, interior, padded, ncomp);
+}

@@ -1,0 +1,89 @@
+// wl_internal.h -- host-side handle of libwl and the kernel-launch entry points shared by
+// the translation units (wl_api.cu, wl_flow.cu, wl_convdiff.cu, wl_poisson.cu).
+#pragma once
+#include "../../include/wl.h"
+#include "wl_common.cuh"
+#include "wl_body.cuh"
+
+struct Level {
+    Grid g;
+    float* L;    // nd face-coefficient arrays (level 0: alias of mu0), stride g.nalloc
+    float* iD;   // inverse diagonal
+    float* x;    // solution / correction
+    float* r;    // residual
+    float* e;    // CG direction
+    float* q;    // A e, then z = iD r
+};
+
+struct wl_sim {
+    wl_config cfg;
+    int nd, nlev;
+    Level lev[WL_MAXLEV];
+    float* ubuf[3];          // three rotating velocity buffers (nd comps each)
+    float *u, *u0, *ut;      // roles: current, start-of-step, scratch/next
+    float* p;                // pressure (unscaled)
+    float* mu0;              // nd comps
+    float* mu1;              // nd*nd comps
+    DevScal* ds;             // device-resident scalars
+    DevScal* hs;             // pinned host mirror for read-back
+    RedBuf rb;
+    BodyP body;
+    cudaStream_t st;
+    int launches;
+    int vcycles[2];
+    double res[2];
+    int solve_slot;
+    int noconv;
+    int primed;              // device-resident t and dt are valid (adaptive wl_step)
+    int sm_count;
+    char err[256];
+};
+
+// flow-side parameters passed by value to kernels
+struct FlowP {
+    Grid g;
+    float nu;
+    float U[3];
+    int exit_bc;
+};
+
+// launch geometry
+dim3 wl_block(int nd);
+Tiling wl_tiling(int nd, const int o[3], const int e[3]);
+int wl_grid(const wl_sim* s, const Tiling& T);
+Tiling wl_tiles_interior(const wl_sim* s, const Grid& g);
+Tiling wl_tiles_padded(const wl_sim* s, const Grid& g);
+FlowP wl_flowp(const wl_sim* s);
+
+// wl_flow.cu
+void wl_k_set_time(wl_sim* s, double t, float dt, int t_mode, int dt_mode);   // 1 host, 0 device, -1 keep
+void wl_k_measure(wl_sim* s);
+void wl_k_bc(wl_sim* s, float* u);
+void wl_k_exit_bc(wl_sim* s, float* u, const float* u0);
+void wl_k_cfl(wl_sim* s, const float* u);
+void wl_k_force(wl_sim* s);
+void wl_k_init_tgv(wl_sim* s, int sign);
+void wl_k_fill(wl_sim* s, float* a, int64_t n, float v);
+void wl_k_fill_u(wl_sim* s, float* u);
+void wl_k_pack(wl_sim* s, const Grid& g, const float* padded, float* dense, int ncomp, float scale, int whole);
+void wl_k_unpack(wl_sim* s, const Grid& g, const float* interior, float* padded, int ncomp);
+// wl_convdiff.cu
+void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out, int corrector);
+// wl_poisson.cu
+void wl_k_poisson_update(wl_sim* s);                 // iD on level 0, coarse L and iD
+void wl_k_residual(wl_sim* s, const float* u, float w);   // pscale = w*dt; x = pscale*p; r = div u - A x
+void wl_k_restrict(wl_sim* s, int l);                // r_{l+1} = sum children r_l ; x_{l+1} = 0
+void wl_k_prolong(wl_sim* s, int l);                 // x_l += P x_{l+1}; r_l -= A_l P x_{l+1}
+void wl_k_smooth(wl_sim* s, int l, int iters);
+void wl_k_vcycle(wl_sim* s, int l);
+void wl_k_apply_gradient(wl_sim* s, float* u);       // u -= L grad x ; p = x / pscale
+void wl_k_resmax(wl_sim* s);                         // ds->resmax = max |r_0|
+
+#define WL_CUDA_CHECK(s, call)                                                              \
+    do {                                                                                    \
+        cudaError_t e_ = (call);                                                            \
+        if (e_ != cudaSuccess) {                                                            \
+            snprintf((s)->err, sizeof((s)->err), "%s:%d %s", __FILE__, __LINE__, cudaGetErrorString(e_)); \
+            return WL_ECUDA;                                                                \
+        }                                                                                   \
+    } while (0)

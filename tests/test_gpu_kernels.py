@@ -1,0 +1,297 @@
+"""GPU parity, stage by stage: each libwl kernel applied once vs the fp64 oracle on the same
+seeded inputs (BASELINE.json north_star: relative L-infinity <= 2e-5).  All calls go through
+the C ABI (paper_2407_16032_b200.wl is argument marshalling only).
+
+Sizes span several 32x4x4 (3-D) / 32x16 (2-D) tiles and ragged tails: 32^3, 48x32x40, 64x48.
+"""
+import numpy as np
+import pytest
+
+import wl_inputs as wi
+
+pytestmark = pytest.mark.gpu
+
+TOL = 2e-5
+
+
+def _sims(cfg):
+    from oracle import wl_oracle as wo
+    from paper_2407_16032_b200 import wl
+    return wo.OracleSim(cfg), wl.Sim(cfg)
+
+
+def O(o, name, level=0, padded=False):
+    """Oracle array with the singleton z axis of 2-D cases dropped: (ncomp, [Nz,] Ny, Nx)."""
+    a = o.arr(name, level) if padded else o.interior(name, level)
+    return a[:, 0] if o.nd == 2 else a
+
+
+def relerr(a, b):
+    """max |a - b| / max |b| (b = oracle)."""
+    b = np.asarray(b, dtype=np.float64)
+    a = np.asarray(a, dtype=np.float64)
+    scale = max(np.abs(b).max(), 1e-30)
+    return np.abs(a - b).max() / scale
+
+
+def diag(iD):
+    """Poisson diagonal D from the stored 1/D (0 where the cell is decoupled)."""
+    iD = np.asarray(iD, dtype=np.float64)
+    return np.where(iD != 0, 1.0 / np.where(iD != 0, iD, 1.0), 0.0)
+
+
+def _body(kind, dims, moving=False):
+    nd = len(dims)
+    c = tuple(0.45 * n + 0.3 for n in dims)          # off-lattice centre
+    if kind == "none":
+        return {}
+    if kind == "sphere":
+        kw = dict(body_kind=wi.BODY_SPHERE, centre=c, R=0.22 * min(dims))
+    else:
+        kw = dict(body_kind=wi.BODY_TORUS, centre=c, R=0.25 * min(dims[1:]), r=0.09 * min(dims[1:]), axis=0)
+    if moving:
+        kw.update(motion=wi.MOTION_HEAVE_SIN, heave_dir=1, amp=0.1 * dims[1], freq=0.013, phase=0.3)
+    return kw
+
+
+CASES = [
+    # (dims, periodic, exit_bc, body, moving)
+    ((32, 32, 32), (1, 1, 1), 0, "none", False),
+    ((32, 32, 32), (0, 0, 0), 1, "sphere", False),
+    ((48, 32, 40), (0, 0, 0), 1, "torus", False),
+    ((48, 32, 40), (0, 1, 1), 1, "sphere", True),
+    ((48, 32, 40), (1, 1, 1), 0, "sphere", False),
+    ((64, 48), (1, 1), 0, "none", False),
+    ((64, 48), (0, 0), 1, "sphere", True),
+    ((64, 48), (0, 1), 0, "sphere", False),
+]
+
+
+def _cfg(case, **kw):
+    dims, per, ex, body, moving = case
+    base = dict(ndim=len(dims), dims=dims, periodic=per, exit_bc=ex, U=(1.0, 0.0, 0.0), nu=0.02)
+    base.update(_body(body, dims, moving))
+    base.update(kw)
+    return wi.make(**base)
+
+
+def _ids(c):
+    return "x".join(map(str, c[0])) + "-p" + "".join(map(str, c[1])) + ("-exit" if c[2] else "") + "-" + c[3] + ("-mov" if c[4] else "")
+
+
+def _load_state(o, g, dims, seed=wi.SEED, p_too=True):
+    u = wi.random_velocity(dims, seed=seed)
+    o.set_fields(u=u)
+    g.set_fields(u=np.ascontiguousarray(u, dtype=np.float32))
+    if p_too:
+        p = wi.random_scalar(dims, seed=seed + 5)
+        o.set_fields(p=p)
+        g.set_fields(p=np.ascontiguousarray(p, dtype=np.float32))
+
+
+@pytest.mark.parametrize("case", CASES, ids=_ids)
+def test_measure_and_poisson_coefficients(case):
+    """O2 + O7/O8 set-up: mu0, mu1 at every face, Poisson diagonal, coarse coefficients."""
+    cfg = _cfg(case)
+    o, g = _sims(cfg)
+    for t in (0.0, 7.3):
+        o.measure(t)
+        g.measure(t)
+        assert relerr(g.dbg_get("mu0", padded=True), O(o, "mu0", padded=True)) <= TOL
+        m1o = O(o, "mu1", padded=True)
+        m1g = g.dbg_get("mu1", padded=True)
+        assert np.abs(m1g - m1o).max() <= TOL * max(1.0, np.abs(m1o).max())
+        for l in range(o.nlevels):
+            assert g.level_dims(l) == tuple(O(o, "iD", l).shape[1:][::-1])
+            assert relerr(g.dbg_get("L", l), O(o, "L", l)) <= TOL
+            # iD = 1/D is ill-conditioned where the cell is nearly buried (D -> 0): compare D,
+            # and the decoupling pattern away from the threshold 2n*1e-6
+            Do, Dg = diag(O(o, "iD", l)), diag(g.dbg_get("iD", l))
+            thr = 2 * len(case[0]) * 1e-6
+            clear = (np.abs(Do) < 0.9 * thr) | (np.abs(Do) > 1.1 * thr)
+            assert np.array_equal((Dg != 0)[clear], (Do != 0)[clear])
+            both = (Dg != 0) & (Do != 0)
+            assert np.abs(Dg - Do)[both].max() <= TOL * np.abs(Do).max()
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("case", CASES, ids=_ids)
+def test_bc_fill(case):
+    """O5: every ghost cell (edges included) after the BC fill, whole padded array."""
+    cfg = _cfg(case)
+    o, g = _sims(cfg)
+    _load_state(o, g, case[0], p_too=False)          # set_fields applies the BC fill
+    uo, ug = O(o, "u", padded=True), g.dbg_get("u", padded=True)
+    assert ug.shape == uo.shape
+    assert np.abs(ug - uo).max() <= 1e-6
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("corrector", [0, 1])
+@pytest.mark.parametrize("case", CASES, ids=_ids)
+def test_conv_diff_bdim(case, corrector):
+    """O3 + O4 (+ O6 average): fused conv_diff / BDIM blend / Heun average, applied once."""
+    cfg = _cfg(case)
+    o, g = _sims(cfg)
+    dims = case[0]
+    dt = 0.31
+    if case[4]:
+        o.measure(3.0); g.measure(3.0)
+    # u0 = one field, u = another (the corrector reads both)
+    _load_state(o, g, dims, seed=wi.SEED, p_too=False)
+    o.arr("u0")[...] = o.arr("u")
+    g.dbg_save_u0()
+    if corrector:
+        _load_state(o, g, dims, seed=wi.SEED + 11, p_too=False)
+        o.conv_diff("u")
+    else:
+        o.conv_diff("u0")
+    o.bdim(dt, corrector)
+    g.dbg_conv_diff_bdim(dt, corrector)
+    assert relerr(g.dbg_get("u"), O(o, "u")) <= TOL
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("case", [c for c in CASES if c[2]], ids=_ids)
+def test_exit_bc(case):
+    """O6: convective exit plane and its mass-flux correction."""
+    cfg = _cfg(case)
+    o, g = _sims(cfg)
+    _load_state(o, g, case[0], p_too=False)
+    o.arr("u0")[...] = o.arr("u")
+    g.dbg_save_u0()
+    o.exit_bc(0.4)
+    g.dbg_exit_bc(0.4)
+    uo, ug = O(o, "u", padded=True)[0], g.dbg_get("u", padded=True)[0]
+    if len(case[0]) == 3:
+        a, b = ug[1:-1, 1:-1, -1], uo[1:-1, 1:-1, -1]
+    else:
+        a, b = ug[1:-1, -1], uo[1:-1, -1]
+    assert relerr(a, b) <= TOL
+    assert abs(a.astype(np.float64).mean() - 1.0) < 1e-6        # outflow = nominal inflow
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("case", CASES, ids=_ids)
+def test_residual_restrict_prolong(case):
+    """O7 residual r = div u - A x, O8 residual restriction and prolongation + increment."""
+    cfg = _cfg(case)
+    o, g = _sims(cfg)
+    dims = case[0]
+    _load_state(o, g, dims, p_too=False)
+    x0 = wi.random_scalar(dims, seed=77)
+    o.interior("x")[0][...] = x0
+    g.dbg_set("x", x0[None])
+    o.arr("sig")[...] = o.divergence()
+    o.residual()
+    g.dbg_residual()
+    assert relerr(g.dbg_get("r"), O(o, "r")) <= TOL
+    for l in range(o.nlevels - 1):
+        o.restrict(l)
+        g.dbg_restrict(l)
+        assert relerr(g.dbg_get("r", l + 1), O(o, "r", l + 1)) <= TOL
+    for l in range(o.nlevels - 2, -1, -1):
+        ld = g.level_dims(l + 1)
+        xc = wi.random_scalar(ld, seed=100 + l)
+        o.interior("x", l + 1)[0][...] = xc
+        g.dbg_set("x", xc[None], l + 1)
+        o.prolong_increment(l)
+        g.dbg_prolong(l)
+        assert relerr(g.dbg_get("x", l), O(o, "x", l)) <= TOL
+        assert relerr(g.dbg_get("r", l), O(o, "r", l)) <= TOL
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("iters", [1, 6])
+@pytest.mark.parametrize("case", CASES, ids=_ids)
+def test_pcg_smoother(case, iters):
+    """O8 smoother on every level: Jacobi-PCG, `iters` iterations from a seeded residual."""
+    cfg = _cfg(case)
+    o, g = _sims(cfg)
+    for l in range(o.nlevels):
+        ld = g.level_dims(l)
+        r0 = wi.random_scalar(ld, seed=300 + l)
+        r0 -= r0.mean()
+        # a physical residual scales with the Poisson diagonal in nearly buried cells (u -> V there);
+        # white noise times 1/D ~ 1e5 would only test the conditioning of 1/D
+        r0 = r0 * np.minimum(1.0, np.abs(diag(O(o, "iD", l)[0])))
+        o.interior("r", l)[0][...] = r0
+        o.arr("x", l)[...] = 0.0
+        g.dbg_set("r", r0[None], l)
+        g.dbg_set("x", np.zeros_like(r0)[None], l)
+        # same coefficients on both sides: 1/D from the measure/diagonal kernels is checked in
+        # test_measure_and_poisson_coefficients; here only the smoother's own arithmetic is
+        g.dbg_set("iD", O(o, "iD", l), l)
+        o.smooth(l, iters)
+        g.dbg_smooth(l, iters)
+        # CG amplifies rounding differences with the iteration count: 2e-5 for one iteration
+        # (a single kernel sequence), 1e-4 for six (the step-level tolerance)
+        tol = TOL if iters == 1 else 1e-4
+        assert relerr(g.dbg_get("x", l), O(o, "x", l)) <= tol
+        # r falls to round-off on the tiny coarse levels: measure it against the initial residual
+        assert np.abs(g.dbg_get("r", l) - O(o, "r", l)).max() <= tol * np.abs(r0).max()
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("case", CASES, ids=_ids)
+def test_vcycle_and_project(case):
+    """O8 V-cycle once; O7 project(w) with fixed V-cycles: velocity, pressure (mean-free), divergence."""
+    cfg = _cfg(case)
+    o, g = _sims(cfg)
+    dims = case[0]
+    _load_state(o, g, dims)
+    # the state a projection really sees: one predictor stage first (u -> V inside the body),
+    # BC fill, convective exit (which makes the Neumann problem compatible)
+    o.arr("u0")[...] = o.arr("u"); g.dbg_save_u0()
+    o.conv_diff("u0"); o.bdim(0.3, 0); g.dbg_conv_diff_bdim(0.3, 0)
+    o.bc(); g.dbg_bc()
+    if case[2]:
+        o.exit_bc(0.3); g.dbg_exit_bc(0.3)
+    for w in (1.0, 0.5):
+        o.project(w, 0.3)
+        g.dbg_project(w, 0.3)
+        o.bc(); g.dbg_bc()
+        assert relerr(g.dbg_get("u"), O(o, "u")) <= 1e-4
+        po, pg = O(o, "p")[0], g.dbg_get("p")[0].astype(np.float64)
+        # pressure is defined up to a constant, and is ill-conditioned in nearly buried cells
+        # (weak coupling: it does not affect u); compare it where the diagonal is O(1)
+        fluid = np.abs(diag(O(o, "iD")[0])) >= 0.1 * 2 * len(dims)
+        po = po - po[fluid].mean(); pg = pg - pg[fluid].mean()
+        assert np.abs(pg - po)[fluid].max() <= 1e-3 * max(np.abs(po[fluid]).max(), 1e-30)
+    o.close(); g.close()
+
+
+@pytest.mark.parametrize("case", CASES, ids=_ids)
+def test_cfl_and_force(case):
+    """O10 CFL reduction and O11 pressure-force integral."""
+    cfg = _cfg(case)
+    o, g = _sims(cfg)
+    _load_state(o, g, case[0])
+    assert g.cfl() == pytest.approx(o.cfl(), rel=TOL)
+    for t in (0.0, 11.0):
+        Fo, Fg = o.pressure_force(t), g.pressure_force(t)
+        scale = max(np.abs(Fo).max(), 1e-30)
+        if case[3] == "none":
+            assert np.all(Fg == 0.0) and np.all(Fo == 0.0)
+        else:
+            assert np.abs(Fg - Fo).max() <= 1e-4 * scale
+    o.close(); g.close()
+
+
+def test_init_tgv_matches_oracle_and_is_divergence_free():
+    for dims in ((64, 64), (32, 32, 32)):
+        cfg = wi.tgv2d(64) if len(dims) == 2 else wi.tgv3d(32)
+        o, g = _sims(cfg)
+        o.init_tgv(1); g.init_tgv(1)
+        assert np.abs(g.dbg_get("u", padded=True) - O(o, "u", padded=True)).max() <= 1e-7
+        o.close(); g.close()
+
+
+def test_error_paths():
+    from paper_2407_16032_b200 import wl
+    bad = wi.make(ndim=3, dims=(2, 8, 8))
+    assert wl.workspace_bytes(bad) == 0
+    with pytest.raises(wl.WLError):
+        wl.Sim(bad)
+    bad = wi.make(ndim=3, dims=(8, 8, 8), nu=-1.0)
+    assert wl.workspace_bytes(bad) == 0
