@@ -157,6 +157,15 @@ int wl_dbg_set(wl_sim* s, const char* name, int level, const float* in, size_t i
 int wl_dbg_get_padded(wl_sim* s, const char* name, int level, float* out, size_t out_floats);
 int wl_level_dims(const wl_sim* s, int level, int dims_out[3]);
 
+/* Per-kernel-class timing for bench.py's roofline figure.  With enable != 0
+ * every kernel the handle launches is bracketed by two CUDA events on its stream; enabling or
+ * disabling synchronises and discards earlier records.  wl_prof_read synchronises and returns,
+ * for class `cls` = 0, 1, ..., the class name (kernel name; ".coarse" = multigrid levels > 0),
+ * the summed device time in ms and the number of launches since wl_prof_enable.  Returns 1
+ * (not an error) once `cls` is past the last class. */
+int wl_prof_enable(wl_sim* s, int enable);
+int wl_prof_read(wl_sim* s, int cls, char* name_out, size_t name_bytes, double* ms_total, int* launches);
+
 const char* wl_last_error(const wl_sim* s);
 int wl_stats(wl_sim* s, wl_stats_t* out);
 int wl_abi_version(void);

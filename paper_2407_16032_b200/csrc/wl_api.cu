@@ -4,6 +4,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <cmath>
+#include <new>
 #include "wl_internal.h"
 
 // ------------------------------------------------------------------ launch geometry
@@ -234,7 +235,7 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     if (!config_ok(cfg)) return WL_EINVAL;
     size_t need = layout(nullptr, cfg, nullptr);
     if (!dev_ws || ws_bytes < need || ((uintptr_t)dev_ws & 255u)) return WL_ENOMEM;
-    wl_sim* s = (wl_sim*)calloc(1, sizeof(wl_sim));
+    wl_sim* s = new (std::nothrow) wl_sim();     // value-initialised: every POD member zero
     if (!s) return WL_ENOMEM;
     s->cfg = *cfg;
     s->st = (cudaStream_t)cuda_stream;
@@ -245,20 +246,20 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
-        free(s);
+        delete s;
         return WL_ECUDA;
     }
     s->sm_count = prop.multiProcessorCount;
-    if (cudaMallocHost((void**)&s->hs, sizeof(DevScal)) != cudaSuccess) { free(s); return WL_ECUDA; }
+    if (cudaMallocHost((void**)&s->hs, sizeof(DevScal)) != cudaSuccess) { delete s; return WL_ECUDA; }
     memset(s->hs, 0, sizeof(DevScal));
-    if (cudaMemsetAsync(dev_ws, 0, need, s->st) != cudaSuccess) { cudaFreeHost(s->hs); free(s); return WL_ECUDA; }
+    if (cudaMemsetAsync(dev_ws, 0, need, s->st) != cudaSuccess) { cudaFreeHost(s->hs); delete s; return WL_ECUDA; }
     // initial state (R-V): u = U everywhere (all three buffers, so the exit plane is defined), p = 0, measure(0)
     for (int k = 0; k < 3; ++k) wl_k_fill_u(s, s->ubuf[k]);
     wl_k_set_time(s, 0.0, cfg->dt0, 1, 1);
     wl_k_measure(s);
     bc_all(s, s->u);
     int rc = sync(s);
-    if (rc != WL_OK) { cudaFreeHost(s->hs); free(s); return rc; }
+    if (rc != WL_OK) { cudaFreeHost(s->hs); delete s; return rc; }
     *out = s;
     return WL_OK;
 }
@@ -268,7 +269,9 @@ extern "C" int wl_sim_destroy(wl_sim* s)
     if (!s) return WL_EINVAL;
     cudaStreamSynchronize(s->st);
     if (s->hs) cudaFreeHost(s->hs);
-    free(s);
+    for (ProfRec& r : s->prof_recs) s->prof_pool.push_back(r);
+    for (ProfRec& r : s->prof_pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    delete s;
     return WL_OK;
 }
 
@@ -412,6 +415,44 @@ extern "C" int wl_level_dims(const wl_sim* s, int level, int dims_out[3])
 {
     if (!s || level < 0 || level >= s->nlev) return WL_EINVAL;
     for (int d = 0; d < 3; ++d) dims_out[d] = s->lev[level].g.n[d];
+    return WL_OK;
+}
+
+// ---- per-kernel-class timing (CUDA events on the handle's stream)
+static const char* const kern_names[WLK_COUNT] = {
+    "set_time", "measure", "poisson_update", "conv_diff_bdim", "bc", "exit_bc", "residual", "restrict", "prolong",
+    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc"
+};
+
+extern "C" int wl_prof_enable(wl_sim* s, int enable)
+{
+    if (!s) return WL_EINVAL;
+    int rc = sync(s);
+    if (rc != WL_OK) return rc;
+    for (ProfRec& r : s->prof_recs) s->prof_pool.push_back(r);
+    s->prof_recs.clear();
+    s->prof_on = enable ? 1 : 0;
+    return WL_OK;
+}
+
+extern "C" int wl_prof_read(wl_sim* s, int cls, char* name_out, size_t name_bytes, double* ms_total, int* launches)
+{
+    if (!s || cls < 0) return WL_EINVAL;
+    if (cls >= 2 * WLK_COUNT) return 1;
+    int rc = sync(s);
+    if (rc != WL_OK) return rc;
+    double ms = 0.0;
+    int n = 0;
+    for (const ProfRec& r : s->prof_recs) {
+        if (r.cls != cls) continue;
+        float t = 0.0f;
+        WL_CUDA_CHECK(s, cudaEventElapsedTime(&t, r.a, r.b));
+        ms += (double)t;
+        ++n;
+    }
+    if (name_out && name_bytes) snprintf(name_out, name_bytes, "%s%s", kern_names[cls / 2], (cls & 1) ? ".coarse" : "");
+    if (ms_total) *ms_total = ms;
+    if (launches) *launches = n;
     return WL_OK;
 }
 

@@ -170,7 +170,7 @@ void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out,
 {
     FlowP P = wl_flowp(s);
     Tiling T = wl_tiles_interior(s, P.g);
-    s->launches++;
+    ProfScope ps(s, WLK_CONVDIFF);
     if (s->nd == 3)
         k_conv_diff_bdim<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(P, T, w, u0, s->mu0, s->mu1, out, s->ds, corrector);
     else

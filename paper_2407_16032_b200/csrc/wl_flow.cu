@@ -273,11 +273,10 @@ __global__ void __launch_bounds__(512) k_unpack(Grid g, Tiling T, const float* _
 }
 
 // ================================================================== host launchers
-#define LAUNCH(s) ((s)->launches++)
 
 void wl_k_set_time(wl_sim* s, double t, float dt, int t_mode, int dt_mode)
 {
-    LAUNCH(s);
+    ProfScope ps(s, WLK_SET_TIME);
     k_set_time<<<1, 1, 0, s->st>>>(s->ds, s->cfg.body, t, dt, t_mode, dt_mode);
 }
 
@@ -285,9 +284,11 @@ void wl_k_measure(wl_sim* s)
 {
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_padded(s, g);
-    LAUNCH(s);
-    if (s->nd == 3) k_measure<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1);
-    else            k_measure<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1);
+    {
+        ProfScope ps(s, WLK_MEASURE);
+        if (s->nd == 3) k_measure<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1);
+        else            k_measure<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1);
+    }
     wl_k_poisson_update(s);
 }
 
@@ -298,7 +299,7 @@ void wl_k_bc(wl_sim* s, float* u)
     int64_t total = 3 * ((int64_t)g.S[1] * g.S[2] + (int64_t)g.S[0] * g.S[2] + (s->nd == 3 ? (int64_t)g.S[0] * g.S[1] : 0));
     int blocks = (int)((total + 255) / 256);
     if (blocks > s->sm_count * 8) blocks = s->sm_count * 8;
-    LAUNCH(s);
+    ProfScope ps(s, WLK_BC);
     if (s->nd == 3) k_bc<3><<<blocks, 256, 0, s->st>>>(P, u);
     else            k_bc<2><<<blocks, 256, 0, s->st>>>(P, u);
 }
@@ -310,13 +311,15 @@ void wl_k_exit_bc(wl_sim* s, float* u, const float* u0)
     int cnt = g.n[1] * (s->nd == 3 ? g.n[2] : 1);
     int blocks = (cnt + 255) / 256;
     if (blocks > s->sm_count) blocks = s->sm_count;
-    s->launches += 2;
-    if (s->nd == 3) {
-        k_exit_a<3><<<blocks, 256, 0, s->st>>>(P, u, u0, s->ds, s->rb);
-        k_exit_b<3><<<blocks, 256, 0, s->st>>>(P, u, s->ds);
-    } else {
-        k_exit_a<2><<<blocks, 256, 0, s->st>>>(P, u, u0, s->ds, s->rb);
-        k_exit_b<2><<<blocks, 256, 0, s->st>>>(P, u, s->ds);
+    {
+        ProfScope ps(s, WLK_EXIT_BC);
+        if (s->nd == 3) k_exit_a<3><<<blocks, 256, 0, s->st>>>(P, u, u0, s->ds, s->rb);
+        else            k_exit_a<2><<<blocks, 256, 0, s->st>>>(P, u, u0, s->ds, s->rb);
+    }
+    {
+        ProfScope ps(s, WLK_EXIT_BC);
+        if (s->nd == 3) k_exit_b<3><<<blocks, 256, 0, s->st>>>(P, u, s->ds);
+        else            k_exit_b<2><<<blocks, 256, 0, s->st>>>(P, u, s->ds);
     }
 }
 
@@ -325,7 +328,7 @@ void wl_k_cfl(wl_sim* s, const float* u)
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_interior(s, g);
     const wl_config& c = s->cfg;
-    LAUNCH(s);
+    ProfScope ps(s, WLK_CFL);
     if (s->nd == 3) k_cfl<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, u, s->ds, s->rb, c.nu, c.cfl_c, c.cfl_cnu, c.dt_max);
     else            k_cfl<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, u, s->ds, s->rb, c.nu, c.cfl_c, c.cfl_cnu, c.dt_max);
 }
@@ -334,7 +337,7 @@ void wl_k_force(wl_sim* s)
 {
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_interior(s, g);
-    LAUNCH(s);
+    ProfScope ps(s, WLK_FORCE);
     if (s->nd == 3) k_force<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->p, s->ds, s->rb);
     else            k_force<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->p, s->ds, s->rb);
 }
@@ -343,7 +346,7 @@ void wl_k_init_tgv(wl_sim* s, int sign)
 {
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_padded(s, g);
-    LAUNCH(s);
+    ProfScope ps(s, WLK_MISC);
     if (s->nd == 3) k_init_tgv<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->u, s->p, sign);
     else            k_init_tgv<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->u, s->p, sign);
 }
@@ -353,7 +356,7 @@ void wl_k_fill(wl_sim* s, float* a, int64_t n, float v)
     int blocks = (int)((n + 1023) / 1024);
     if (blocks > s->sm_count * 8) blocks = s->sm_count * 8;
     if (blocks < 1) blocks = 1;
-    LAUNCH(s);
+    ProfScope ps(s, WLK_MISC);
     k_fill<<<blocks, 256, 0, s->st>>>(a, n, v);
 }
 
@@ -366,7 +369,7 @@ void wl_k_fill_u(wl_sim* s, float* u)
 void wl_k_pack(wl_sim* s, const Grid& g, const float* padded, float* interior, int ncomp, float scale, int whole)
 {
     Tiling T = whole ? wl_tiles_padded(s, g) : wl_tiles_interior(s, g);
-    LAUNCH(s);
+    ProfScope ps(s, WLK_MISC);
     if (s->nd == 3) k_pack<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, padded, interior, ncomp, scale);
     else            k_pack<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, padded, interior, ncomp, scale);
 }
@@ -374,7 +377,7 @@ void wl_k_pack(wl_sim* s, const Grid& g, const float* padded, float* interior, i
 void wl_k_unpack(wl_sim* s, const Grid& g, const float* interior, float* padded, int ncomp)
 {
     Tiling T = wl_tiles_interior(s, g);
-    LAUNCH(s);
+    ProfScope ps(s, WLK_MISC);
     if (s->nd == 3) k_unpack<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, interior, padded, ncomp);
     else            k_unpack<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, interior, padded, ncomp);
 }

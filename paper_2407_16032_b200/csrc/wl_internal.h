@@ -4,6 +4,15 @@
 #include "../../include/wl.h"
 #include "wl_common.cuh"
 #include "wl_body.cuh"
+#include <vector>
+
+// kernel classes for launch accounting and the optional per-class CUDA-event timing (wl_prof_*)
+enum WlKern {
+    WLK_SET_TIME, WLK_MEASURE, WLK_POISSON_UPDATE, WLK_CONVDIFF, WLK_BC, WLK_EXIT_BC, WLK_RESIDUAL,
+    WLK_RESTRICT, WLK_PROLONG, WLK_PCG_INIT, WLK_PCG_MATVEC, WLK_PCG_UPDATE, WLK_PCG_DIR,
+    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_COUNT
+};
+struct ProfRec { cudaEvent_t a, b; int cls; };
 
 struct Level {
     Grid g;
@@ -37,6 +46,29 @@ struct wl_sim {
     int primed;              // device-resident t and dt are valid (adaptive wl_step)
     int sm_count;
     char err[256];
+    // profiling (off by default): every launch bracketed by two events on the stream
+    int prof_on;
+    std::vector<ProfRec> prof_recs;      // records in use since the last read
+    std::vector<ProfRec> prof_pool;      // events kept for reuse
+};
+
+// One kernel launch: counts it and, when profiling is on, brackets it with CUDA events.
+// Class index = 2*kind + (coarse ? 1 : 0): multigrid levels > 0 are accounted separately.
+struct ProfScope {
+    wl_sim* s; cudaEvent_t stop; 
+    ProfScope(wl_sim* s_, int kind, int coarse = 0) : s(s_), stop(nullptr)
+    {
+        s->launches++;
+        if (!s->prof_on) return;
+        ProfRec r;
+        if (!s->prof_pool.empty()) { r = s->prof_pool.back(); s->prof_pool.pop_back(); }
+        else { cudaEventCreate(&r.a); cudaEventCreate(&r.b); }
+        r.cls = 2 * kind + (coarse ? 1 : 0);
+        cudaEventRecord(r.a, s->st);
+        stop = r.b;
+        s->prof_recs.push_back(r);
+    }
+    ~ProfScope() { if (stop) cudaEventRecord(stop, s->st); }
 };
 
 // flow-side parameters passed by value to kernels

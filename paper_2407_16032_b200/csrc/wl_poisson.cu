@@ -300,9 +300,9 @@ __global__ void __launch_bounds__(512) k_resmax(Grid g, Tiling T, const float* _
 }
 
 // ================================================================== host launchers
-#define DISPATCH(s, kern, T, ...)                                                            \
+#define DISPATCH(s, cls, coarse, kern, T, ...)                                               \
     do {                                                                                     \
-        (s)->launches++;                                                                     \
+        ProfScope ps_(s, cls, coarse);                                                       \
         if ((s)->nd == 3) kern<3><<<wl_grid(s, T), wl_block(3), 0, (s)->st>>>(__VA_ARGS__);  \
         else              kern<2><<<wl_grid(s, T), wl_block(2), 0, (s)->st>>>(__VA_ARGS__);  \
     } while (0)
@@ -316,10 +316,10 @@ void wl_k_poisson_update(wl_sim* s)
             int o[3] = { 1, 1, s->nd == 3 ? 1 : 0 };
             int e[3] = { lv.g.n[0] + 1, lv.g.n[1] + 1, s->nd == 3 ? lv.g.n[2] + 1 : 1 };
             Tiling T = wl_tiling(s->nd, o, e);
-            DISPATCH(s, k_restrict_L, T, lf.g, lv.g, T, lf.L, lv.L);
+            DISPATCH(s, WLK_POISSON_UPDATE, l > 1, k_restrict_L, T, lf.g, lv.g, T, lf.L, lv.L);
         }
         Tiling T = wl_tiles_interior(s, lv.g);
-        DISPATCH(s, k_diag, T, lv.g, T, lv.L, lv.iD);
+        DISPATCH(s, WLK_POISSON_UPDATE, l > 0, k_diag, T, lv.g, T, lv.L, lv.iD);
     }
 }
 
@@ -327,28 +327,28 @@ void wl_k_residual(wl_sim* s, const float* u, float w)
 {
     Level& lv = s->lev[0];
     Tiling T = wl_tiles_interior(s, lv.g);
-    DISPATCH(s, k_residual, T, lv.g, T, u, lv.L, s->p, lv.x, lv.r, s->ds, w);
+    DISPATCH(s, WLK_RESIDUAL, 0, k_residual, T, lv.g, T, u, lv.L, s->p, lv.x, lv.r, s->ds, w);
 }
 
 void wl_k_apply_gradient(wl_sim* s, float* u)
 {
     Level& lv = s->lev[0];
     Tiling T = wl_tiles_interior(s, lv.g);
-    DISPATCH(s, k_apply_gradient, T, lv.g, T, u, lv.L, lv.x, s->p, s->ds);
+    DISPATCH(s, WLK_GRADIENT, 0, k_apply_gradient, T, lv.g, T, u, lv.L, lv.x, s->p, s->ds);
 }
 
 void wl_k_restrict(wl_sim* s, int l)
 {
     Level &lf = s->lev[l], &lc = s->lev[l + 1];
     Tiling T = wl_tiles_interior(s, lc.g);
-    DISPATCH(s, k_restrict_r, T, lf.g, lc.g, T, lf.r, lc.r, lc.x);
+    DISPATCH(s, WLK_RESTRICT, l > 0, k_restrict_r, T, lf.g, lc.g, T, lf.r, lc.r, lc.x);
 }
 
 void wl_k_prolong(wl_sim* s, int l)
 {
     Level &lf = s->lev[l], &lc = s->lev[l + 1];
     Tiling T = wl_tiles_interior(s, lf.g);
-    DISPATCH(s, k_prolong, T, lf.g, lc.g, T, lf.L, lc.x, lf.x, lf.r);
+    DISPATCH(s, WLK_PROLONG, l > 0, k_prolong, T, lf.g, lc.g, T, lf.L, lc.x, lf.x, lf.r);
 }
 
 void wl_k_smooth(wl_sim* s, int l, int iters)
@@ -356,12 +356,12 @@ void wl_k_smooth(wl_sim* s, int l, int iters)
     Level& lv = s->lev[l];
     Tiling T = wl_tiles_interior(s, lv.g);
     PcgScal* sc = &s->ds->pcg[l];
-    DISPATCH(s, k_pcg_init, T, lv.g, T, lv.r, lv.iD, lv.e, sc, s->rb);
+    DISPATCH(s, WLK_PCG_INIT, l > 0, k_pcg_init, T, lv.g, T, lv.r, lv.iD, lv.e, sc, s->rb);
     for (int k = 1; k <= iters; ++k) {
-        DISPATCH(s, k_pcg_matvec, T, lv.g, T, lv.L, lv.e, lv.q, sc, s->rb);
-        DISPATCH(s, k_pcg_update, T, lv.g, T, lv.x, lv.r, lv.e, lv.q, lv.iD, sc, s->rb, k == iters ? 1 : 0);
+        DISPATCH(s, WLK_PCG_MATVEC, l > 0, k_pcg_matvec, T, lv.g, T, lv.L, lv.e, lv.q, sc, s->rb);
+        DISPATCH(s, WLK_PCG_UPDATE, l > 0, k_pcg_update, T, lv.g, T, lv.x, lv.r, lv.e, lv.q, lv.iD, sc, s->rb, k == iters ? 1 : 0);
         if (k == iters) break;
-        DISPATCH(s, k_pcg_dir, T, lv.g, T, lv.e, lv.q, sc);
+        DISPATCH(s, WLK_PCG_DIR, l > 0, k_pcg_dir, T, lv.g, T, lv.e, lv.q, sc);
     }
 }
 
@@ -378,5 +378,5 @@ void wl_k_resmax(wl_sim* s)
 {
     Level& lv = s->lev[0];
     Tiling T = wl_tiles_interior(s, lv.g);
-    DISPATCH(s, k_resmax, T, lv.g, T, lv.r, s->ds, s->rb);
+    DISPATCH(s, WLK_RESMAX, 0, k_resmax, T, lv.g, T, lv.r, s->ds, s->rb);
 }

@@ -25,6 +25,7 @@ EXPORTS = [
     "wl_dbg_conv_diff_bdim", "wl_dbg_save_u0", "wl_dbg_bc", "wl_dbg_exit_bc", "wl_dbg_project",
     "wl_dbg_residual", "wl_dbg_restrict", "wl_dbg_prolong", "wl_dbg_smooth", "wl_dbg_vcycle",
     "wl_dbg_get", "wl_dbg_set", "wl_dbg_get_padded", "wl_level_dims", "wl_last_error", "wl_stats", "wl_abi_version",
+    "wl_prof_enable", "wl_prof_read",
 ]
 
 
@@ -97,6 +98,8 @@ def load(build_if_missing: bool = True):
     L.wl_last_error.argtypes = [vp]
     L.wl_stats.argtypes = [vp, C.POINTER(Stats)]
     L.wl_abi_version.restype = ip
+    L.wl_prof_enable.argtypes = [vp, ip]
+    L.wl_prof_read.argtypes = [vp, ip, C.c_char_p, C.c_size_t, C.POINTER(C.c_double), C.POINTER(C.c_int)]
     _lib = L
     return L
 
@@ -249,6 +252,23 @@ class Sim:
         self._chk(self._L.wl_stats(self._h, C.byref(st)))
         return {"vcycles": [st.vcycles[0], st.vcycles[1]], "res": [st.res[0], st.res[1]],
                 "nlevels": st.nlevels, "kernel_launches": st.kernel_launches, "nan_flag": st.nan_flag}
+
+    def prof_enable(self, enable: bool = True):
+        self._chk(self._L.wl_prof_enable(self._h, int(enable)))
+
+    def prof_read(self) -> dict:
+        """{kernel class: (total ms, launches)} since prof_enable; classes never launched are omitted."""
+        out = {}
+        cls = 0
+        while True:
+            name = C.create_string_buffer(48)
+            ms, n = C.c_double(), C.c_int()
+            rc = self._chk(self._L.wl_prof_read(self._h, cls, name, 48, C.byref(ms), C.byref(n)))
+            if rc == 1:
+                return out
+            if n.value:
+                out[name.value.decode()] = (ms.value, n.value)
+            cls += 1
 
     def synchronize(self):
         self._stream.synchronize()
