@@ -39,6 +39,12 @@ int wl_grid(const wl_sim* s, const Tiling& T)
     if (cap > WL_MAX_PARTIALS) cap = WL_MAX_PARTIALS;
     return T.ntiles < cap ? (T.ntiles > 0 ? T.ntiles : 1) : cap;
 }
+int wl_vgrid(const wl_sim* s, const VT& vt)
+{
+    int cap = s->sm_count * 4;
+    if (cap > WL_MAX_PARTIALS) cap = WL_MAX_PARTIALS;
+    return vt.ntiles < cap ? (vt.ntiles > 0 ? vt.ntiles : 1) : cap;
+}
 FlowP wl_flowp(const wl_sim* s)
 {
     FlowP P;
@@ -73,12 +79,28 @@ static Grid make_grid(int nd, const int* n, const int* per)
         g.S[d] = d < nd ? n[d] + 2 : 1;
         g.per[d] = d < nd ? (per[d] ? 1 : 0) : 0;
     }
-    g.P = ((g.n[0] + 9 + 7) / 8) * 8;
+    // offset 7 + c0 of the last float4 group (and of its +4 neighbour) stays inside the row
+    g.P = ((g.n[0] + 12 + 7) / 8) * 8;
     g.sy = g.P;
     g.sz = nd == 3 ? (int64_t)g.P * g.S[1] : 0;
     int64_t tot = (int64_t)g.P * g.S[1] * g.S[2];
     g.nalloc = ((tot + 63) / 64) * 64;
     return g;
+}
+
+static VT make_vt(int nd, const Grid& g)
+{
+    VT t;
+    t.ngx = (g.n[0] + 3) / 4;
+    t.lxl = 0;
+    while ((1 << t.lxl) < t.ngx && t.lxl < 5) ++t.lxl;
+    const int lx = 1 << t.lxl, ly = WL_VB >> t.lxl;
+    t.ntx = (t.ngx + lx - 1) / lx;
+    t.nty = (g.n[1] + ly - 1) / ly;
+    t.zc = nd == 3 ? (g.n[2] < 8 ? g.n[2] : 8) : 1;
+    t.ntz = nd == 3 ? (g.n[2] + t.zc - 1) / t.zc : 1;
+    t.ntiles = t.ntx * t.nty * t.ntz;
+    return t;
 }
 
 static int level_dims(const wl_config* c, int dims[WL_MAXLEV][3])
@@ -134,8 +156,18 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
         float* x = (float*)cv.take(scl);
         float* r = (float*)cv.take(scl);
         float* e = (float*)cv.take(scl);
+        float* e2 = (float*)cv.take(scl);
         float* q = (float*)cv.take(scl);
-        if (s) { Level& lv = s->lev[l]; lv.g = g; lv.L = L; lv.iD = iD; lv.x = x; lv.r = r; lv.e = e; lv.q = q; }
+        VT vt = make_vt(nd, g);
+        int* plain = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
+        int* uniform = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
+        if (s) {
+            Level& lv = s->lev[l];
+            lv.g = g; lv.L = L; lv.iD = iD; lv.x = x; lv.r = r; lv.e = e; lv.e2 = e2; lv.q = q;
+            lv.vt = vt; lv.plain = plain; lv.uniform = uniform;
+            lv.Lc = nd == 3 ? (float)(1 << l) : 1.0f;
+            lv.iDc = 1.0f / (-(2.0f * nd) * lv.Lc);
+        }
     }
     return cv.off;
 }

@@ -4,6 +4,7 @@
 #include "../../include/wl.h"
 #include "wl_common.cuh"
 #include "wl_body.cuh"
+#include "wl_vec.cuh"
 #include <vector>
 
 // kernel classes for launch accounting and the optional per-class CUDA-event timing (wl_prof_*)
@@ -20,8 +21,14 @@ struct Level {
     float* iD;   // inverse diagonal
     float* x;    // solution / correction
     float* r;    // residual
-    float* e;    // CG direction
-    float* q;    // A e, then z = iD r
+    float* e;    // CG direction (ping)
+    float* e2;   // CG direction (pong): pass A reads one and writes the other
+    float* q;    // A e
+    VT vt;       // vector tiling of this level
+    int* uniform; // per-tile flag: every face coefficient of every cell of the tile equals Lc
+    int* plain;  // per-tile flag: the tile and its face-neighbour tiles are uniform (kernels skip L and iD loads)
+    float Lc;    // face coefficient of a body-free, boundary-free cell on this level (R-S: 1, or 2^l in 3-D)
+    float iDc;   // 1 / (-2 n Lc)
 };
 
 struct wl_sim {
@@ -83,6 +90,7 @@ struct FlowP {
 dim3 wl_block(int nd);
 Tiling wl_tiling(int nd, const int o[3], const int e[3]);
 int wl_grid(const wl_sim* s, const Tiling& T);
+int wl_vgrid(const wl_sim* s, const VT& vt);
 Tiling wl_tiles_interior(const wl_sim* s, const Grid& g);
 Tiling wl_tiles_padded(const wl_sim* s, const Grid& g);
 FlowP wl_flowp(const wl_sim* s);

@@ -2,7 +2,8 @@
 seeded inputs (BASELINE.json north_star: relative L-infinity <= 2e-5).  All calls go through
 the C ABI (paper_2407_16032_b200.wl is argument marshalling only).
 
-Sizes span several 32x4x4 (3-D) / 32x16 (2-D) tiles and ragged tails: 32^3, 48x32x40, 64x48.
+Sizes span several tiles of the vector kernels (4*LX x LY x 8 cells, LX*LY = 256) and of the scalar
+kernels (32x4x4 / 32x16) with ragged tails: 32^3, 48x32x40, 64x48, 160x48x40, 136x40x24, 272x36.
 """
 import numpy as np
 import pytest
@@ -64,6 +65,11 @@ CASES = [
     ((64, 48), (1, 1), 0, "none", False),
     ((64, 48), (0, 0), 1, "sphere", True),
     ((64, 48), (0, 1), 0, "sphere", False),
+    # wide enough for several float4 x 32-lane tiles per row: body-free ("plain") tiles, tiles cut by
+    # the body and by the domain boundary, and a ragged tail in x (136 = 34 groups) all occur
+    ((160, 48, 40), (0, 0, 0), 1, "sphere", False),
+    ((136, 40, 24), (1, 1, 1), 0, "torus", False),
+    ((272, 36), (0, 1), 1, "sphere", False),
 ]
 
 
@@ -219,8 +225,11 @@ def test_pcg_smoother(case, iters):
         o.arr("x", l)[...] = 0.0
         g.dbg_set("r", r0[None], l)
         g.dbg_set("x", np.zeros_like(r0)[None], l)
-        # same coefficients on both sides: 1/D from the measure/diagonal kernels is checked in
-        # test_measure_and_poisson_coefficients; here only the smoother's own arithmetic is
+        # same coefficients on both sides: L and 1/D from the measure/diagonal kernels are checked in
+        # test_measure_and_poisson_coefficients; here only the smoother's own arithmetic is.  (A
+        # smooth seeded residual makes alpha = rho/gamma ~ 20, which multiplies the ~1e-6 fp32
+        # error of mu0 in the body band into the residual.)
+        g.dbg_set("L", O(o, "L", l), l)
         g.dbg_set("iD", O(o, "iD", l), l)
         o.smooth(l, iters)
         g.dbg_smooth(l, iters)
