@@ -145,6 +145,7 @@ int wl_dbg_bc(wl_sim* s);
 int wl_dbg_exit_bc(wl_sim* s, float dt);
 int wl_dbg_project(wl_sim* s, float w, float dt);
 int wl_dbg_residual(wl_sim* s);                                /* sigma = div u; r = sigma - A x on level 0 */
+int wl_dbg_apply_gradient(wl_sim* s);                          /* P:88 kernel with the current x and pscale: u -= L grad x; p = x/pscale */
 int wl_dbg_restrict(wl_sim* s, int level);
 int wl_dbg_prolong(wl_sim* s, int level);
 int wl_dbg_smooth(wl_sim* s, int level, int iters);

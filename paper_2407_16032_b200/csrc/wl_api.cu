@@ -532,6 +532,7 @@ extern "C" int wl_dbg_residual(wl_sim* s)
     WL_CUDA_CHECK(s, cudaMemcpyAsync(s->p, s->lev[0].q, sizeof(float) * g.nalloc, cudaMemcpyDeviceToDevice, s->st));
     return check(s);
 }
+extern "C" int wl_dbg_apply_gradient(wl_sim* s) { if (!s) return WL_EINVAL; wl_k_apply_gradient(s, s->u); return check(s); }
 extern "C" int wl_dbg_restrict(wl_sim* s, int l) { if (!s || l < 0 || l + 1 >= s->nlev) return WL_EINVAL; wl_k_restrict(s, l); return check(s); }
 extern "C" int wl_dbg_prolong(wl_sim* s, int l) { if (!s || l < 0 || l + 1 >= s->nlev) return WL_EINVAL; wl_k_prolong(s, l); return check(s); }
 extern "C" int wl_dbg_smooth(wl_sim* s, int l, int iters) { if (!s || l < 0 || l >= s->nlev || iters < 1) return WL_EINVAL; wl_k_smooth(s, l, iters); return check(s); }

@@ -57,7 +57,8 @@ def main():
             s.dbg_smooth(1, 2)
         s.dbg_prolong(0)
         s.dbg_smooth(0, 3)
-        s.dbg_project(1.0, dt)
+        s.dbg_residual()
+        s.dbg_apply_gradient()
         s.cfl()
         if cfg["body_kind"] != wi.BODY_NONE:
             s.pressure_force(1.0)

@@ -23,7 +23,7 @@ EXPORTS = [
     "wl_workspace_bytes", "wl_sim_create", "wl_sim_destroy", "wl_set_fields", "wl_init_tgv", "wl_measure",
     "wl_mom_step", "wl_cfl", "wl_pressure_force", "wl_get_fields", "wl_step",
     "wl_dbg_conv_diff_bdim", "wl_dbg_save_u0", "wl_dbg_bc", "wl_dbg_exit_bc", "wl_dbg_project",
-    "wl_dbg_residual", "wl_dbg_restrict", "wl_dbg_prolong", "wl_dbg_smooth", "wl_dbg_vcycle",
+    "wl_dbg_residual", "wl_dbg_apply_gradient", "wl_dbg_restrict", "wl_dbg_prolong", "wl_dbg_smooth", "wl_dbg_vcycle",
     "wl_dbg_get", "wl_dbg_set", "wl_dbg_get_padded", "wl_level_dims", "wl_last_error", "wl_stats", "wl_abi_version",
     "wl_prof_enable", "wl_prof_read",
 ]
@@ -87,6 +87,7 @@ def load(build_if_missing: bool = True):
     L.wl_dbg_exit_bc.argtypes = [vp, C.c_float]
     L.wl_dbg_project.argtypes = [vp, C.c_float, C.c_float]
     L.wl_dbg_residual.argtypes = [vp]
+    L.wl_dbg_apply_gradient.argtypes = [vp]
     for name in ("wl_dbg_restrict", "wl_dbg_prolong", "wl_dbg_vcycle"):
         getattr(L, name).argtypes = [vp, ip]
     L.wl_dbg_smooth.argtypes = [vp, ip, ip]
@@ -310,6 +311,9 @@ class Sim:
 
     def dbg_residual(self):
         self._chk(self._L.wl_dbg_residual(self._h))
+
+    def dbg_apply_gradient(self):
+        self._chk(self._L.wl_dbg_apply_gradient(self._h))
 
     def dbg_restrict(self, level):
         self._chk(self._L.wl_dbg_restrict(self._h, int(level)))
