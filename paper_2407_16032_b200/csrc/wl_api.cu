@@ -142,10 +142,18 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
     float* p = (float*)cv.take(sc);
     float* mu0 = (float*)cv.take(sc * nd);
     float* mu1 = (float*)cv.take(sc * nd * nd);
+    // band list: faces within eps of the body surface; a generous share of all faces (overflow falls back to a scan)
+    int64_t ncell = (int64_t)dims[0][0] * dims[0][1] * dims[0][2];
+    int64_t bcap = ncell * nd / 4;
+    if (bcap < 4096) bcap = 4096;
+    if (bcap > (1 << 26)) bcap = 1 << 26;
+    if (c->body.kind == WL_BODY_NONE) bcap = 64;
+    long long* band = (long long*)cv.take(sizeof(long long) * (size_t)bcap);
     if (s) {
         s->ds = ds; s->rb.partial = partial; s->rb.counter = counter;
         for (int k = 0; k < 3; ++k) s->ubuf[k] = ub[k];
         s->p = p; s->mu0 = mu0; s->mu1 = mu1;
+        s->band_list = band; s->band_cap = (int)bcap;
         s->nlev = nlev; s->nd = nd;
     }
     for (int l = 0; l < nlev; ++l) {
@@ -453,7 +461,7 @@ extern "C" int wl_level_dims(const wl_sim* s, int level, int dims_out[3])
 // ---- per-kernel-class timing (CUDA events on the handle's stream)
 static const char* const kern_names[WLK_COUNT] = {
     "set_time", "measure", "poisson_update", "conv_diff_bdim", "bc", "exit_bc", "residual", "restrict", "prolong",
-    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc"
+    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc", "conv_diff_band"
 };
 
 extern "C" int wl_prof_enable(wl_sim* s, int enable)

@@ -63,7 +63,7 @@ struct DevScal {
     double force[3];
     double resmax;
     int    nan_flag;
-    int    pad;
+    int    band_count;   // faces with mu1 != 0 found by the last measure! (may exceed the list capacity)
 };
 
 // reduction scratch: partial sums of up to 4 values per block + the arrival counter

@@ -4,8 +4,16 @@
 //   f   = u0 + dt r - V ;  B_i = V_i + mu0 f_i + sum_j mu1_ij (f_i[c+d_j] - f_i[c-d_j])/2
 //                                          (Eq. 1-2; R-B, R-C)
 //   predictor: u = B ; corrector: u = (u' + B)/2            (P:76, P:139 scale_u!; R-K, R-L)
-// One pass over the grid: f is never stored.  mu1 is non-zero only within eps of the body
-// surface; only there the neighbours' f (six more evaluations of r) are recomputed.
+// f is never stored.  Two kernels:
+//  * k_cd_tile: the whole grid.  A block owns a 128 x 8 column of cells and marches along z; the
+//    three velocity components of the five planes z-2..z+2 (with a two-cell halo in x and y,
+//    periodic wrap applied while loading) sit in a shared-memory ring, so every value is read from
+//    HBM/L2 once per tile and all stencil reads are conflict-free 16-byte shared loads.  Each
+//    thread owns four consecutive x cells: x-face fluxes are shared inside the thread.  It
+//    writes u = V + mu0 f (with the Heun average in the corrector) and never reads mu1.
+//  * k_cd_band: mu1 is non-zero only within eps of the body surface; measure! leaves a compact
+//    list of those faces (wl_flow.cu) and this kernel adds sum_j mu1_ij (f_i[c+d_j]-f_i[c-d_j])/2
+//    there, recomputing the six neighbouring r from global memory.
 #include <cstdio>
 #include "wl_internal.h"
 
@@ -114,65 +122,386 @@ __device__ float f_at(const FlowP& P, const float* __restrict__ w, const float* 
     return u0[I * g.nalloc + gidx(g, c[0], c[1], c[2])] + dt * r - Vi;
 }
 
+
+// ====================================================================== the tile kernel
+#define CD_TX 32                       // threads along x, four cells each
+#define CD_TY 8                        // rows per block
+#define CD_NT (CD_TX * CD_TY)
+#define CD_G (CD_TX + 2)               // float4 groups per shared row: cells bx-4 .. bx+4*CD_TX+3
+#define CD_W (4 * CD_G)                // floats per shared row
+#define CD_R (CD_TY + 4)               // shared rows: by-2 .. by+CD_TY+1
+#define CD_PLANE (CD_W * CD_R)         // floats per component per plane
+#define CD_NP 5                        // ring of planes z-2 .. z+2
+
+__device__ __forceinline__ int wrap_any(int c, int N)      // 1..N for any c
+{
+    int m = (c - 1) % N;
+    return (m < 0 ? m + N : m) + 1;
+}
+__device__ __forceinline__ int src_coord(int c, int N, int per)
+{
+    if (per) return wrap_any(c, N);
+    return c < 0 ? 0 : (c > N + 1 ? N + 1 : c);   // clamped values are never used (R-H fallback)
+}
+
+// One 16-byte group of a shared plane: component comp, shared row `row`, group grp, plane cz.
+template <int ND>
+__device__ __forceinline__ float4 cd_fetch(const Grid& g, const float* __restrict__ w, int item, int bx, int by, int cz)
+{
+    const int comp = item / (CD_R * CD_G);
+    const int rem = item - comp * (CD_R * CD_G);
+    const int row = rem / CD_G, grp = rem - row * CD_G;
+    const int cy = src_coord(by - 2 + row, g.n[1], g.per[1]);
+    const int xs = bx - 4 + 4 * grp;
+    const float* src = w + comp * g.nalloc + (int64_t)WL_OFF + (int64_t)cy * g.sy + (int64_t)cz * g.sz;
+    if (xs >= 1 && xs + 3 <= g.n[0]) return ld4(src, xs);
+    float4 v;
+    v.x = __ldg(src + src_coord(xs, g.n[0], g.per[0]));
+    v.y = __ldg(src + src_coord(xs + 1, g.n[0], g.per[0]));
+    v.z = __ldg(src + src_coord(xs + 2, g.n[0], g.per[0]));
+    v.w = __ldg(src + src_coord(xs + 3, g.n[0], g.per[0]));
+    return v;
+}
+
+#define CD_ITEMS(ND) ((ND) * CD_R * CD_G)
+#define CD_STAGE(ND) ((CD_ITEMS(ND) + CD_NT - 1) / CD_NT)
+
+template <int ND>
+__device__ __forceinline__ void cd_load_regs(const Grid& g, const float* __restrict__ w, int bx, int by, int cz, float4 (&st)[CD_STAGE(ND)])
+{
+#pragma unroll
+    for (int k = 0; k < CD_STAGE(ND); ++k) {
+        const int item = threadIdx.x + k * CD_NT;
+        if (item < CD_ITEMS(ND)) st[k] = cd_fetch<ND>(g, w, item, bx, by, cz);
+    }
+}
+template <int ND>
+__device__ __forceinline__ void cd_store_regs(float* __restrict__ slot, const float4 (&st)[CD_STAGE(ND)])
+{
+#pragma unroll
+    for (int k = 0; k < CD_STAGE(ND); ++k) {
+        const int item = threadIdx.x + k * CD_NT;
+        if (item < CD_ITEMS(ND)) reinterpret_cast<float4*>(slot)[item] = st[k];   // slot layout = [comp][row][grp]
+    }
+}
+
+// limited flux through one face: wm | wc are the values either side, wup / wun the far-upwind
+// values for phi > 0 / phi <= 0, fbp / fbn the boundary fallbacks of R-H
+__device__ __forceinline__ float face_flux(float phi, float wup, float wm, float wc, float wun, bool fbp, bool fbn, float nu)
+{
+    const bool pos = phi > 0.0f;
+    const bool fb = pos ? fbp : fbn;
+    const float U = pos ? wup : wun, C = pos ? wm : wc, D = pos ? wc : wm;
+    const float psi = fb ? 0.5f * (wm + wc) : quick(U, C, D);
+    return phi * psi - nu * (wc - wm);
+}
+
+// read-only view of the shared ring for one thread: p[comp][dz + 2] = plane z+dz of component comp
+struct CdView {
+    const float* p[3][CD_NP];
+    int tx, ty;
+};
+// group tx+1+dg of shared row ty+2+dy: the thread's own four cells are dg = 0
+__device__ __forceinline__ void v4(const CdView& v, int comp, int dz, int dy, int dg, float* o)
+{
+    const float4 t = reinterpret_cast<const float4*>(v.p[comp][dz + 2])[(v.ty + 2 + dy) * CD_G + v.tx + 1 + dg];
+    o[0] = t.x; o[1] = t.y; o[2] = t.z; o[3] = t.w;
+}
+// one value: col counts from the thread's first cell (-1 = x-1, 4 = x+4)
+__device__ __forceinline__ float v1(const CdView& v, int comp, int dz, int dy, int col)
+{
+    return v.p[comp][dz + 2][(v.ty + 2 + dy) * CD_W + 4 * (v.tx + 1) + col];
+}
+
+// r_I at the thread's four cells (gx..gx+3, gy, gz) from the shared planes; a[] returns the own row
+// of w_I (cells gx-4 .. gx+7)
 template <int ND, int I>
-__device__ __forceinline__ void blend_comp(const FlowP& P, const float* __restrict__ w, const float* __restrict__ u0,
-                                           const float* __restrict__ mu0, const float* __restrict__ mu1,
-                                           float* __restrict__ out, const Sten<ND>& S, int64_t id, float dt, float Vi, int corrector)
+__device__ __forceinline__ void cd_rhs(const FlowP& P, const CdView& v, int gx, int gy, int gz, float (&a)[12], float (&r)[4])
 {
     const Grid& g = P.g;
-    float r = rhs_comp<ND, I>(P, w, S);
-    float f = u0[I * g.nalloc + id] + dt * r - Vi;
-    float B = Vi + mu0[I * g.nalloc + id] * f;
-    float m1[3];
-    bool band = false;
+    const float nu = P.nu;
+    v4(v, I, 0, 0, -1, a); v4(v, I, 0, 0, 0, a + 4); v4(v, I, 0, 0, 1, a + 8);
+    // ---- x faces gx .. gx+4 (shared between the thread's cells)
+    {
+        float px[5];
+        if (I == 0) {
 #pragma unroll
-    for (int j = 0; j < ND; ++j) {
-        m1[j] = mu1[(I * ND + j) * g.nalloc + id];
-        band = band || (m1[j] != 0.0f);
-    }
-    if (band) {
+            for (int f = 0; f < 5; ++f) px[f] = 0.5f * (a[3 + f] + a[4 + f]);
+        } else {
+            float lo[5], hi[5];
+            v4(v, 0, 0, 0, 0, hi); hi[4] = v1(v, 0, 0, 0, 4);
+            if (I == 1) { v4(v, 0, 0, -1, 0, lo); lo[4] = v1(v, 0, 0, -1, 4); }
+            else        { v4(v, 0, -1, 0, 0, lo); lo[4] = v1(v, 0, -1, 0, 4); }
 #pragma unroll
-        for (int j = 0; j < ND; ++j) {
-            int cp[3] = { S.c[0], S.c[1], S.c[2] }, cm[3] = { S.c[0], S.c[1], S.c[2] };
-            cp[j] += 1; cm[j] -= 1;
-            float fp = f_at<ND, I>(P, w, u0, dt, Vi, cp[0], cp[1], cp[2]);
-            float fm = f_at<ND, I>(P, w, u0, dt, Vi, cm[0], cm[1], cm[2]);
-            B += m1[j] * 0.5f * (fp - fm);
+            for (int f = 0; f < 5; ++f) px[f] = 0.5f * (lo[f] + hi[f]);
         }
+        float F[5];
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+            const int cj = gx + f;
+            const bool fbp = !g.per[0] && cj <= 1 + (I == 0 ? 1 : 0), fbn = !g.per[0] && cj >= g.n[0] + 1;
+            F[f] = face_flux(px[f], a[2 + f], a[3 + f], a[4 + f], a[5 + f], fbp, fbn, nu);
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) r[k] = F[k] - F[k + 1];
     }
-    out[I * g.nalloc + id] = corrector ? 0.5f * (w[I * g.nalloc + id] + B) : B;
+    // ---- y faces: lower (gy) and upper (gy+1)
+    {
+        float m2[4], m1[4], p1[4], p2[4], pl[4], pu[4];
+        v4(v, I, 0, -2, 0, m2); v4(v, I, 0, -1, 0, m1); v4(v, I, 0, 1, 0, p1); v4(v, I, 0, 2, 0, p2);
+        if (I == 1) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { pl[k] = 0.5f * (m1[k] + a[4 + k]); pu[k] = 0.5f * (a[4 + k] + p1[k]); }
+        } else if (I == 0) {
+            float b0[4], b1[4];
+            v4(v, 1, 0, 0, 0, b0); v4(v, 1, 0, 1, 0, b1);
+            const float e0 = v1(v, 1, 0, 0, -1), e1 = v1(v, 1, 0, 1, -1);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                pl[k] = 0.5f * ((k == 0 ? e0 : b0[k == 0 ? 0 : k - 1]) + b0[k]);
+                pu[k] = 0.5f * ((k == 0 ? e1 : b1[k == 0 ? 0 : k - 1]) + b1[k]);
+            }
+        } else {
+            float b0[4], b1[4], c0[4], c1[4];
+            v4(v, 1, -1, 0, 0, b0); v4(v, 1, 0, 0, 0, c0); v4(v, 1, -1, 1, 0, b1); v4(v, 1, 0, 1, 0, c1);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { pl[k] = 0.5f * (b0[k] + c0[k]); pu[k] = 0.5f * (b1[k] + c1[k]); }
+        }
+        const bool np = !g.per[1];
+        const bool lfbp = np && gy <= 1 + (I == 1 ? 1 : 0), lfbn = np && gy >= g.n[1] + 1;
+        const bool ufbp = np && gy + 1 <= 1 + (I == 1 ? 1 : 0), ufbn = np && gy + 1 >= g.n[1] + 1;
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            r[k] += face_flux(pl[k], m2[k], m1[k], a[4 + k], p1[k], lfbp, lfbn, nu)
+                  - face_flux(pu[k], m1[k], a[4 + k], p1[k], p2[k], ufbp, ufbn, nu);
+    }
+    // ---- z faces
+    if (ND == 3) {
+        float m2[4], m1[4], p1[4], p2[4], pl[4], pu[4];
+        v4(v, I, -2, 0, 0, m2); v4(v, I, -1, 0, 0, m1); v4(v, I, 1, 0, 0, p1); v4(v, I, 2, 0, 0, p2);
+        if (I == 2) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { pl[k] = 0.5f * (m1[k] + a[4 + k]); pu[k] = 0.5f * (a[4 + k] + p1[k]); }
+        } else if (I == 0) {
+            float b0[4], b1[4];
+            v4(v, 2, 0, 0, 0, b0); v4(v, 2, 1, 0, 0, b1);
+            const float e0 = v1(v, 2, 0, 0, -1), e1 = v1(v, 2, 1, 0, -1);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                pl[k] = 0.5f * ((k == 0 ? e0 : b0[k == 0 ? 0 : k - 1]) + b0[k]);
+                pu[k] = 0.5f * ((k == 0 ? e1 : b1[k == 0 ? 0 : k - 1]) + b1[k]);
+            }
+        } else {
+            float b0[4], b1[4], c0[4], c1[4];
+            v4(v, 2, 0, -1, 0, b0); v4(v, 2, 0, 0, 0, c0); v4(v, 2, 1, -1, 0, b1); v4(v, 2, 1, 0, 0, c1);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { pl[k] = 0.5f * (b0[k] + c0[k]); pu[k] = 0.5f * (b1[k] + c1[k]); }
+        }
+        const bool np = !g.per[2];
+        const bool lfbp = np && gz <= 1 + (I == 2 ? 1 : 0), lfbn = np && gz >= g.n[2] + 1;
+        const bool ufbp = np && gz + 1 <= 1 + (I == 2 ? 1 : 0), ufbn = np && gz + 1 >= g.n[2] + 1;
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            r[k] += face_flux(pl[k], m2[k], m1[k], a[4 + k], p1[k], lfbp, lfbn, nu)
+                  - face_flux(pu[k], m1[k], a[4 + k], p1[k], p2[k], ufbp, ufbn, nu);
+    }
+}
+
+struct CdT { int ntx, nty, ntz, ntiles, zc; };
+
+template <int ND, int I>
+__device__ __forceinline__ void cd_comp(const FlowP& P, const CdView& v, int gx, int gy, int gz, int nv,
+                                        const float* __restrict__ u0, const float* __restrict__ mu0, const float* __restrict__ w,
+                                        float* __restrict__ out, float dt, float Vi, int corrector)
+{
+    const Grid& g = P.g;
+    float a[12], r[4], o[4], uu[4], mm[4];
+    cd_rhs<ND, I>(P, v, gx, gy, gz, a, r);
+    if (nv <= 0) return;
+    const int64_t id = gidx(g, gx, gy, gz);
+    unpack4(ld4(mu0 + I * g.nalloc, id), mm);
+    if (corrector) unpack4(ld4(u0 + I * g.nalloc, id), uu);
+    else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) uu[k] = a[4 + k];
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float f = uu[k] + dt * r[k] - Vi;
+        const float B = Vi + mm[k] * f;
+        o[k] = corrector ? 0.5f * (a[4 + k] + B) : B;
+    }
+    st4(out + I * g.nalloc, id, o, nv);
+    // the corrector leaves the convective-exit plane at the predictor's value (R-N); the output is
+    // another buffer, so carry the plane over
+    if (I == 0 && corrector && P.exit_bc) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (gx + k == g.n[0]) out[id + k + 1] = a[5 + k];
+    }
 }
 
 template <int ND>
-__global__ void __launch_bounds__(512) k_conv_diff_bdim(FlowP P, Tiling T, const float* __restrict__ w, const float* __restrict__ u0,
-                                                        const float* __restrict__ mu0, const float* __restrict__ mu1,
-                                                        float* __restrict__ out, const DevScal* __restrict__ ds, int corrector)
+__global__ void __launch_bounds__(CD_NT, 2) k_cd_tile(FlowP P, CdT T, const float* __restrict__ w, const float* __restrict__ u0,
+                                                      const float* __restrict__ mu0, float* __restrict__ out,
+                                                      const DevScal* __restrict__ ds, int corrector)
 {
+    extern __shared__ float4 cd_smem[];
+    float* ring = reinterpret_cast<float*>(cd_smem);
     const Grid& g = P.g;
     const float dt = ds->dt;
     const float V0 = ds->vel[0], V1 = ds->vel[1], V2 = ds->vel[2];
+    constexpr int NP = ND == 3 ? CD_NP : 1;
+    constexpr int SLOT = ND * CD_PLANE;            // floats per ring slot
+    CdView v;
+    v.tx = threadIdx.x & (CD_TX - 1);
+    v.ty = threadIdx.x / CD_TX;
     for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
-        int c0, c1, c2;
-        if (!tile_cell(T, tile, c0, c1, c2)) continue;
-        int64_t id = gidx(g, c0, c1, c2);
-        Sten<ND> S;
-        S.set(g, c0, c1, c2);
-        blend_comp<ND, 0>(P, w, u0, mu0, mu1, out, S, id, dt, V0, corrector);
-        blend_comp<ND, 1>(P, w, u0, mu0, mu1, out, S, id, dt, V1, corrector);
-        if (ND == 3) blend_comp<ND, 2>(P, w, u0, mu0, mu1, out, S, id, dt, V2, corrector);
-        // the corrector leaves the convective-exit plane at the predictor's value (R-N); the
-        // output is another buffer, so carry the plane over
-        if (corrector && P.exit_bc && c0 == g.n[0]) out[id + 1] = w[id + 1];
+        const int tix = tile % T.ntx, rem = tile / T.ntx;
+        const int tiy = rem % T.nty, tiz = rem / T.nty;
+        const int bx = 1 + 4 * CD_TX * tix, by = 1 + CD_TY * tiy;
+        const int z0 = ND == 3 ? 1 + T.zc * tiz : 0;
+        const int z1 = ND == 3 ? min(z0 + T.zc - 1, g.n[2]) : 0;
+        const int gx = bx + 4 * v.tx, gy = by + v.ty;
+        int nv = g.n[0] - gx + 1;
+        nv = nv > 4 ? 4 : nv;
+        if (gy > g.n[1]) nv = 0;
+        __syncthreads();                           // the previous tile's reads are done
+        {
+            float4 st[CD_STAGE(ND)];
+#pragma unroll 1
+            for (int d = 0; d < NP; ++d) {
+                const int cz = ND == 3 ? src_coord(z0 - 2 + d, g.n[2], g.per[2]) : 0;
+                cd_load_regs<ND>(g, w, bx, by, cz, st);
+                cd_store_regs<ND>(ring + d * SLOT, st);
+            }
+        }
+        __syncthreads();
+        int s0 = 0;                                // ring slot of plane z-2
+#pragma unroll 1
+        for (int z = z0; z <= z1; ++z) {
+            float4 st[CD_STAGE(ND)];
+            const bool more = ND == 3 && z < z1;
+            if (more) cd_load_regs<ND>(g, w, bx, by, src_coord(z + 3, g.n[2], g.per[2]), st);
+#pragma unroll
+            for (int d = 0; d < NP; ++d) {
+                int s = s0 + d;
+                if (s >= NP) s -= NP;
+#pragma unroll
+                for (int c = 0; c < ND; ++c) v.p[c][ND == 3 ? d : 2] = ring + s * SLOT + c * CD_PLANE;
+            }
+            cd_comp<ND, 0>(P, v, gx, gy, z, nv, u0, mu0, w, out, dt, V0, corrector);
+            cd_comp<ND, 1>(P, v, gx, gy, z, nv, u0, mu0, w, out, dt, V1, corrector);
+            if (ND == 3) cd_comp<ND, 2>(P, v, gx, gy, z, nv, u0, mu0, w, out, dt, V2, corrector);
+            if (more) {
+                __syncthreads();
+                cd_store_regs<ND>(ring + s0 * SLOT, st);
+                s0 = s0 + 1 == NP ? 0 : s0 + 1;
+                __syncthreads();
+            }
+        }
     }
+}
+
+// ====================================================================== the band kernel
+template <int ND, int I>
+__device__ __forceinline__ void band_face(const FlowP& P, const float* __restrict__ w, const float* __restrict__ u0,
+                                          const float* __restrict__ mu1, float* __restrict__ out, int c0, int c1, int c2,
+                                          float dt, float Vi, float scale)
+{
+    const Grid& g = P.g;
+    const int64_t id = gidx(g, c0, c1, c2);
+    float acc = 0.0f;
+    bool any = false;
+#pragma unroll
+    for (int j = 0; j < ND; ++j) {
+        const float m1 = mu1[(I * ND + j) * g.nalloc + id];
+        if (m1 == 0.0f) continue;
+        int cp[3] = { c0, c1, c2 }, cm[3] = { c0, c1, c2 };
+        cp[j] += 1; cm[j] -= 1;
+        const float fp = f_at<ND, I>(P, w, u0, dt, Vi, cp[0], cp[1], cp[2]);
+        const float fm = f_at<ND, I>(P, w, u0, dt, Vi, cm[0], cm[1], cm[2]);
+        acc += m1 * 0.5f * (fp - fm);
+        any = true;
+    }
+    if (any) out[I * g.nalloc + id] += scale * acc;
+}
+
+template <int ND>
+__global__ void __launch_bounds__(128) k_cd_band(FlowP P, const float* __restrict__ w, const float* __restrict__ u0,
+                                                 const float* __restrict__ mu1, float* __restrict__ out,
+                                                 const DevScal* __restrict__ ds, const long long* __restrict__ list, int cap, int corrector)
+{
+    const Grid& g = P.g;
+    const float dt = ds->dt;
+    const float V[3] = { ds->vel[0], ds->vel[1], ds->vel[2] };
+    const float scale = corrector ? 0.5f : 1.0f;
+    const int cnt = ds->band_count;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x, t0 = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (cnt <= cap) {
+        for (int64_t e = t0; e < cnt; e += stride) {
+            const long long code = list[e];
+            const int i = (int)(code & 3);
+            int64_t q = (code >> 2) - WL_OFF;
+            const int c2 = ND == 3 ? (int)(q / g.sz) : 0;
+            if (ND == 3) q -= (int64_t)c2 * g.sz;
+            const int c1 = (int)(q / g.sy), c0 = (int)(q - (int64_t)c1 * g.sy);
+            if (i == 0) band_face<ND, 0>(P, w, u0, mu1, out, c0, c1, c2, dt, V[0], scale);
+            else if (i == 1) band_face<ND, 1>(P, w, u0, mu1, out, c0, c1, c2, dt, V[1], scale);
+            else if (ND == 3) band_face<ND, 2>(P, w, u0, mu1, out, c0, c1, c2, dt, V[2], scale);
+        }
+    } else {
+        // the list overflowed (a body far larger than the capacity heuristic): scan every interior face
+        const int64_t n01 = (int64_t)g.n[0] * g.n[1], tot = n01 * g.n[2];
+        for (int64_t e = t0; e < tot; e += stride) {
+            const int c2 = ND == 3 ? 1 + (int)(e / n01) : 0;
+            const int64_t q = e % n01;
+            const int c1 = 1 + (int)(q / g.n[0]), c0 = 1 + (int)(q % g.n[0]);
+            band_face<ND, 0>(P, w, u0, mu1, out, c0, c1, c2, dt, V[0], scale);
+            band_face<ND, 1>(P, w, u0, mu1, out, c0, c1, c2, dt, V[1], scale);
+            if (ND == 3) band_face<ND, 2>(P, w, u0, mu1, out, c0, c1, c2, dt, V[2], scale);
+        }
+    }
+}
+
+// ====================================================================== host launcher
+static CdT cd_tiling(const wl_sim* s, const Grid& g)
+{
+    CdT T;
+    T.ntx = (g.n[0] + 4 * CD_TX - 1) / (4 * CD_TX);
+    T.nty = (g.n[1] + CD_TY - 1) / CD_TY;
+    T.zc = 1; T.ntz = 1;
+    if (s->nd == 3) {
+        // planes per tile: long marches amortise the four halo planes; keep >= ~6 tiles per resident block
+        int zc = 32;
+        while (zc > 8 && (int64_t)T.ntx * T.nty * ((g.n[2] + zc - 1) / zc) < (int64_t)s->sm_count * 12) zc /= 2;
+        if (zc > g.n[2]) zc = g.n[2];
+        T.zc = zc;
+        T.ntz = (g.n[2] + zc - 1) / zc;
+    }
+    T.ntiles = T.ntx * T.nty * T.ntz;
+    return T;
 }
 
 void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out, int corrector)
 {
     FlowP P = wl_flowp(s);
-    Tiling T = wl_tiles_interior(s, P.g);
-    ProfScope ps(s, WLK_CONVDIFF);
-    if (s->nd == 3)
-        k_conv_diff_bdim<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(P, T, w, u0, s->mu0, s->mu1, out, s->ds, corrector);
-    else
-        k_conv_diff_bdim<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(P, T, w, u0, s->mu0, s->mu1, out, s->ds, corrector);
+    CdT T = cd_tiling(s, P.g);
+    const size_t smem = sizeof(float) * (size_t)(s->nd == 3 ? CD_NP : 1) * s->nd * CD_PLANE;
+    if (!s->cd_attr_set) {
+        cudaFuncSetAttribute(k_cd_tile<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * CD_NP * 3 * CD_PLANE));
+        cudaFuncSetAttribute(k_cd_tile<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * 2 * CD_PLANE));
+        s->cd_attr_set = 1;
+    }
+    {
+        ProfScope ps(s, WLK_CONVDIFF);
+        if (s->nd == 3) k_cd_tile<3><<<T.ntiles, CD_NT, smem, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
+        else            k_cd_tile<2><<<T.ntiles, CD_NT, smem, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
+    }
+    if (s->cfg.body.kind != WL_BODY_NONE) {
+        ProfScope ps(s, WLK_CONVDIFF_BAND);
+        const int blocks = s->sm_count * 8;
+        if (s->nd == 3) k_cd_band<3><<<blocks, 128, 0, s->st>>>(P, w, u0, s->mu1, out, s->ds, s->band_list, s->band_cap, corrector);
+        else            k_cd_band<2><<<blocks, 128, 0, s->st>>>(P, w, u0, s->mu1, out, s->ds, s->band_list, s->band_cap, corrector);
+    }
 }

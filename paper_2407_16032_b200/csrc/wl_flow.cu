@@ -34,7 +34,8 @@ __global__ void k_set_time(DevScal* ds, wl_body b, double t_host, float dt_host,
 // problem).  V is a uniform vector for the translation maps supported and lives in DevScal.
 template <int ND>
 __global__ void __launch_bounds__(512) k_measure(Grid g, Tiling T, BodyP b, const DevScal* __restrict__ ds,
-                                                 float* __restrict__ mu0, float* __restrict__ mu1)
+                                                 float* __restrict__ mu0, float* __restrict__ mu1,
+                                                 DevScal* dsw, long long* __restrict__ band, int band_cap)
 {
     double ctr[3] = { ds->centre[0], ds->centre[1], ds->centre[2] };
     for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
@@ -60,8 +61,22 @@ __global__ void __launch_bounds__(512) k_measure(Grid g, Tiling T, BodyP b, cons
             }
             if (!g.per[i] && (c[i] == 1 || c[i] == g.n[i] + 1)) m0 = 0.0f;
             mu0[i * g.nalloc + id] = m0;
+            bool any = false;
 #pragma unroll
-            for (int j = 0; j < ND; ++j) mu1[(i * ND + j) * g.nalloc + id] = m1 * nrm[j];
+            for (int j = 0; j < ND; ++j) {
+                const float v = m1 * nrm[j];
+                mu1[(i * ND + j) * g.nalloc + id] = v;
+                any = any || v != 0.0f;
+            }
+            // the band list of conv_diff!/BDIM!: interior faces whose mu1 is non-zero (entry order is
+            // irrelevant: every entry is processed independently)
+            bool inner = true;
+#pragma unroll
+            for (int k = 0; k < ND; ++k) inner = inner && c[k] >= 1 && c[k] <= g.n[k];
+            if (any && inner) {
+                const int slot = atomicAdd(&dsw->band_count, 1);
+                if (slot < band_cap) band[slot] = ((long long)id << 2) | i;
+            }
         }
     }
 }
@@ -284,10 +299,11 @@ void wl_k_measure(wl_sim* s)
 {
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_padded(s, g);
+    cudaMemsetAsync(&s->ds->band_count, 0, sizeof(int), s->st);
     {
         ProfScope ps(s, WLK_MEASURE);
-        if (s->nd == 3) k_measure<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1);
-        else            k_measure<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1);
+        if (s->nd == 3) k_measure<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1, s->ds, s->band_list, s->band_cap);
+        else            k_measure<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1, s->ds, s->band_list, s->band_cap);
     }
     wl_k_poisson_update(s);
 }

@@ -11,7 +11,7 @@
 enum WlKern {
     WLK_SET_TIME, WLK_MEASURE, WLK_POISSON_UPDATE, WLK_CONVDIFF, WLK_BC, WLK_EXIT_BC, WLK_RESIDUAL,
     WLK_RESTRICT, WLK_PROLONG, WLK_PCG_INIT, WLK_PCG_MATVEC, WLK_PCG_UPDATE, WLK_PCG_DIR,
-    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_COUNT
+    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_CONVDIFF_BAND, WLK_COUNT
 };
 struct ProfRec { cudaEvent_t a, b; int cls; };
 
@@ -40,6 +40,9 @@ struct wl_sim {
     float* p;                // pressure (unscaled)
     float* mu0;              // nd comps
     float* mu1;              // nd*nd comps
+    long long* band_list;    // faces with mu1 != 0, written by measure!: (array offset << 2) | component
+    int band_cap;            // capacity of band_list (entries)
+    int cd_attr_set;         // dynamic shared-memory attribute of the conv_diff kernels is set
     DevScal* ds;             // device-resident scalars
     DevScal* hs;             // pinned host mirror for read-back
     RedBuf rb;
