@@ -583,6 +583,13 @@ static double level_maxabs_r(const wlo_sim *s, const wlo_level *g)
  * by round-off (alpha = rho/gamma) and blows up -- in fp32 already on the 8x8 level of the
  * 2-D Taylor-Green case, whose residual is a single eigenmode (converged after two iterations).
  * A relative test makes the fp64 oracle and an fp32 implementation take the same branch.
+ * Reading R-T2 (compatibility): A is singular -- constants span its null space, buried cells
+ * (D = 0, iD = 0) are decoupled -- so A x = r has a solution only for a residual orthogonal to
+ * the constants.  Before the iteration the mean of r over the coupled cells (iD != 0) is
+ * removed from those cells.  In exact arithmetic that mean is zero (sum div u = boundary flux
+ * = 0, sum A x = 0, restriction and prolongation preserve sums); in floating point it is
+ * round-off, and CG on it diverges once the rest of r has converged below it (alpha = rho/gamma
+ * with rho held up by the null-space part while gamma, which cannot see it, goes to zero).
  * `q` doubles as the z work array.
  */
 #define WLO_TAU 1e-30
@@ -591,6 +598,24 @@ void wlo_smooth(wlo_sim *s, int l, int its)
 {
     wlo_level *g = &s->lev[l];
     int nd = s->nd;
+    {   /* R-T2: r <- r - mean(r) over the coupled cells */
+        double sum = 0, cnt = 0;
+#pragma omp parallel for collapse(2) reduction(+ : sum, cnt)
+        for (int c2 = ZLO(g, nd); c2 <= ZHI(g, nd); ++c2)
+            for (int c1 = 1; c1 <= g->n[1]; ++c1)
+                for (int c0 = 1; c0 <= g->n[0]; ++c0) {
+                    long id = IDX(g, c0, c1, c2);
+                    if (g->iD[id] != 0.0) { sum += g->r[id]; cnt += 1.0; }
+                }
+        double m = cnt > 0 ? sum / cnt : 0.0;
+#pragma omp parallel for collapse(2)
+        for (int c2 = ZLO(g, nd); c2 <= ZHI(g, nd); ++c2)
+            for (int c1 = 1; c1 <= g->n[1]; ++c1)
+                for (int c0 = 1; c0 <= g->n[0]; ++c0) {
+                    long id = IDX(g, c0, c1, c2);
+                    if (g->iD[id] != 0.0) g->r[id] -= m;
+                }
+    }
     double rho = level_dot_riDr(s, g, g->e);    /* z = e = iD r ; rho = r.z */
     double rho0 = rho;
     if (fabs(rho) < WLO_TAU) return;

@@ -234,6 +234,37 @@ def test_smoother_guards():
     s.close()
 
 
+def test_smoother_removes_the_incompatible_part_of_the_residual():
+    """R-T2: constants span the null space of A (per coupled region; buried cells are decoupled), so the
+    smoother works on r - mean(r over coupled cells).  A residual shifted by a constant on the coupled
+    cells must give the same x and leave the same (mean-free) r; on a tiny periodic grid, CG on a
+    residual that is ONLY a constant must not move x at all (without the projection alpha = rho/0)."""
+    cfg = wi.sphere((32, 16, 16), D=8.0, centre=(8.0, 8.0, 8.0))
+    out = []
+    for shift in (0.0, 0.37):
+        s = wo.OracleSim(cfg)
+        live = s.interior("iD")[0] != 0
+        assert (~live).sum() > 0                      # the body buries some cells
+        r = wi.random_scalar((32, 16, 16), seed=21)
+        r[~live] = 0.0
+        r[live] += shift - r[live].mean()
+        s.interior("r")[0][...] = r
+        s.arr("x")[...] = 0.0
+        s.smooth(0, 6)
+        out.append((s.interior("x").copy(), s.interior("r").copy(), live))
+        s.close()
+    (x0, r0, live), (x1, r1, _) = out
+    assert np.abs(x0).max() > 1e-3
+    assert np.allclose(x1, x0, atol=1e-12) and np.allclose(r1, r0, atol=1e-12)
+    assert abs(r1[0][live].mean()) < 1e-14 and np.all(r1[0][~live] == 0.0)
+    s = wo.OracleSim(wi.make(ndim=2, dims=(4, 4), periodic=(1, 1), U=(0.0,) * 3))
+    s.interior("r")[0, 0][...] = 0.25
+    s.arr("x")[...] = 0.0
+    s.smooth(0, 6)
+    assert np.all(s.interior("x") == 0.0) and np.abs(s.interior("r")).max() < 1e-16
+    s.close()
+
+
 def test_restrict_prolong_definitions():
     s = wo.OracleSim(wi.tgv3d(8, max_levels=2))
     g = wi.rng(13)
