@@ -88,7 +88,9 @@ static Grid make_grid(int nd, const int* n, const int* per)
     return g;
 }
 
-static VT make_vt(int nd, const Grid& g)
+// Vector tiling of a level.  Coarse levels are latency-bound, not bandwidth-bound: they take fewer
+// planes per tile so that enough tiles (>= 4 per SM of a 148-SM B200 where the level allows) are in flight.
+static VT make_vt(int nd, const Grid& g, int level)
 {
     VT t;
     t.ngx = (g.n[0] + 3) / 4;
@@ -98,6 +100,8 @@ static VT make_vt(int nd, const Grid& g)
     t.ntx = (t.ngx + lx - 1) / lx;
     t.nty = (g.n[1] + ly - 1) / ly;
     t.zc = nd == 3 ? (g.n[2] < 8 ? g.n[2] : 8) : 1;
+    if (level > 0)
+        while (t.zc > 1 && (int64_t)t.ntx * t.nty * ((g.n[2] + t.zc - 1) / t.zc) < 592) t.zc = (t.zc + 1) / 2;
     t.ntz = nd == 3 ? (g.n[2] + t.zc - 1) / t.zc : 1;
     t.ntiles = t.ntx * t.nty * t.ntz;
     return t;
@@ -135,6 +139,8 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
     DevScal* ds = (DevScal*)cv.take(sizeof(DevScal));
     double* partial = (double*)cv.take(sizeof(double) * 4 * WL_MAX_PARTIALS);
     unsigned int* counter = (unsigned int*)cv.take(256);
+    LevDev* levdev = (LevDev*)cv.take(sizeof(LevDev) * WL_MAXLEV);
+    double* pk_part = (double*)cv.take(sizeof(double) * 2 * 2 * WL_MAX_PARTIALS);
     Grid g0 = make_grid(nd, dims[0], c->periodic);
     size_t sc = sizeof(float) * (size_t)g0.nalloc;
     float* ub[3];
@@ -151,6 +157,7 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
     long long* band = (long long*)cv.take(sizeof(long long) * (size_t)bcap);
     if (s) {
         s->ds = ds; s->rb.partial = partial; s->rb.counter = counter;
+        s->levdev = levdev; s->pk_part = pk_part;
         for (int k = 0; k < 3; ++k) s->ubuf[k] = ub[k];
         s->p = p; s->mu0 = mu0; s->mu1 = mu1;
         s->band_list = band; s->band_cap = (int)bcap;
@@ -166,7 +173,7 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
         float* e = (float*)cv.take(scl);
         float* e2 = (float*)cv.take(scl);
         float* q = (float*)cv.take(scl);
-        VT vt = make_vt(nd, g);
+        VT vt = make_vt(nd, g, l);
         int* plain = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
         int* uniform = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
         if (s) {
@@ -281,6 +288,15 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     s->st = (cudaStream_t)cuda_stream;
     layout(s, cfg, dev_ws);
     s->u = s->ubuf[0]; s->u0 = s->ubuf[1]; s->ut = s->ubuf[2];
+    {   // levels that run inside the persistent coarse-level kernel: from the first level >= 1 small enough
+        long long maxc = 6000000;
+        if (const char* e = getenv("WL_PK_MAX_CELLS")) maxc = atoll(e);
+        s->pk_level = s->nlev;
+        for (int l = s->nlev - 1; l >= 1; --l) {
+            const Grid& g = s->lev[l].g;
+            if ((long long)g.n[0] * g.n[1] * g.n[2] <= maxc) s->pk_level = l; else break;
+        }
+    }
     s->body.kind = cfg->body.kind; s->body.axis = cfg->body.axis;
     s->body.R = cfg->body.R; s->body.r = cfg->body.r; s->body.eps = cfg->eps;
     int dev = 0;
@@ -293,6 +309,15 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     if (cudaMallocHost((void**)&s->hs, sizeof(DevScal)) != cudaSuccess) { delete s; return WL_ECUDA; }
     memset(s->hs, 0, sizeof(DevScal));
     if (cudaMemsetAsync(dev_ws, 0, need, s->st) != cudaSuccess) { cudaFreeHost(s->hs); delete s; return WL_ECUDA; }
+    LevDev hl[WL_MAXLEV];
+    memset(hl, 0, sizeof(hl));
+    for (int l = 0; l < s->nlev; ++l) {
+        const Level& lv = s->lev[l];
+        LevDev& d = hl[l];
+        d.g = lv.g; d.vt = lv.vt; d.L = lv.L; d.iD = lv.iD; d.x = lv.x; d.r = lv.r; d.e = lv.e; d.e2 = lv.e2; d.q = lv.q;
+        d.plain = lv.plain; d.Lc = lv.Lc; d.iDc = lv.iDc;
+    }
+    if (cudaMemcpyAsync(s->levdev, hl, sizeof(hl), cudaMemcpyHostToDevice, s->st) != cudaSuccess) { cudaFreeHost(s->hs); delete s; return WL_ECUDA; }
     // initial state (R-V): u = U everywhere (all three buffers, so the exit plane is defined), p = 0, measure(0)
     for (int k = 0; k < 3; ++k) wl_k_fill_u(s, s->ubuf[k]);
     wl_k_set_time(s, 0.0, cfg->dt0, 1, 1);
@@ -461,7 +486,7 @@ extern "C" int wl_level_dims(const wl_sim* s, int level, int dims_out[3])
 // ---- per-kernel-class timing (CUDA events on the handle's stream)
 static const char* const kern_names[WLK_COUNT] = {
     "set_time", "measure", "poisson_update", "conv_diff_bdim", "bc", "exit_bc", "residual", "restrict", "prolong",
-    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc", "conv_diff_band"
+    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc", "conv_diff_band", "vcycle"
 };
 
 extern "C" int wl_prof_enable(wl_sim* s, int enable)
@@ -543,8 +568,40 @@ extern "C" int wl_dbg_residual(wl_sim* s)
 extern "C" int wl_dbg_apply_gradient(wl_sim* s) { if (!s) return WL_EINVAL; wl_k_apply_gradient(s, s->u); return check(s); }
 extern "C" int wl_dbg_restrict(wl_sim* s, int l) { if (!s || l < 0 || l + 1 >= s->nlev) return WL_EINVAL; wl_k_restrict(s, l); return check(s); }
 extern "C" int wl_dbg_prolong(wl_sim* s, int l) { if (!s || l < 0 || l + 1 >= s->nlev) return WL_EINVAL; wl_k_prolong(s, l); return check(s); }
-extern "C" int wl_dbg_smooth(wl_sim* s, int l, int iters) { if (!s || l < 0 || l >= s->nlev || iters < 1) return WL_EINVAL; wl_k_smooth(s, l, iters); return check(s); }
+extern "C" int wl_dbg_smooth(wl_sim* s, int l, int iters)
+{
+    if (!s || l < 0 || l >= s->nlev || iters < 1) return WL_EINVAL;
+    wl_k_rsum(s, l);          // in a solve the kernel that wrote r leaves this sum
+    wl_k_smooth(s, l, iters);
+    return check(s);
+}
 extern "C" int wl_dbg_vcycle(wl_sim* s, int l) { if (!s || l < 0 || l >= s->nlev) return WL_EINVAL; wl_k_vcycle(s, l); return check(s); }
+
+// runs n coarse-level passes (kind: 0 restrict level->level+1, 1 smooth, 2 prolong level+1->level) as ONE k_coarse launch
+extern "C" int wl_dbg_coarse_prog(wl_sim* s, int n, const int* kinds, const int* levels, const int* iters)
+{
+    if (!s || n < 1 || n > 3 * WL_MAXLEV || !kinds || !levels || !iters) return WL_EINVAL;
+    CoarseProg P; P.n = n;
+    for (int k = 0; k < n; ++k) {
+        const int top = kinds[k] == COP_SMOOTH ? s->nlev - 1 : s->nlev - 2;
+        if (kinds[k] < 0 || kinds[k] > 2 || levels[k] < 0 || levels[k] > top || (kinds[k] == COP_SMOOTH && iters[k] < 1)) return WL_EINVAL;
+        P.op[k].kind = kinds[k]; P.op[k].level = levels[k]; P.op[k].iters = iters[k];
+    }
+    wl_k_coarse_prog(s, P);
+    return check(s);
+}
+
+// PCG scalars of a level: rho, gamma, alpha, beta, rho0, rsum, nlive, live
+extern "C" int wl_dbg_pcg_scalars(wl_sim* s, int level, double out[8])
+{
+    if (!s || level < 0 || level >= s->nlev || !out) return WL_EINVAL;
+    PcgScal h;
+    WL_CUDA_CHECK(s, cudaMemcpyAsync(&h, &s->ds->pcg[level], sizeof(PcgScal), cudaMemcpyDeviceToHost, s->st));
+    int rc = sync(s);
+    if (rc != WL_OK) return rc;
+    out[0] = h.rho; out[1] = h.gamma; out[2] = h.alpha; out[3] = h.beta; out[4] = h.rho0; out[5] = h.rsum; out[6] = h.nlive; out[7] = (double)h.live;
+    return WL_OK;
+}
 
 static int find_array(wl_sim* s, const char* name, int level, float** arr, int* ncomp, const Grid** g)
 {

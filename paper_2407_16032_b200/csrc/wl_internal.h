@@ -11,7 +11,7 @@
 enum WlKern {
     WLK_SET_TIME, WLK_MEASURE, WLK_POISSON_UPDATE, WLK_CONVDIFF, WLK_BC, WLK_EXIT_BC, WLK_RESIDUAL,
     WLK_RESTRICT, WLK_PROLONG, WLK_PCG_INIT, WLK_PCG_MATVEC, WLK_PCG_UPDATE, WLK_PCG_DIR,
-    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_CONVDIFF_BAND, WLK_COUNT
+    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_CONVDIFF_BAND, WLK_COARSE, WLK_COUNT
 };
 struct ProfRec { cudaEvent_t a, b; int cls; };
 
@@ -31,6 +31,19 @@ struct Level {
     float iDc;   // 1 / (-2 n Lc)
 };
 
+// device-side copy of a level (array in the workspace, read by the persistent coarse-level kernel)
+struct LevDev {
+    Grid g; VT vt;
+    float *L, *iD, *x, *r, *e, *e2, *q;
+    int* plain;
+    float Lc, iDc;
+};
+
+// a chain of coarse-level passes run by one k_coarse launch
+enum { COP_RESTRICT = 0, COP_SMOOTH = 1, COP_PROLONG = 2 };   // RESTRICT: level -> level+1; PROLONG: level+1 -> level
+struct CoarseOp { int kind, level, iters; };
+struct CoarseProg { int n; CoarseOp op[3 * WL_MAXLEV]; };
+
 struct wl_sim {
     wl_config cfg;
     int nd, nlev;
@@ -46,6 +59,10 @@ struct wl_sim {
     DevScal* ds;             // device-resident scalars
     DevScal* hs;             // pinned host mirror for read-back
     RedBuf rb;
+    LevDev* levdev;          // device array [nlev]
+    double* pk_part;         // per-block partial sums of k_coarse
+    int pk_level;            // levels >= pk_level run inside k_coarse (nlev: none)
+    int pk_blocks;           // co-resident grid of k_coarse (0: not yet queried)
     BodyP body;
     cudaStream_t st;
     int launches;
@@ -118,6 +135,8 @@ void wl_k_residual(wl_sim* s, const float* u, float w);   // pscale = w*dt; x = 
 void wl_k_restrict(wl_sim* s, int l);                // r_{l+1} = sum children r_l ; x_{l+1} = 0
 void wl_k_prolong(wl_sim* s, int l);                 // x_l += P x_{l+1}; r_l -= A_l P x_{l+1}
 void wl_k_smooth(wl_sim* s, int l, int iters);
+void wl_k_coarse_prog(wl_sim* s, const CoarseProg& P);   // one k_coarse launch
+void wl_k_rsum(wl_sim* s, int l);                    // pcg[l].rsum = sum of r over the coupled cells (stage hooks)
 void wl_k_vcycle(wl_sim* s, int l);
 void wl_k_apply_gradient(wl_sim* s, float* u);       // u -= L grad x ; p = x / pscale
 void wl_k_resmax(wl_sim* s);                         // ds->resmax = max |r_0|

@@ -56,12 +56,15 @@ __device__ __forceinline__ VPos vt_pos(const Grid& g, const VT& t, int tile)
     return p;
 }
 
-__device__ __forceinline__ float4 ld4(const float* __restrict__ a, int64_t i)
+// Plain (coherent) loads: the same tile functions run inside the persistent coarse-level kernel,
+// where arrays written in an earlier phase by another block are read after a grid barrier; the
+// non-coherent path (__ldg) is not allowed there.  In the stand-alone kernels the pointers are
+// const __restrict__ kernel parameters and the compiler selects the read-only path itself.
+__device__ __forceinline__ float4 ld4(const float* a, int64_t i)
 {
-    return __ldg(reinterpret_cast<const float4*>(a + i));
+    return *reinterpret_cast<const float4*>(a + i);
 }
-// loads of arrays that another block of the SAME kernel may be writing are not allowed through
-// the non-coherent path; none of the kernels here does that (outputs go to other buffers).
+__device__ __forceinline__ float ld1(const float* a, int64_t i) { return a[i]; }
 
 __device__ __forceinline__ void st4(float* __restrict__ a, int64_t i, const float (&v)[4], int nv)
 {
