@@ -297,6 +297,8 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
             if ((long long)g.n[0] * g.n[1] * g.n[2] <= maxc) s->pk_level = l; else break;
         }
     }
+    s->fast_A = 1;
+    if (const char* e = getenv("WL_FAST_A")) s->fast_A = atoi(e) != 0;
     s->body.kind = cfg->body.kind; s->body.axis = cfg->body.axis;
     s->body.R = cfg->body.R; s->body.r = cfg->body.r; s->body.eps = cfg->eps;
     int dev = 0;
@@ -486,7 +488,7 @@ extern "C" int wl_level_dims(const wl_sim* s, int level, int dims_out[3])
 // ---- per-kernel-class timing (CUDA events on the handle's stream)
 static const char* const kern_names[WLK_COUNT] = {
     "set_time", "measure", "poisson_update", "conv_diff_bdim", "bc", "exit_bc", "residual", "restrict", "prolong",
-    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc", "conv_diff_band", "vcycle"
+    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc", "conv_diff_band", "vcycle", "pcg_matvec_gen"
 };
 
 extern "C" int wl_prof_enable(wl_sim* s, int enable)
@@ -589,6 +591,14 @@ extern "C" int wl_dbg_coarse_prog(wl_sim* s, int n, const int* kinds, const int*
     }
     wl_k_coarse_prog(s, P);
     return check(s);
+}
+
+// pass start times (ns, %globaltimer) of the last k_coarse launch: n+1 values for n passes
+extern "C" int wl_dbg_coarse_times(wl_sim* s, unsigned long long* out, int n)
+{
+    if (!s || !out || n < 1 || n > 3 * WL_MAXLEV + 1) return WL_EINVAL;
+    WL_CUDA_CHECK(s, cudaMemcpyAsync(out, s->ds->pk_t, sizeof(unsigned long long) * n, cudaMemcpyDeviceToHost, s->st));
+    return sync(s);
 }
 
 // PCG scalars of a level: rho, gamma, alpha, beta, rho0, rsum, nlive, live

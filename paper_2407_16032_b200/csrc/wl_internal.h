@@ -11,7 +11,7 @@
 enum WlKern {
     WLK_SET_TIME, WLK_MEASURE, WLK_POISSON_UPDATE, WLK_CONVDIFF, WLK_BC, WLK_EXIT_BC, WLK_RESIDUAL,
     WLK_RESTRICT, WLK_PROLONG, WLK_PCG_INIT, WLK_PCG_MATVEC, WLK_PCG_UPDATE, WLK_PCG_DIR,
-    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_CONVDIFF_BAND, WLK_COARSE, WLK_COUNT
+    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_CONVDIFF_BAND, WLK_COARSE, WLK_PCG_MATVEC_GEN, WLK_COUNT
 };
 struct ProfRec { cudaEvent_t a, b; int cls; };
 
@@ -63,6 +63,7 @@ struct wl_sim {
     double* pk_part;         // per-block partial sums of k_coarse
     int pk_level;            // levels >= pk_level run inside k_coarse (nlev: none)
     int pk_blocks;           // co-resident grid of k_coarse (0: not yet queried)
+    int fast_A;              // uniform tiles of PCG pass A go through k_pcg_A_fast (env WL_FAST_A=0 switches it off)
     BodyP body;
     cudaStream_t st;
     int launches;
@@ -129,6 +130,9 @@ void wl_k_pack(wl_sim* s, const Grid& g, const float* padded, float* dense, int 
 void wl_k_unpack(wl_sim* s, const Grid& g, const float* interior, float* padded, int ncomp);
 // wl_convdiff.cu
 void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out, int corrector);
+// wl_pcgfast.cu
+int wl_pcg_fast_ok(const wl_sim* s, int l);
+void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout, int finalize);
 // wl_poisson.cu
 void wl_k_poisson_update(wl_sim* s);                 // iD on level 0, coarse L and iD
 void wl_k_residual(wl_sim* s, const float* u, float w);   // pscale = w*dt; x = pscale*p; r = div u - A x

@@ -14,20 +14,21 @@
 // z = iD r is never stored.  Tiles flagged "plain" (all face coefficients equal the level
 // constant) skip the L and iD loads altogether.
 #include <cstdio>
+#include <cstdlib>
 #include "wl_internal.h"
 #include "wl_vec.cuh"
 #include <cooperative_groups.h>
 
-// ---------------------------------------------------------------- tile modes
-// Level::plain[tile] (written by k_diag_flags + k_plain_mode after every measure!):
-//   TM_GEN  general tile: face coefficients L and the inverse diagonal iD are loaded;
-//   TM_PLB  uniform tile (every face coefficient of the tile and of its face-neighbour tiles has its
-//           body-free value: Lc inside, 0 on a non-periodic domain boundary, R-O) that touches a
-//           non-periodic boundary: L and iD follow from the cell position alone, nothing is loaded;
-//   TM_PLI  uniform tile at least one cell away from every non-periodic boundary: L = Lc, iD = iDc.
-#define TM_GEN 0
-#define TM_PLB 1
-#define TM_PLI 2
+// minimum resident blocks per SM the register allocation aims at (tuned on B200, profiles/)
+#ifndef WL_A_MINB
+#define WL_A_MINB 2
+#endif
+#ifndef WL_B_MINB
+#define WL_B_MINB 4
+#endif
+#ifndef WL_PK_MINB
+#define WL_PK_MINB 2
+#endif
 
 // Position bookkeeping of one thread of a TM_PLB tile.  iD of a body-free cell with k boundary
 // faces is 1/(-(2 ND - k) Lc): the same correctly rounded quotient k_diag_flags stores.
@@ -636,10 +637,11 @@ __device__ __forceinline__ void pcgB_tile(const Grid& g, const VPos& p, float Lc
 }
 
 template <int ND, int FIRST>
-__global__ void __launch_bounds__(WL_VB) k_pcg_A(Grid g, VT vt, const int* __restrict__ plain, const float* __restrict__ L, float Lc, float iDc,
+__global__ void __launch_bounds__(WL_VB, WL_A_MINB) k_pcg_A(Grid g, VT vt, const int* __restrict__ plain, const float* __restrict__ L, float Lc, float iDc,
                                                  const float* __restrict__ ein, const float* __restrict__ r, const float* __restrict__ iD,
-                                                 float* __restrict__ eout, float* __restrict__ q, PcgScal* sc, RedBuf rb)
+                                                 float* __restrict__ eout, float* __restrict__ q, PcgScal* sc, RedBuf rb, int gen_only)
 {
+    // gen_only: the uniform tiles have been done by k_pcg_A_fast (wl_pcgfast.cu), which left its sums in sc->acc
     if (!FIRST && !sc->live) return;          // uniform across the grid: written by an earlier kernel
     const float beta = FIRST ? 0.0f : (float)sc->beta;
     const float m = FIRST ? pcg_mean(sc) : 0.0f;
@@ -647,12 +649,15 @@ __global__ void __launch_bounds__(WL_VB) k_pcg_A(Grid g, VT vt, const int* __res
     for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
         VPos p = vt_pos(g, vt, tile);
         if (p.nv == 0) continue;
+        const int mode = plain[tile];
+        if (gen_only && mode != TM_GEN) continue;
 #define CALL(M) pcgA_tile<ND, FIRST, M>(g, p, L, Lc, iDc, ein, r, iD, beta, m, eout, q, v[0], v[1])
-        TILE_MODES(plain[tile], CALL);
+        TILE_MODES(mode, CALL);
 #undef CALL
     }
     if (grid_reduce<2, OpSum>(v, rb)) {
         if (threadIdx.x == 0) {
+            if (gen_only) { v[0] += sc->acc[0]; v[1] += sc->acc[1]; }
             double gamma = v[0];
             int live = 1;
             if (FIRST) {
@@ -667,7 +672,7 @@ __global__ void __launch_bounds__(WL_VB) k_pcg_A(Grid g, VT vt, const int* __res
 }
 
 template <int ND>
-__global__ void __launch_bounds__(WL_VB) k_pcg_B(Grid g, VT vt, const int* __restrict__ plain, float Lc, float iDc, float* __restrict__ x, float* __restrict__ r,
+__global__ void __launch_bounds__(WL_VB, WL_B_MINB) k_pcg_B(Grid g, VT vt, const int* __restrict__ plain, float Lc, float iDc, float* __restrict__ x, float* __restrict__ r,
                                                  const float* __restrict__ e, const float* __restrict__ q, const float* __restrict__ iD,
                                                  PcgScal* sc, RedBuf rb, int first, int last)
 {
@@ -736,6 +741,13 @@ __global__ void __launch_bounds__(WL_VB) k_rsum(Grid g, VT vt, const int* __rest
 // products are summed from per-block partials in a fixed order by every block (bit-identical in all
 // blocks, so every block takes the same branches of the PCG guards).  The passes are the same tile
 // functions the fine-level kernels use.
+__device__ __forceinline__ unsigned long long globaltimer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
 struct PkCtx {
     double* part;        // [2][PK_NV][WL_MAX_PARTIALS] per-block partial sums, alternating by reduction
     int phase;
@@ -835,7 +847,7 @@ __device__ __forceinline__ void pk_smooth(PkCtx& c, const LevDev& lv, PcgScal* s
 }
 
 template <int ND>
-__global__ void __launch_bounds__(WL_VB, 2) k_coarse(const LevDev* levs, const __grid_constant__ CoarseProg prog, DevScal* ds, double* part)
+__global__ void __launch_bounds__(WL_VB, WL_PK_MINB) k_coarse(const LevDev* levs, const __grid_constant__ CoarseProg prog, DevScal* ds, double* part)
 {
     __shared__ LevDev la, lb;
     PkCtx c;
@@ -844,6 +856,7 @@ __global__ void __launch_bounds__(WL_VB, 2) k_coarse(const LevDev* levs, const _
     int rsum_level = -1;
     for (int o = 0; o < prog.n; ++o) {
         const CoarseOp op = prog.op[o];
+        if (blockIdx.x == 0 && threadIdx.x == 0) ds->pk_t[o] = globaltimer_ns();
         __syncthreads();
         if (threadIdx.x == 0) {     // level descriptors of this pass into shared memory (typed copies: no punning)
             la = levs[op.level];
@@ -881,6 +894,7 @@ __global__ void __launch_bounds__(WL_VB, 2) k_coarse(const LevDev* levs, const _
             if (blockIdx.x == 0 && threadIdx.x == 0) ds->pcg[op.level].rsum = v[0];
         }
     }
+    if (blockIdx.x == 0 && threadIdx.x == 0) ds->pk_t[prog.n] = globaltimer_ns();
 }
 
 // ================================================================== host launchers
@@ -939,7 +953,8 @@ static void coarse_launch(wl_sim* s, const CoarseProg& prog)
         int per_sm = 0;
         if (s->nd == 3) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_coarse<3>, WL_VB, 0);
         else            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_coarse<2>, WL_VB, 0);
-        if (per_sm > 2) per_sm = 2;
+        if (per_sm > WL_PK_MINB) per_sm = WL_PK_MINB;
+        if (const char* e = getenv("WL_PK_BPS")) { int v = atoi(e); if (v >= 1 && v < per_sm) per_sm = v; }
         if (per_sm < 1) per_sm = 1;
         int nb = per_sm * s->sm_count;
         if (nb > WL_MAX_PARTIALS) nb = WL_MAX_PARTIALS;
@@ -985,13 +1000,19 @@ void wl_k_smooth(wl_sim* s, int l, int iters)
     PcgScal* sc = &s->ds->pcg[l];
     float* ea = lv.e;      // direction written by the running A pass
     float* eb = lv.e2;     // previous direction
+    // uniform tiles of a 3-D level go through the shared-memory kernel; tiles cut by a body through k_pcg_A
+    const int fast = s->fast_A && wl_pcg_fast_ok(s, l);
+    const int has_body = s->cfg.body.kind != WL_BODY_NONE;
     for (int k = 1; k <= iters; ++k) {
-        if (k == 1)
-            VDISPATCH(s, WLK_PCG_MATVEC, l > 0, lv.vt, (k_pcg_A<2, 1>), (k_pcg_A<3, 1>), lv.g, lv.vt, lv.plain, lv.L, lv.Lc, lv.iDc,
-                      eb, lv.r, lv.iD, ea, lv.q, sc, s->rb);
+        if (fast) wl_k_pcg_A_fast(s, l, k == 1, eb, ea, !has_body);
+        const int gen_only = fast;
+        if (fast && !has_body) { /* no general tiles anywhere */ }
+        else if (k == 1)
+            VDISPATCH(s, fast ? WLK_PCG_MATVEC_GEN : WLK_PCG_MATVEC, l > 0, lv.vt, (k_pcg_A<2, 1>), (k_pcg_A<3, 1>), lv.g, lv.vt, lv.plain, lv.L, lv.Lc, lv.iDc,
+                      eb, lv.r, lv.iD, ea, lv.q, sc, s->rb, gen_only);
         else
-            VDISPATCH(s, WLK_PCG_MATVEC, l > 0, lv.vt, (k_pcg_A<2, 0>), (k_pcg_A<3, 0>), lv.g, lv.vt, lv.plain, lv.L, lv.Lc, lv.iDc,
-                      eb, lv.r, lv.iD, ea, lv.q, sc, s->rb);
+            VDISPATCH(s, fast ? WLK_PCG_MATVEC_GEN : WLK_PCG_MATVEC, l > 0, lv.vt, (k_pcg_A<2, 0>), (k_pcg_A<3, 0>), lv.g, lv.vt, lv.plain, lv.L, lv.Lc, lv.iDc,
+                      eb, lv.r, lv.iD, ea, lv.q, sc, s->rb, gen_only);
         VDISPATCH(s, WLK_PCG_UPDATE, l > 0, lv.vt, k_pcg_B<2>, k_pcg_B<3>, lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, lv.x, lv.r, ea, lv.q, lv.iD, sc, s->rb,
                   k == 1 ? 1 : 0, k == iters ? 1 : 0);
         float* t = ea; ea = eb; eb = t;

@@ -78,3 +78,15 @@ __device__ __forceinline__ void unpack4(const float4& v, float (&o)[4]) { o[0] =
 // row offsets of the y / z neighbours with periodic wrap (solver arrays keep no ghost values)
 __device__ __forceinline__ int nb_lo(int c, int n, int per) { return (c == 1 && per) ? n : c - 1; }
 __device__ __forceinline__ int nb_hi(int c, int n, int per) { return (c == n && per) ? 1 : c + 1; }
+
+// ---------------------------------------------------------------- tile modes
+// Level::plain[tile] (written by k_diag_flags + k_plain_mode after every measure!):
+//   TM_GEN  general tile: face coefficients L and the inverse diagonal iD are loaded;
+//   TM_PLB  uniform tile (every face coefficient of the tile and of its face-neighbour tiles has its
+//           body-free value: Lc inside, 0 on a non-periodic domain boundary, R-O) that touches a
+//           non-periodic boundary: L and iD follow from the cell position alone, nothing is loaded;
+//   TM_PLI  uniform tile at least one cell away from every non-periodic boundary: L = Lc, iD = iDc.
+#define TM_GEN 0
+#define TM_PLB 1
+#define TM_PLI 2
+
