@@ -289,7 +289,7 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     layout(s, cfg, dev_ws);
     s->u = s->ubuf[0]; s->u0 = s->ubuf[1]; s->ut = s->ubuf[2];
     {   // levels that run inside the persistent coarse-level kernel: from the first level >= 1 small enough
-        long long maxc = 6000000;
+        long long maxc = 1000000;
         if (const char* e = getenv("WL_PK_MAX_CELLS")) maxc = atoll(e);
         s->pk_level = s->nlev;
         for (int l = s->nlev - 1; l >= 1; --l) {
@@ -488,7 +488,7 @@ extern "C" int wl_level_dims(const wl_sim* s, int level, int dims_out[3])
 // ---- per-kernel-class timing (CUDA events on the handle's stream)
 static const char* const kern_names[WLK_COUNT] = {
     "set_time", "measure", "poisson_update", "conv_diff_bdim", "bc", "exit_bc", "residual", "restrict", "prolong",
-    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc", "conv_diff_band", "vcycle", "pcg_matvec_gen"
+    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc", "conv_diff_band", "vcycle"
 };
 
 extern "C" int wl_prof_enable(wl_sim* s, int enable)

@@ -46,7 +46,6 @@ __host__ __device__ __forceinline__ int wrapc(int c, int N, int per)
 // each one back).
 struct PcgScal {
     double rho, gamma, alpha, beta, rho0;
-    double acc[2];  // dot-product sums of the uniform tiles (k_pcg_A_fast), taken up by the general-tile kernel
     double rsum;    // sum of r over the coupled cells (iD != 0), left by the kernel that last wrote r (R-T2)
     double nlive;   // number of coupled cells of the level (k_diag_flags)
     int live;   // 0 once a guard of DESIGN.md R-T has fired: later kernels of this smoother call are no-ops

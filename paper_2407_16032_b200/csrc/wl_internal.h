@@ -11,7 +11,7 @@
 enum WlKern {
     WLK_SET_TIME, WLK_MEASURE, WLK_POISSON_UPDATE, WLK_CONVDIFF, WLK_BC, WLK_EXIT_BC, WLK_RESIDUAL,
     WLK_RESTRICT, WLK_PROLONG, WLK_PCG_INIT, WLK_PCG_MATVEC, WLK_PCG_UPDATE, WLK_PCG_DIR,
-    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_CONVDIFF_BAND, WLK_COARSE, WLK_PCG_MATVEC_GEN, WLK_COUNT
+    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_CONVDIFF_BAND, WLK_COARSE, WLK_COUNT
 };
 struct ProfRec { cudaEvent_t a, b; int cls; };
 
@@ -132,7 +132,7 @@ void wl_k_unpack(wl_sim* s, const Grid& g, const float* interior, float* padded,
 void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out, int corrector);
 // wl_pcgfast.cu
 int wl_pcg_fast_ok(const wl_sim* s, int l);
-void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout, int finalize);
+void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout);
 // wl_poisson.cu
 void wl_k_poisson_update(wl_sim* s);                 // iD on level 0, coarse L and iD
 void wl_k_residual(wl_sim* s, const float* u, float w);   // pscale = w*dt; x = pscale*p; r = div u - A x

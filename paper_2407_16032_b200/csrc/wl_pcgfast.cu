@@ -12,8 +12,8 @@
 // and the seven-point stencil reads its y neighbours from there, its x neighbours by shuffle and its z
 // neighbours from the thread's own registers.  Face coefficients and 1/D are analytic (tile modes
 // TM_PLI / TM_PLB, wl_vec.cuh): nothing but e and r is loaded.  General tiles (TM_GEN: a body or its
-// one-cell neighbourhood) are left to k_pcg_A of wl_poisson.cu, which adds its share of the dot
-// products to the sums this kernel leaves in PcgScal::acc.
+// one-cell neighbourhood, a few per cent of a level) take the same route; they load 1/D where e' is
+// formed and the face coefficients of their own cells where the stencil is applied, unprefetched.
 #include <cstdio>
 #include "wl_internal.h"
 
@@ -55,14 +55,15 @@ __device__ __forceinline__ float fa_dir(float ee, float rr, float d, float beta,
     return FIRST ? __fmul_rn(d, rr - m) : __fmaf_rn(beta, ee, __fmul_rn(d, rr));
 }
 
-// One tile.  PLB (static): the tile touches a non-periodic domain boundary, coefficients and 1/D depend on the
-// cell position; otherwise they are the constants Lc and iDc.  Everything that does not depend on the plane is
+// One tile.  MODE (static): TM_PLB, the tile touches a non-periodic domain boundary and coefficients and 1/D
+// depend on the cell position; TM_PLI, they are the constants Lc and iDc; TM_GEN, they are loaded.  Everything that does not depend on the plane is
 // computed once per tile; the stage of a plane rotates through FA_S slots without a division.
-template <int FIRST, bool PLB, int LXL>
+template <int FIRST, int MODE, int LXL>
 __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, float Lc, float iDc, const FaTab& T, float beta, float m,
-                                        const float* __restrict__ ein, const float* __restrict__ r, float* __restrict__ eout, float* __restrict__ q,
-                                        float* raw, float* ebuf, double (&acc)[2])
+                                        const float* __restrict__ ein, const float* __restrict__ r, const float* __restrict__ L, const float* __restrict__ iD,
+                                        float* __restrict__ eout, float* __restrict__ q, float* raw, float* ebuf, double (&acc)[2])
 {
+    constexpr bool PLB = MODE == TM_PLB, GEN = MODE == TM_GEN;
     constexpr int NA = FIRST ? 1 : 2;
     constexpr int LX = 1 << LXL, LY = WL_VB >> LXL;
     constexpr int RW = 4 * LX + 8, PL = RW * (LY + 2), SP = NA * PL;
@@ -134,6 +135,12 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
         const float* st = raw + slot * SP;
         float* eb = ebuf + (p & 1) * PL;
         const bool bz = PLB && fa_bnd(p, g.n[2], g.per[2]);     // block-uniform
+        const int zo = GEN ? fa_src(p, g.n[2], g.per[2]) * sz : 0;
+        if (GEN) {                            // a tile cut by a body: 1/D is loaded, at the positions the operands came from
+            if (own) unpack4(ld4(iD, off_own + zo), d_in);
+            if (full && hrow) unpack4(ld4(iD, off_h + zo), dh_in);
+            if (full && hcol) dx_in = ld1(iD, off_x + zo);
+        }
         if (!own) {
 #pragma unroll
             for (int k = 0; k < 4; ++k) { ep[k] = 0.0f; rm[k] = 0.0f; }
@@ -194,14 +201,35 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
         const float w[6] = { xm, zc[0], zc[1], zc[2], zc[3], xp };
         const float ymv[4] = { ym.x, ym.y, ym.z, ym.w }, ypv[4] = { yp.x, yp.y, yp.z, yp.w };
         float qq[4];
+        if (GEN) {                            // face coefficients of the own cells from L (= mu0 on level 0)
+            float lx[5] = { 0.f, 0.f, 0.f, 0.f, 0.f }, ly[4] = { 0.f, 0.f, 0.f, 0.f }, lyp[4] = { 0.f, 0.f, 0.f, 0.f };
+            float lz[4] = { 0.f, 0.f, 0.f, 0.f }, lzp[4] = { 0.f, 0.f, 0.f, 0.f };
+            if (valid) {
+                const int i = off_own + z * sz;
+                const float4 a = ld4(L, i);
+                lx[0] = a.x; lx[1] = a.y; lx[2] = a.z; lx[3] = a.w; lx[4] = ld1(L, i + 4);
+                unpack4(ld4(L + g.nalloc, i), ly); unpack4(ld4(L + g.nalloc, i + sy), lyp);
+                unpack4(ld4(L + 2 * g.nalloc, i), lz); unpack4(ld4(L + 2 * g.nalloc, i + sz), lzp);
+            }
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const float ec = w[k + 1];
-            float a = 0.0f;
-            a += cxh[k] * (w[k + 2] - ec) - cxl[k] * (ec - w[k]);
-            a += cyh * (ypv[k] - ec) - cyl * (ec - ymv[k]);
-            a += czh * (zp[k] - ec) - czl * (ec - zm[k]);
-            qq[k] = a;
+            for (int k = 0; k < 4; ++k) {
+                const float ec = w[k + 1];
+                float a = 0.0f;
+                a += lx[k + 1] * (w[k + 2] - ec) - lx[k] * (ec - w[k]);
+                a += lyp[k] * (ypv[k] - ec) - ly[k] * (ec - ymv[k]);
+                a += lzp[k] * (zp[k] - ec) - lz[k] * (ec - zm[k]);
+                qq[k] = a;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const float ec = w[k + 1];
+                float a = 0.0f;
+                a += cxh[k] * (w[k + 2] - ec) - cxl[k] * (ec - w[k]);
+                a += cyh * (ypv[k] - ec) - cyl * (ec - ymv[k]);
+                a += czh * (zp[k] - ec) - czl * (ec - zm[k]);
+                qq[k] = a;
+            }
         }
         if (valid) {
             const int i = off_own + z * sz;     // own row is interior here: fa_src(c1) == c1
@@ -227,7 +255,8 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
 template <int FIRST, int LXL>
 __global__ void __launch_bounds__(WL_VB, WL_FA_MINB) k_pcg_A_fast(Grid g, VT vt, const int* __restrict__ plain, float Lc, float iDc,
                                                           const float* __restrict__ ein, const float* __restrict__ r,
-                                                          float* __restrict__ eout, float* __restrict__ q, PcgScal* sc, RedBuf rb, int finalize)
+                                                          const float* __restrict__ L, const float* __restrict__ iD,
+                                                          float* __restrict__ eout, float* __restrict__ q, PcgScal* sc, RedBuf rb)
 {
     extern __shared__ float4 fa_smem4[];
     float* sm = reinterpret_cast<float*>(fa_smem4);
@@ -244,23 +273,21 @@ __global__ void __launch_bounds__(WL_VB, WL_FA_MINB) k_pcg_A_fast(Grid g, VT vt,
     double acc[2] = { 0.0, 0.0 };
     for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
         const int mode = plain[tile];         // block-uniform
-        if (mode == TM_PLI)      fa_tile<FIRST, false, LXL>(g, vt, tile, Lc, iDc, T, beta, m, ein, r, eout, q, raw, ebuf, acc);
-        else if (mode == TM_PLB) fa_tile<FIRST, true, LXL>(g, vt, tile, Lc, iDc, T, beta, m, ein, r, eout, q, raw, ebuf, acc);
+        if (mode == TM_PLI)      fa_tile<FIRST, TM_PLI, LXL>(g, vt, tile, Lc, iDc, T, beta, m, ein, r, L, iD, eout, q, raw, ebuf, acc);
+        else if (mode == TM_PLB) fa_tile<FIRST, TM_PLB, LXL>(g, vt, tile, Lc, iDc, T, beta, m, ein, r, L, iD, eout, q, raw, ebuf, acc);
+        else                     fa_tile<FIRST, TM_GEN, LXL>(g, vt, tile, Lc, iDc, T, beta, m, ein, r, L, iD, eout, q, raw, ebuf, acc);
     }
     if (grid_reduce<2, OpSum>(acc, rb)) {
         if (threadIdx.x == 0) {
-            if (!finalize) { sc->acc[0] = acc[0]; sc->acc[1] = acc[1]; }
-            else {
-                const double gamma = acc[0];
-                int live = 1;
-                if (FIRST) {
-                    sc->rho = acc[1]; sc->rho0 = acc[1]; sc->beta = 0.0;
-                    live = fabs(acc[1]) < WL_TAU ? 0 : 1;
-                }
-                sc->gamma = gamma;
-                if (gamma == 0.0 || !isfinite(gamma) || !live) { sc->live = 0; sc->alpha = 0.0; }
-                else { sc->live = 1; sc->alpha = sc->rho / gamma; }
+            const double gamma = acc[0];
+            int live = 1;
+            if (FIRST) {
+                sc->rho = acc[1]; sc->rho0 = acc[1]; sc->beta = 0.0;
+                live = fabs(acc[1]) < WL_TAU ? 0 : 1;
             }
+            sc->gamma = gamma;
+            if (gamma == 0.0 || !isfinite(gamma) || !live) { sc->live = 0; sc->alpha = 0.0; }
+            else { sc->live = 1; sc->alpha = sc->rho / gamma; }
         }
     }
 }
@@ -279,8 +306,8 @@ int wl_pcg_fast_ok(const wl_sim* s, int l)
     return s->nd == 3 && lv.g.n[0] % 4 == 0 && lv.g.nalloc < ((int64_t)1 << 31) && lv.vt.lxl >= 3 && lv.vt.lxl <= 5;
 }
 
-// pass A on the uniform tiles of level l; finalize = 0 leaves the sums in PcgScal::acc for the general-tile kernel
-void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout, int finalize)
+// pass A on level l (every tile mode)
+void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout)
 {
     Level& lv = s->lev[l];
     PcgScal* sc = &s->ds->pcg[l];
@@ -288,7 +315,7 @@ void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout,
     int grid = lv.vt.ntiles < s->sm_count * 4 ? lv.vt.ntiles : s->sm_count * 4;
     if (grid > WL_MAX_PARTIALS) grid = WL_MAX_PARTIALS;
     ProfScope ps_(s, WLK_PCG_MATVEC, l > 0);
-#define FA_LAUNCH(F, X) k_pcg_A_fast<F, X><<<grid, WL_VB, smem, s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, ein, lv.r, eout, lv.q, sc, s->rb, finalize)
+#define FA_LAUNCH(F, X) k_pcg_A_fast<F, X><<<grid, WL_VB, smem, s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, ein, lv.r, lv.L, lv.iD, eout, lv.q, sc, s->rb)
     switch (lv.vt.lxl) {
     case 5: if (first) FA_LAUNCH(1, 5); else FA_LAUNCH(0, 5); break;
     case 4: if (first) FA_LAUNCH(1, 4); else FA_LAUNCH(0, 4); break;

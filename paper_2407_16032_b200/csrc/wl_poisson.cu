@@ -639,9 +639,8 @@ __device__ __forceinline__ void pcgB_tile(const Grid& g, const VPos& p, float Lc
 template <int ND, int FIRST>
 __global__ void __launch_bounds__(WL_VB, WL_A_MINB) k_pcg_A(Grid g, VT vt, const int* __restrict__ plain, const float* __restrict__ L, float Lc, float iDc,
                                                  const float* __restrict__ ein, const float* __restrict__ r, const float* __restrict__ iD,
-                                                 float* __restrict__ eout, float* __restrict__ q, PcgScal* sc, RedBuf rb, int gen_only)
+                                                 float* __restrict__ eout, float* __restrict__ q, PcgScal* sc, RedBuf rb)
 {
-    // gen_only: the uniform tiles have been done by k_pcg_A_fast (wl_pcgfast.cu), which left its sums in sc->acc
     if (!FIRST && !sc->live) return;          // uniform across the grid: written by an earlier kernel
     const float beta = FIRST ? 0.0f : (float)sc->beta;
     const float m = FIRST ? pcg_mean(sc) : 0.0f;
@@ -649,15 +648,12 @@ __global__ void __launch_bounds__(WL_VB, WL_A_MINB) k_pcg_A(Grid g, VT vt, const
     for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
         VPos p = vt_pos(g, vt, tile);
         if (p.nv == 0) continue;
-        const int mode = plain[tile];
-        if (gen_only && mode != TM_GEN) continue;
 #define CALL(M) pcgA_tile<ND, FIRST, M>(g, p, L, Lc, iDc, ein, r, iD, beta, m, eout, q, v[0], v[1])
-        TILE_MODES(mode, CALL);
+        TILE_MODES(plain[tile], CALL);
 #undef CALL
     }
     if (grid_reduce<2, OpSum>(v, rb)) {
         if (threadIdx.x == 0) {
-            if (gen_only) { v[0] += sc->acc[0]; v[1] += sc->acc[1]; }
             double gamma = v[0];
             int live = 1;
             if (FIRST) {
@@ -1000,19 +996,16 @@ void wl_k_smooth(wl_sim* s, int l, int iters)
     PcgScal* sc = &s->ds->pcg[l];
     float* ea = lv.e;      // direction written by the running A pass
     float* eb = lv.e2;     // previous direction
-    // uniform tiles of a 3-D level go through the shared-memory kernel; tiles cut by a body through k_pcg_A
+    // 3-D levels go through the shared-memory kernel of wl_pcgfast.cu
     const int fast = s->fast_A && wl_pcg_fast_ok(s, l);
-    const int has_body = s->cfg.body.kind != WL_BODY_NONE;
     for (int k = 1; k <= iters; ++k) {
-        if (fast) wl_k_pcg_A_fast(s, l, k == 1, eb, ea, !has_body);
-        const int gen_only = fast;
-        if (fast && !has_body) { /* no general tiles anywhere */ }
+        if (fast) wl_k_pcg_A_fast(s, l, k == 1, eb, ea);
         else if (k == 1)
-            VDISPATCH(s, fast ? WLK_PCG_MATVEC_GEN : WLK_PCG_MATVEC, l > 0, lv.vt, (k_pcg_A<2, 1>), (k_pcg_A<3, 1>), lv.g, lv.vt, lv.plain, lv.L, lv.Lc, lv.iDc,
-                      eb, lv.r, lv.iD, ea, lv.q, sc, s->rb, gen_only);
+            VDISPATCH(s, WLK_PCG_MATVEC, l > 0, lv.vt, (k_pcg_A<2, 1>), (k_pcg_A<3, 1>), lv.g, lv.vt, lv.plain, lv.L, lv.Lc, lv.iDc,
+                      eb, lv.r, lv.iD, ea, lv.q, sc, s->rb);
         else
-            VDISPATCH(s, fast ? WLK_PCG_MATVEC_GEN : WLK_PCG_MATVEC, l > 0, lv.vt, (k_pcg_A<2, 0>), (k_pcg_A<3, 0>), lv.g, lv.vt, lv.plain, lv.L, lv.Lc, lv.iDc,
-                      eb, lv.r, lv.iD, ea, lv.q, sc, s->rb, gen_only);
+            VDISPATCH(s, WLK_PCG_MATVEC, l > 0, lv.vt, (k_pcg_A<2, 0>), (k_pcg_A<3, 0>), lv.g, lv.vt, lv.plain, lv.L, lv.Lc, lv.iDc,
+                      eb, lv.r, lv.iD, ea, lv.q, sc, s->rb);
         VDISPATCH(s, WLK_PCG_UPDATE, l > 0, lv.vt, k_pcg_B<2>, k_pcg_B<3>, lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, lv.x, lv.r, ea, lv.q, lv.iD, sc, s->rb,
                   k == 1 ? 1 : 0, k == iters ? 1 : 0);
         float* t = ea; ea = eb; eb = t;
