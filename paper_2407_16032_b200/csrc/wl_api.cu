@@ -140,7 +140,7 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
     double* partial = (double*)cv.take(sizeof(double) * 4 * WL_MAX_PARTIALS);
     unsigned int* counter = (unsigned int*)cv.take(256);
     LevDev* levdev = (LevDev*)cv.take(sizeof(LevDev) * WL_MAXLEV);
-    double* pk_part = (double*)cv.take(sizeof(double) * 2 * 2 * WL_MAX_PARTIALS);
+    double* pk_part = (double*)cv.take(sizeof(double) * 2 * 16 * WL_MAX_PARTIALS);    // room for slots of up to 16 doubles
     Grid g0 = make_grid(nd, dims[0], c->periodic);
     size_t sc = sizeof(float) * (size_t)g0.nalloc;
     float* ub[3];
@@ -586,7 +586,7 @@ extern "C" int wl_dbg_coarse_prog(wl_sim* s, int n, const int* kinds, const int*
     CoarseProg P; P.n = n;
     for (int k = 0; k < n; ++k) {
         const int top = kinds[k] == COP_SMOOTH ? s->nlev - 1 : s->nlev - 2;
-        if (kinds[k] < 0 || kinds[k] > 2 || levels[k] < 0 || levels[k] > top || (kinds[k] == COP_SMOOTH && iters[k] < 1)) return WL_EINVAL;
+        if (kinds[k] < 0 || kinds[k] > 4 || levels[k] < 0 || levels[k] > top || (kinds[k] == COP_SMOOTH && iters[k] < 1)) return WL_EINVAL;
         P.op[k].kind = kinds[k]; P.op[k].level = levels[k]; P.op[k].iters = iters[k];
     }
     wl_k_coarse_prog(s, P);

@@ -40,7 +40,7 @@ struct LevDev {
 };
 
 // a chain of coarse-level passes run by one k_coarse launch
-enum { COP_RESTRICT = 0, COP_SMOOTH = 1, COP_PROLONG = 2 };   // RESTRICT: level -> level+1; PROLONG: level+1 -> level
+enum { COP_RESTRICT = 0, COP_SMOOTH = 1, COP_PROLONG = 2, COP_NOP = 3, COP_BAR = 4 };   // RESTRICT: level -> level+1; PROLONG: level+1 -> level
 struct CoarseOp { int kind, level, iters; };
 struct CoarseProg { int n; CoarseOp op[3 * WL_MAXLEV]; };
 

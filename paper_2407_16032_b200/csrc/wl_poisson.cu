@@ -26,6 +26,9 @@
 #ifndef WL_B_MINB
 #define WL_B_MINB 4
 #endif
+#ifndef WL_PK_SLOT
+#define WL_PK_SLOT 4      // doubles per block slot of the k_coarse partial sums: one 32-byte sector each
+#endif
 #ifndef WL_PK_MINB
 #define WL_PK_MINB 2
 #endif
@@ -745,7 +748,7 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
 }
 
 struct PkCtx {
-    double* part;        // [2][PK_NV][WL_MAX_PARTIALS] per-block partial sums, alternating by reduction
+    double* part;        // [2][WL_MAX_PARTIALS][WL_PK_SLOT] per-block partial sums (one slot per block), alternating by reduction
     int phase;
 };
 #define PK_NV 2
@@ -759,7 +762,7 @@ __device__ __forceinline__ void pk_reduce(PkCtx& c, double (&v)[NV])
 {
     __shared__ double sm[PK_NV][32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = WL_VB >> 5;
-    double* part = c.part + (size_t)(c.phase & 1) * PK_NV * WL_MAX_PARTIALS;
+    double* part = c.part + (size_t)(c.phase & 1) * WL_PK_SLOT * WL_MAX_PARTIALS;
     c.phase++;
 #pragma unroll
     for (int k = 0; k < NV; ++k) {
@@ -772,22 +775,37 @@ __device__ __forceinline__ void pk_reduce(PkCtx& c, double (&v)[NV])
         for (int k = 0; k < NV; ++k) {
             double w = lane < nw ? sm[k][lane] : 0.0;
             w = warp_red<OpSum>(w);
-            if (lane == 0) part[k * WL_MAX_PARTIALS + blockIdx.x] = w;
+            if (lane == 0) part[blockIdx.x * WL_PK_SLOT + k] = w;
         }
     }
     pk_barrier(c);
-    if (wid == 0) {
+    // every block adds all partials in the same fixed order: thread-strided (all loads in flight at once; a
+    // single warp walking the list pays one L2 round trip per step), then the same warp/shared tree as above
+    {
+        double w[NV][2];
+        const int G = (int)gridDim.x;
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int b = tid + j * WL_VB;
+#pragma unroll
+            for (int k = 0; k < NV; ++k) w[k][j] = b < G ? __ldcg(&part[b * WL_PK_SLOT + k]) : 0.0;
+        }
 #pragma unroll
         for (int k = 0; k < NV; ++k) {
-            double w = 0.0;
-            for (int b = lane; b < (int)gridDim.x; b += 32) w += __ldcg(&part[k * WL_MAX_PARTIALS + b]);
-            w = warp_red<OpSum>(w);
-            if (lane == 0) sm[k][0] = w;
+            double t = w[k][0] + w[k][1];
+            for (int b = tid + 2 * WL_VB; b < G; b += WL_VB) t += __ldcg(&part[b * WL_PK_SLOT + k]);   // grids beyond 512 blocks
+            t = warp_red<OpSum>(t);
+            if (lane == 0) sm[k][wid] = t;
         }
     }
     __syncthreads();
 #pragma unroll
-    for (int k = 0; k < NV; ++k) v[k] = sm[k][0];
+    for (int k = 0; k < NV; ++k) {
+        double t = 0.0;
+#pragma unroll
+        for (int i = 0; i < (WL_VB >> 5); ++i) t += sm[k][i];
+        v[k] = t;
+    }
     __syncthreads();
 }
 
@@ -859,7 +877,12 @@ __global__ void __launch_bounds__(WL_VB, WL_PK_MINB) k_coarse(const LevDev* levs
             lb = levs[op.level + (op.kind == COP_SMOOTH ? 0 : 1)];
         }
         __syncthreads();
-        if (op.kind == COP_SMOOTH) {
+        if (op.kind == COP_NOP) {                    // timing probes: one reduction / one bare grid barrier
+            double v[1] = { 1.0 };
+            pk_reduce<1>(c, v);
+        } else if (op.kind == COP_BAR) {
+            pk_barrier(c);
+        } else if (op.kind == COP_SMOOTH) {
             PcgScal* sc = &ds->pcg[op.level];
             const double rs = rsum_level == op.level ? rsum : sc->rsum;
             pk_smooth<ND>(c, la, sc, op.iters, rs);
