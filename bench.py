@@ -44,30 +44,27 @@ METRIC = "ns per cell per time step (3D fp32)"
 UNIT = "ns/cell/step"
 
 # Algorithmic bytes per fine-grid cell of each kernel class (fp32, every array read/written once
-# per pass, halos ignored): DESIGN.md section 6 restates SURVEY.md 8(d)'s table for the kernels as
-# they are fused in libwl.
+# per pass, halos ignored) ON BODY-FREE TILES, where face coefficients and 1/D are analytic and not
+# loaded: DESIGN.md section 6 restates SURVEY.md 8(d)'s table for the kernels as they are fused in
+# libwl.  These are the smallest counts (tiles cut by a body also read L and iD), so the achieved
+# GB/s computed from them is a lower bound.
 ALG_BYTES = {
-    "conv_diff_bdim": None,   # depends on body / corrector: computed below
-    "residual": 4 * (3 + 1 + 3 + 2),        # u, p, L -> x, r
-    "pcg_init": 4 * (2 + 1),                # r, iD -> e
-    "pcg_matvec": 4 * (1 + 3 + 1),          # e, L -> q
-    "pcg_update": 4 * (5 + 3),              # x, e, r, q, iD -> x, r, z (z not written by the last iteration)
-    "pcg_dir": 4 * (2 + 1),                 # e, z -> e
-    "pcg_fused": 4 * (6 + 3 + 3),           # (r, q, x, e, iD, + L 3) -> x, r, e... see DESIGN.md
-    "restrict": 4 * (1 + 2 / 8),
-    "prolong": 4 * (2 + 3 + 1 / 8 + 2),
-    "apply_gradient": 4 * (3 + 3 + 1 + 3 + 1),
+    "conv_diff_bdim": None,   # mean of predictor and corrector: computed below
+    "residual": 4 * (3 + 1 + 2),            # u, p -> x, r
+    "pcg_matvec": 4 * (2 + 2),              # pass A: e, r -> e', q (first iteration: r -> e', q)
+    "pcg_update": 4 * (4 + 2),              # pass B: x, r, e', q -> x, r
+    "restrict": 4 * (1 + 2 / 8),            # r -> r_c, x_c
+    "prolong": 4 * (2 + 1 / 8 + 2),         # x, r, x_c -> x, r
+    "apply_gradient": 4 * (3 + 1 + 3 + 1),  # u, x -> u, p
     "cfl": 4 * 3,
     "measure": 4 * (3 + 9),
 }
 
 
 def conv_alg_bytes(cfg) -> float:
-    """conv_diff+BDIM, mean of the predictor and corrector passes (floats read + written) * 4."""
-    body = cfg["body_kind"] != wi.BODY_NONE
-    rd_p = 3 + (3 + 9 if body else 0)          # w (= u0), mu0, mu1 ; V is 3 scalars
-    rd_c = 6 + (3 + 9 if body else 0)          # w, u0, mu0, mu1
-    return 4 * ((rd_p + 3) + (rd_c + 3)) / 2
+    """conv_diff+BDIM tile kernel, mean of the predictor (w, mu0 -> u) and corrector (w, u0, mu0 -> u)
+    passes; mu1 is read only on the band list (k_cd_band), V is three scalars."""
+    return 4 * ((3 + 3 + 3) + (3 + 3 + 3 + 3)) / 2
 
 
 def ncells(cfg) -> int:
@@ -327,10 +324,11 @@ def run_gpu(args) -> None:
     breakdown = {}
     for name, (ms, n) in sorted(prof.items(), key=lambda kv: -kv[1][0]):
         ent = {"ms_per_step": ms / args.steps, "launches_per_step": n / args.steps, "share": ms / tot_prof}
-        if name in alg and alg[name]:
+        if name in alg and alg[name]:                 # fine-level classes only (".coarse" = multigrid levels >= 1)
             ent["alg_gbs"] = alg[name] * cells * n / (ms * 1e-3) / 1e9
         breakdown[name] = ent
-    dom = next(iter(breakdown))
+    # the dominant kernel with a roofline: the fine-level class that takes the most time
+    dom = next((nm for nm in breakdown if alg.get(nm)), next(iter(breakdown)))
     dom_ms, dom_n = prof[dom]
     base = dom.split(".")[0]
     achieved = (alg.get(base) or 0) * cells * dom_n / (dom_ms * 1e-3) / 1e9 if not dom.endswith(".coarse") else None
