@@ -88,6 +88,14 @@ static Grid make_grid(int nd, const int* n, const int* per)
     return g;
 }
 
+// levels with at most this many cells run inside the persistent coarse-level kernels (k_coarse / k_tiny)
+static long long pk_max_cells()
+{
+    long long maxc = 1000000;
+    if (const char* e = getenv("WL_PK_MAX_CELLS")) maxc = atoll(e);
+    return maxc;
+}
+
 // Vector tiling of a level.  Coarse levels are latency-bound, not bandwidth-bound: they take fewer
 // planes per tile so that enough tiles (>= 4 per SM of a 148-SM B200 where the level allows) are in flight.
 static VT make_vt(int nd, const Grid& g, int level)
@@ -100,7 +108,7 @@ static VT make_vt(int nd, const Grid& g, int level)
     t.ntx = (t.ngx + lx - 1) / lx;
     t.nty = (g.n[1] + ly - 1) / ly;
     t.zc = nd == 3 ? (g.n[2] < 8 ? g.n[2] : 8) : 1;
-    if (level > 0)
+    if (level > 0 && (long long)g.n[0] * g.n[1] * g.n[2] <= pk_max_cells())
         while (t.zc > 1 && (int64_t)t.ntx * t.nty * ((g.n[2] + t.zc - 1) / t.zc) < 592) t.zc = (t.zc + 1) / 2;
     t.ntz = nd == 3 ? (g.n[2] + t.zc - 1) / t.zc : 1;
     t.ntiles = t.ntx * t.nty * t.ntz;
@@ -289,8 +297,7 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     layout(s, cfg, dev_ws);
     s->u = s->ubuf[0]; s->u0 = s->ubuf[1]; s->ut = s->ubuf[2];
     {   // levels that run inside the persistent coarse-level kernel: from the first level >= 1 small enough
-        long long maxc = 1000000;
-        if (const char* e = getenv("WL_PK_MAX_CELLS")) maxc = atoll(e);
+        const long long maxc = pk_max_cells();
         s->pk_level = s->nlev;
         for (int l = s->nlev - 1; l >= 1; --l) {
             const Grid& g = s->lev[l].g;
@@ -298,6 +305,8 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
         }
     }
     s->fast_A = 1;
+    s->tiny_on = 1;
+    if (const char* e = getenv("WL_TINY")) s->tiny_on = atoi(e) != 0;
     if (const char* e = getenv("WL_FAST_A")) s->fast_A = atoi(e) != 0;
     s->body.kind = cfg->body.kind; s->body.axis = cfg->body.axis;
     s->body.R = cfg->body.R; s->body.r = cfg->body.r; s->body.eps = cfg->eps;
