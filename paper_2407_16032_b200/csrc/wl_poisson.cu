@@ -35,6 +35,15 @@
 #ifndef WL_PK_SLOT
 #define WL_PK_SLOT 4      // doubles per block slot of the k_coarse partial sums: one 32-byte sector each
 #endif
+#ifndef WL_G_MINB
+#define WL_G_MINB 4
+#endif
+#ifndef WL_R_MINB
+#define WL_R_MINB 2
+#endif
+#ifndef WL_P_MINB
+#define WL_P_MINB 4
+#endif
 #ifndef WL_PK_MINB
 #define WL_PK_MINB 2
 #endif
@@ -391,7 +400,7 @@ __device__ __forceinline__ void residual_tile(const Grid& g, const VPos& p, cons
 }
 
 template <int ND>
-__global__ void __launch_bounds__(WL_VB) k_residual(Grid g, VT vt, const int* __restrict__ plain, const float* __restrict__ u, const float* __restrict__ L, float Lc,
+__global__ void __launch_bounds__(WL_VB, WL_R_MINB) k_residual(Grid g, VT vt, const int* __restrict__ plain, const float* __restrict__ u, const float* __restrict__ L, float Lc,
                                                     const float* __restrict__ iD, const float* __restrict__ p, float* __restrict__ x, float* __restrict__ r,
                                                     DevScal* ds, float w, RedBuf rb)
 {
@@ -458,7 +467,7 @@ __device__ __forceinline__ void gradient_tile(const Grid& g, const VPos& p, floa
 }
 
 template <int ND>
-__global__ void __launch_bounds__(WL_VB) k_apply_gradient(Grid g, VT vt, const int* __restrict__ plain, float* __restrict__ u, const float* __restrict__ L, float Lc,
+__global__ void __launch_bounds__(WL_VB, WL_G_MINB) k_apply_gradient(Grid g, VT vt, const int* __restrict__ plain, float* __restrict__ u, const float* __restrict__ L, float Lc,
                                                           const float* __restrict__ x, float* __restrict__ p, const DevScal* __restrict__ ds)
 {
     const float isc = 1.0f / ds->pscale;
@@ -566,7 +575,7 @@ __device__ __forceinline__ void prolong_tile(const Grid& gf, const Grid& gc, con
 }
 
 template <int ND>
-__global__ void __launch_bounds__(WL_VB) k_prolong(Grid gf, Grid gc, VT vt, const int* __restrict__ plain, const float* __restrict__ L, float Lc, const float* __restrict__ iD,
+__global__ void __launch_bounds__(WL_VB, WL_P_MINB) k_prolong(Grid gf, Grid gc, VT vt, const int* __restrict__ plain, const float* __restrict__ L, float Lc, const float* __restrict__ iD,
                                                    const float* __restrict__ xc, float* __restrict__ xf, float* __restrict__ rf, PcgScal* scf, RedBuf rb)
 {
     double v[1] = { 0.0 };
