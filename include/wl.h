@@ -150,6 +150,17 @@ int wl_dbg_restrict(wl_sim* s, int level);
 int wl_dbg_prolong(wl_sim* s, int level);
 int wl_dbg_smooth(wl_sim* s, int level, int iters);
 int wl_dbg_vcycle(wl_sim* s, int level);
+/* Runs n coarse-level passes as one chain through the persistent kernels: kinds[k] = 0 restrict
+ * levels[k] -> levels[k]+1, 1 smooth level levels[k] with iters[k] PCG iterations, 2 prolong levels[k]+1 ->
+ * levels[k], 3 one grid-wide reduction only, 4 one barrier only (timing probes).  Consecutive passes of the same
+ * kind of launch (whole-GPU cooperative k_coarse / one-cluster k_tiny) share a launch.  n <= 48. */
+int wl_dbg_coarse_prog(wl_sim* s, int n, const int* kinds, const int* levels, const int* iters);
+/* %globaltimer (ns) at the start of every pass of the LAST persistent-kernel launch and at its end: n values
+ * (n - 1 passes).  Synchronises. */
+int wl_dbg_coarse_times(wl_sim* s, unsigned long long* out, int n);
+/* Device-resident PCG scalars of a level: rho, gamma, alpha, beta, rho0, sum of r over the coupled cells (R-T2),
+ * number of coupled cells, live flag.  Synchronises. */
+int wl_dbg_pcg_scalars(wl_sim* s, int level, double out[8]);
 /* Raw access to a solver array for tests: name in {"u","u0","p","mu0","mu1","L","iD","x","r"};
  * interior-sized copy into `out` (host), ncomp arrays; returns ncomp or a negative status. */
 int wl_dbg_get(wl_sim* s, const char* name, int level, float* out, size_t out_floats);

@@ -24,6 +24,7 @@ EXPORTS = [
     "wl_mom_step", "wl_cfl", "wl_pressure_force", "wl_get_fields", "wl_step",
     "wl_dbg_conv_diff_bdim", "wl_dbg_save_u0", "wl_dbg_bc", "wl_dbg_exit_bc", "wl_dbg_project",
     "wl_dbg_residual", "wl_dbg_apply_gradient", "wl_dbg_restrict", "wl_dbg_prolong", "wl_dbg_smooth", "wl_dbg_vcycle",
+    "wl_dbg_coarse_prog", "wl_dbg_coarse_times", "wl_dbg_pcg_scalars",
     "wl_dbg_get", "wl_dbg_set", "wl_dbg_get_padded", "wl_level_dims", "wl_last_error", "wl_stats", "wl_abi_version",
     "wl_prof_enable", "wl_prof_read",
 ]
@@ -91,6 +92,9 @@ def load(build_if_missing: bool = True):
     for name in ("wl_dbg_restrict", "wl_dbg_prolong", "wl_dbg_vcycle"):
         getattr(L, name).argtypes = [vp, ip]
     L.wl_dbg_smooth.argtypes = [vp, ip, ip]
+    L.wl_dbg_coarse_prog.argtypes = [vp, ip, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    L.wl_dbg_coarse_times.argtypes = [vp, C.POINTER(C.c_ulonglong), ip]
+    L.wl_dbg_pcg_scalars.argtypes = [vp, ip, C.POINTER(C.c_double)]
     L.wl_dbg_get.argtypes = [vp, C.c_char_p, ip, vp, C.c_size_t]
     L.wl_dbg_set.argtypes = [vp, C.c_char_p, ip, vp, C.c_size_t]
     L.wl_dbg_get_padded.argtypes = [vp, C.c_char_p, ip, vp, C.c_size_t]
@@ -326,3 +330,20 @@ class Sim:
 
     def dbg_vcycle(self, level=0):
         self._chk(self._L.wl_dbg_vcycle(self._h, int(level)))
+
+    def dbg_coarse_prog(self, ops):
+        """ops: sequence of (kind, level, iters); see wl_dbg_coarse_prog in include/wl.h."""
+        n = len(ops)
+        A = C.c_int * n
+        self._chk(self._L.wl_dbg_coarse_prog(self._h, n, A(*[int(o[0]) for o in ops]), A(*[int(o[1]) for o in ops]),
+                                             A(*[int(o[2]) for o in ops])))
+
+    def dbg_coarse_times(self, n):
+        out = (C.c_ulonglong * n)()
+        self._chk(self._L.wl_dbg_coarse_times(self._h, out, n))
+        return [int(v) for v in out]
+
+    def dbg_pcg_scalars(self, level):
+        out = (C.c_double * 8)()
+        self._chk(self._L.wl_dbg_pcg_scalars(self._h, int(level), out))
+        return dict(zip(("rho", "gamma", "alpha", "beta", "rho0", "rsum", "nlive", "live"), [float(v) for v in out]))

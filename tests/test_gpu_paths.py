@@ -1,0 +1,144 @@
+"""GPU parity of the alternative kernel paths of the projection: the shared-memory PCG pass A
+(`k_pcg_A_fast`) against the register-marching one, the persistent coarse-level kernels (`k_coarse`, cooperative;
+`k_tiny`, one thread-block cluster) against stand-alone launches, a fused chain of coarse passes against the same
+passes launched one by one -- each against the fp64 oracle, and against one another.  The environment switches
+(WL_FAST_A, WL_TINY, WL_PK_MAX_CELLS) are read when a simulation is created."""
+import os
+
+import numpy as np
+import pytest
+
+import wl_inputs as wi
+from test_gpu_kernels import CASES, O, TOL, _cfg, _ids, _load_state, _sims, diag, relerr
+
+pytestmark = pytest.mark.gpu
+
+SWITCHES = [
+    {},                                     # default: fast pass A, k_coarse for levels <= 1 M cells, k_tiny below
+    {"WL_FAST_A": "0"},                     # register-marching pass A everywhere
+    {"WL_TINY": "0"},                       # tiny levels inside the cooperative kernel
+    {"WL_PK_MAX_CELLS": "0"},               # every level by stand-alone kernels
+]
+
+
+class _env:
+    def __init__(self, kv):
+        self.kv = kv
+
+    def __enter__(self):
+        self.old = {k: os.environ.get(k) for k in self.kv}
+        os.environ.update(self.kv)
+
+    def __exit__(self, *a):
+        for k, v in self.old.items():
+            if v is None:
+                os.environ.pop(k, None)
+            else:
+                os.environ[k] = v
+
+
+WIDE = [c for c in CASES if len(c[0]) == 3 and c[0][0] >= 136] + [((64, 64, 64), (0, 1, 0), 1, "sphere", False)]
+
+
+@pytest.mark.parametrize("case", WIDE, ids=_ids)
+def test_every_path_matches_the_oracle_and_the_others(case):
+    """Three full steps (fixed two V-cycles) through each path: velocity vs the oracle <= 1e-4, and the paths
+    agree with one another to round-off amplified by three steps."""
+    from oracle import wl_oracle as wo
+    from paper_2407_16032_b200 import wl
+    cfg = _cfg(case)
+    o = wo.OracleSim(cfg)
+    u0 = wi.random_velocity(case[0], seed=wi.SEED + 3)
+    o.set_fields(u=u0)
+    dt = 0.25
+    for _ in range(3):
+        o.mom_step(dt)
+    uo = O(o, "u")
+    outs = []
+    for sw in SWITCHES:
+        with _env(sw):
+            g = wl.Sim(cfg)
+        g.set_fields(u=np.ascontiguousarray(u0, dtype=np.float32))
+        for _ in range(3):
+            g.mom_step(dt)
+        u, _p = g.fields()
+        assert g.stats()["nan_flag"] == 0
+        assert relerr(u, uo) <= 1e-4, sw
+        outs.append(u.astype(np.float64))
+        g.close()
+    for u in outs[1:]:
+        assert np.abs(u - outs[0]).max() <= 2e-5 * np.abs(uo).max()
+    o.close()
+
+
+@pytest.mark.parametrize("case", [CASES[0], CASES[2], CASES[8], CASES[9]], ids=_ids)
+def test_fused_coarse_chain_equals_single_passes(case):
+    """The V-cycle below level 0 as ONE chain (wl_dbg_coarse_prog) and as one launch per pass give the oracle's
+    x and r on every level; after each smooth the stored sum of r over the coupled cells is reset (R-T2)."""
+    cfg = _cfg(case)
+    dims = case[0]
+    res = []
+    for fused in (True, False):
+        o, g = _sims(cfg)
+        _load_state(o, g, dims)
+        o.arr("u0")[...] = o.arr("u"); g.dbg_save_u0()
+        o.conv_diff("u0"); o.bdim(0.3, 0); g.dbg_conv_diff_bdim(0.3, 0)
+        o.bc(); g.dbg_bc()
+        if case[2]:
+            o.exit_bc(0.3); g.dbg_exit_bc(0.3)
+        x0 = np.zeros(dims[::-1])
+        o.interior("x")[0][...] = x0; g.dbg_set("x", x0[None].astype(np.float32))
+        o.arr("sig")[...] = o.divergence(); o.residual(); g.dbg_residual()
+        n = o.nlevels
+        ops = []
+        for l in range(n - 1):
+            o.restrict(l); o.arr("x", l + 1)[...] = 0.0
+            ops.append((0, l, 0))
+        for l in range(n - 1, 0, -1):
+            o.smooth(l, 6); ops.append((1, l, 6))
+            o.prolong_increment(l - 1); ops.append((2, l - 1, 0))
+        if fused:
+            g.dbg_coarse_prog(ops)
+        else:
+            for op in ops:
+                g.dbg_coarse_prog([op])
+        r0 = np.abs(O(o, "r", 0)).max()
+        lev = []
+        for l in range(n):
+            xg, rg = g.dbg_get("x", l), g.dbg_get("r", l)
+            assert relerr(xg, O(o, "x", l)) <= 1e-4
+            assert np.abs(rg - O(o, "r", l)).max() <= 1e-4 * max(r0, np.abs(O(o, "r", l)).max())
+            lev.append((xg, rg))
+        for l in range(1, n):
+            sc = g.dbg_pcg_scalars(l)
+            assert sc["rsum"] == 0.0                                   # reset by the smoother
+            assert sc["nlive"] == float((O(o, "iD", l)[0] != 0).sum())
+        res.append(lev)
+        o.close(); g.close()
+    for (xa, ra), (xb, rb) in zip(*res):
+        assert np.array_equal(xa, xb) and np.array_equal(ra, rb)       # same kernels, same order: bit-identical
+
+
+def test_smoother_removes_residual_mean_on_the_gpu():
+    """R-T2 on the device: a residual shifted by a constant on the coupled cells gives the same x (oracle pin
+    test_smoother_removes_the_incompatible_part_of_the_residual, here for libwl on every level)."""
+    cfg = _cfg(CASES[8])
+    o, g = _sims(cfg)
+    for l in range(o.nlevels):
+        ld = g.level_dims(l)
+        live = O(o, "iD", l)[0] != 0
+        out = []
+        for shift in (0.0, 0.05):
+            r = wi.random_scalar(ld, seed=500 + l)
+            r = r * np.minimum(1.0, np.abs(diag(O(o, "iD", l)[0])))
+            r[~live] = 0.0
+            r[live] += shift - r[live].mean()
+            g.dbg_set("r", r[None].astype(np.float32), l)
+            g.dbg_set("x", np.zeros_like(r)[None].astype(np.float32), l)
+            g.dbg_smooth(l, 3)
+            out.append((g.dbg_get("x", l).astype(np.float64), g.dbg_get("r", l).astype(np.float64)))
+        (xa, ra), (xb, rb) = out
+        # the shifted residual is rounded to fp32 before the smoother sees it: 3 CG iterations amplify that round-off
+        assert np.abs(xb - xa).max() <= 1e-4 * max(np.abs(xa).max(), 1e-30)
+        assert abs(rb[0][live].mean()) <= 1e-6
+    o.close(); g.close()
