@@ -49,40 +49,43 @@ __device__ __forceinline__ float bdim_mu1(float d, float eps)
     return eps * (0.25f - 0.25f * a * a - (a * sp + (1.0f + cp) * 0.3183098861837907f) * 0.15915494309189535f);
 }
 
-// Signed distance and unit normal at body-frame position xi (translation map: J = I).
-template <int ND>
-__device__ __forceinline__ float body_sdf(const BodyP& b, const float (&xi)[3], float (&nrm)[3])
+// Signed distance and unit normal at body-frame position xi (translation map: J = I).  T = double in measure!
+// (a face 100 cells from the origin carries 6e-6 of fp32 round-off in its position, which mu0's slope 1/2eps turns
+// into 3e-6 of mu0: evaluated in fp64 and rounded once, d is good to 6e-8), T = float elsewhere.
+template <int ND, class T>
+__device__ __forceinline__ T body_sdf(const BodyP& b, const T (&xi)[3], T (&nrm)[3])
 {
-    nrm[0] = nrm[1] = nrm[2] = 0.0f;
+    nrm[0] = nrm[1] = nrm[2] = T(0);
+    const T tiny = T(1e-12);
     if (b.kind == WLB_SPHERE) {
-        float rr = 0.0f;
+        T rr = T(0);
 #pragma unroll
         for (int k = 0; k < ND; ++k) rr += xi[k] * xi[k];
-        rr = sqrtf(rr);
-        if (rr >= 1e-12f) {
-            float inv = 1.0f / rr;
+        rr = sqrt(rr);
+        if (rr >= tiny) {
+            T inv = T(1) / rr;
 #pragma unroll
             for (int k = 0; k < ND; ++k) nrm[k] = xi[k] * inv;
         }
-        return rr - b.R;
+        return rr - (T)b.R;
     }
     // torus: axis a, rho = distance from the axis
-    float xa, xb, xc;
+    T xa, xb, xc;
     if (b.axis == 0) { xa = xi[0]; xb = xi[1]; xc = xi[2]; }
     else if (b.axis == 1) { xa = xi[1]; xb = xi[2]; xc = xi[0]; }
     else { xa = xi[2]; xb = xi[0]; xc = xi[1]; }
-    float rho = sqrtf(xb * xb + xc * xc);
-    float w = rho - b.R;
-    float gq = sqrtf(w * w + xa * xa);
-    float na = 0.0f, nb = 0.0f, nc = 0.0f;
-    if (gq >= 1e-12f && rho >= 1e-12f) {
-        float ig = 1.0f / gq, wr = (w * ig) / rho;
+    T rho = sqrt(xb * xb + xc * xc);
+    T w = rho - (T)b.R;
+    T gq = sqrt(w * w + xa * xa);
+    T na = T(0), nb = T(0), nc = T(0);
+    if (gq >= tiny && rho >= tiny) {
+        T ig = T(1) / gq, wr = (w * ig) / rho;
         na = xa * ig; nb = wr * xb; nc = wr * xc;
-    } else if (gq >= 1e-12f) {
+    } else if (gq >= tiny) {
         na = xa / gq;
     }
     if (b.axis == 0) { nrm[0] = na; nrm[1] = nb; nrm[2] = nc; }
     else if (b.axis == 1) { nrm[1] = na; nrm[2] = nb; nrm[0] = nc; }
     else { nrm[2] = na; nrm[0] = nb; nrm[1] = nc; }
-    return gq - b.r;
+    return gq - (T)b.r;
 }

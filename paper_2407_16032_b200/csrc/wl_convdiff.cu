@@ -15,6 +15,7 @@
 //    list of those faces (wl_flow.cu) and this kernel adds sum_j mu1_ij (f_i[c+d_j]-f_i[c-d_j])/2
 //    there, recomputing the six neighbouring r from global memory.
 #include <cstdio>
+#include <cstdlib>
 #include "wl_internal.h"
 
 __device__ __forceinline__ float med3(float a, float b, float c)
@@ -403,6 +404,285 @@ __global__ void __launch_bounds__(CD_NT, 2) k_cd_tile(FlowP P, CdT T, const floa
     }
 }
 
+// ====================================================================== the tile kernel, one component per thread
+// k_cd_tile computes every limited face flux of a cell for each of its two neighbours: 63 per thread and plane,
+// 128 registers, two 256-thread blocks per SM -- instruction-bound at 15 % of the DRAM rate (profiles/r1b).
+// k_cd_tile2 works from the same five-plane ring but (a) a thread owns four cells of ONE component (blocks of
+// 256 x ND threads; warps are component-uniform), (b) the flux through a y face is computed once, by the thread above
+// it, and handed down through shared memory, (c) the flux through the upper z face is kept for the next plane of the
+// march, where it is the lower one.  41 instead of 63 fluxes per four cells of the three components, identical
+// values (a flux is the same expression of the same operands whichever thread evaluates it).
+#define CD2_NT(ND) (CD_NT * (ND))
+#define CD2_STAGE(ND) ((CD_ITEMS(ND) + CD2_NT(ND) - 1) / CD2_NT(ND))
+
+template <int ND>
+__device__ __forceinline__ void cd2_load_regs(const Grid& g, const float* __restrict__ w, int bx, int by, int cz, float4 (&st)[CD2_STAGE(ND)])
+{
+#pragma unroll
+    for (int k = 0; k < CD2_STAGE(ND); ++k) {
+        const int item = threadIdx.x + k * CD2_NT(ND);
+        if (item < CD_ITEMS(ND)) st[k] = cd_fetch<ND>(g, w, item, bx, by, cz);
+    }
+}
+template <int ND>
+__device__ __forceinline__ void cd2_store_regs(float* __restrict__ slot, const float4 (&st)[CD2_STAGE(ND)])
+{
+#pragma unroll
+    for (int k = 0; k < CD2_STAGE(ND); ++k) {
+        const int item = threadIdx.x + k * CD2_NT(ND);
+        if (item < CD_ITEMS(ND)) reinterpret_cast<float4*>(slot)[item] = st[k];
+    }
+}
+
+// what a thread carries from the flux phase to the output phase of a plane
+struct Cd2Part {
+    float rx[4];     // F_x[k] - F_x[k+1]
+    float fyl[4];    // flux through the lower y face (handed to the thread below as its upper one)
+    float fyu[4];    // flux through the upper y face: computed here only in the top row of the block
+    float fzd[4];    // F_z lower - F_z upper
+    float wc[5];     // w_I at the own cells and the next one (convective-exit carry)
+};
+
+// fluxes of component I at the thread's four cells of plane gz.  fz: in (unless `first`) the flux through the lower z
+// face left by the previous plane; out the flux through the upper z face.
+template <int ND, int I>
+__device__ __forceinline__ void cd2_fluxes(const FlowP& P, const CdView& v, int gx, int gy, int gz, bool top, bool first, float (&fz)[4], Cd2Part& o)
+{
+    const Grid& g = P.g;
+    const float nu = P.nu;
+    float a[12];
+    v4(v, I, 0, 0, -1, a); v4(v, I, 0, 0, 0, a + 4); v4(v, I, 0, 0, 1, a + 8);
+#pragma unroll
+    for (int k = 0; k < 5; ++k) o.wc[k] = a[4 + k];
+    // ---- x faces gx .. gx+4 (shared between the thread's cells)
+    {
+        float px[5];
+        if (I == 0) {
+#pragma unroll
+            for (int f = 0; f < 5; ++f) px[f] = 0.5f * (a[3 + f] + a[4 + f]);
+        } else {
+            float lo[5], hi[5];
+            v4(v, 0, 0, 0, 0, hi); hi[4] = v1(v, 0, 0, 0, 4);
+            if (I == 1) { v4(v, 0, 0, -1, 0, lo); lo[4] = v1(v, 0, 0, -1, 4); }
+            else        { v4(v, 0, -1, 0, 0, lo); lo[4] = v1(v, 0, -1, 0, 4); }
+#pragma unroll
+            for (int f = 0; f < 5; ++f) px[f] = 0.5f * (lo[f] + hi[f]);
+        }
+        float F[5];
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+            const int cj = gx + f;
+            const bool fbp = !g.per[0] && cj <= 1 + (I == 0 ? 1 : 0), fbn = !g.per[0] && cj >= g.n[0] + 1;
+            F[f] = face_flux(px[f], a[2 + f], a[3 + f], a[4 + f], a[5 + f], fbp, fbn, nu);
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) o.rx[k] = F[k] - F[k + 1];
+    }
+    // ---- y faces: the lower one (gy) always, the upper one (gy+1) in the top row of the block only
+    {
+        float m2[4], m1[4], p1[4], pl[4];
+        v4(v, I, 0, -2, 0, m2); v4(v, I, 0, -1, 0, m1); v4(v, I, 0, 1, 0, p1);
+        float b0[4], c0[4], e0 = 0.0f;
+        if (I == 1) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) pl[k] = 0.5f * (m1[k] + a[4 + k]);
+        } else if (I == 0) {
+            v4(v, 1, 0, 0, 0, b0); e0 = v1(v, 1, 0, 0, -1);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) pl[k] = 0.5f * ((k == 0 ? e0 : b0[k == 0 ? 0 : k - 1]) + b0[k]);
+        } else {
+            v4(v, 1, -1, 0, 0, b0); v4(v, 1, 0, 0, 0, c0);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) pl[k] = 0.5f * (b0[k] + c0[k]);
+        }
+        const bool np = !g.per[1];
+        const bool lfbp = np && gy <= 1 + (I == 1 ? 1 : 0), lfbn = np && gy >= g.n[1] + 1;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) o.fyl[k] = face_flux(pl[k], m2[k], m1[k], a[4 + k], p1[k], lfbp, lfbn, nu);
+        if (top) {
+            float p2[4], pu[4], b1[4], c1[4];
+            v4(v, I, 0, 2, 0, p2);
+            if (I == 1) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) pu[k] = 0.5f * (a[4 + k] + p1[k]);
+            } else if (I == 0) {
+                v4(v, 1, 0, 1, 0, b1);
+                const float e1 = v1(v, 1, 0, 1, -1);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) pu[k] = 0.5f * ((k == 0 ? e1 : b1[k == 0 ? 0 : k - 1]) + b1[k]);
+            } else {
+                v4(v, 1, -1, 1, 0, b1); v4(v, 1, 0, 1, 0, c1);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) pu[k] = 0.5f * (b1[k] + c1[k]);
+            }
+            const bool ufbp = np && gy + 1 <= 1 + (I == 1 ? 1 : 0), ufbn = np && gy + 1 >= g.n[1] + 1;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) o.fyu[k] = face_flux(pu[k], m1[k], a[4 + k], p1[k], p2[k], ufbp, ufbn, nu);
+        }
+    }
+
+    // ---- z faces: the upper one (gz+1) always; the lower one (gz) only on the first plane of the march
+    if (ND == 3) {
+        float m1[4], p1[4], p2[4], pu[4];
+        v4(v, I, -1, 0, 0, m1); v4(v, I, 1, 0, 0, p1); v4(v, I, 2, 0, 0, p2);
+        const bool np = !g.per[2];
+        if (first) {
+            float m2[4], pl[4], b0[4], c0[4];
+            v4(v, I, -2, 0, 0, m2);
+            if (I == 2) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) pl[k] = 0.5f * (m1[k] + a[4 + k]);
+            } else if (I == 0) {
+                v4(v, 2, 0, 0, 0, b0);
+                const float e0 = v1(v, 2, 0, 0, -1);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) pl[k] = 0.5f * ((k == 0 ? e0 : b0[k == 0 ? 0 : k - 1]) + b0[k]);
+            } else {
+                v4(v, 2, 0, -1, 0, b0); v4(v, 2, 0, 0, 0, c0);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) pl[k] = 0.5f * (b0[k] + c0[k]);
+            }
+            const bool lfbp = np && gz <= 1 + (I == 2 ? 1 : 0), lfbn = np && gz >= g.n[2] + 1;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) fz[k] = face_flux(pl[k], m2[k], m1[k], a[4 + k], p1[k], lfbp, lfbn, nu);
+        }
+        float b1[4], c1[4];
+        if (I == 2) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) pu[k] = 0.5f * (a[4 + k] + p1[k]);
+        } else if (I == 0) {
+            v4(v, 2, 1, 0, 0, b1);
+            const float e1 = v1(v, 2, 1, 0, -1);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) pu[k] = 0.5f * ((k == 0 ? e1 : b1[k == 0 ? 0 : k - 1]) + b1[k]);
+        } else {
+            v4(v, 2, 1, -1, 0, b1); v4(v, 2, 1, 0, 0, c1);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) pu[k] = 0.5f * (b1[k] + c1[k]);
+        }
+        const bool ufbp = np && gz + 1 <= 1 + (I == 2 ? 1 : 0), ufbn = np && gz + 1 >= g.n[2] + 1;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const float up = face_flux(pu[k], m1[k], a[4 + k], p1[k], p2[k], ufbp, ufbn, nu);
+            o.fzd[k] = fz[k] - up;
+            fz[k] = up;
+        }
+    }
+}
+
+// output phase: r = rx + (fyl - fyu) + fzd; f = u0 + dt r - V; B = V + mu0 f; predictor u = B, corrector u = (u' + B)/2
+template <int ND, int I>
+__device__ __forceinline__ void cd2_output(const FlowP& P, int gx, int gy, int gz, int nv, const Cd2Part& q, const float (&fyu)[4],
+                                           const float* __restrict__ u0, const float* __restrict__ mu0, float* __restrict__ out,
+                                           float dt, float Vi, int corrector)
+{
+    const Grid& g = P.g;
+    if (nv <= 0) return;
+    float o[4], uu[4], mm[4];
+    const int64_t id = gidx(g, gx, gy, gz);
+    unpack4(ld4(mu0 + I * g.nalloc, id), mm);
+    if (corrector) unpack4(ld4(u0 + I * g.nalloc, id), uu);
+    else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) uu[k] = q.wc[k];
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        float r = q.rx[k];
+        r += q.fyl[k] - fyu[k];
+        if (ND == 3) r += q.fzd[k];
+        const float f = uu[k] + dt * r - Vi;
+        const float B = Vi + mm[k] * f;
+        o[k] = corrector ? 0.5f * (q.wc[k] + B) : B;
+    }
+    st4(out + I * g.nalloc, id, o, nv);
+    if (I == 0 && corrector && P.exit_bc) {       // the corrector carries the convective-exit plane over (R-N)
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (gx + k == g.n[0]) out[id + k + 1] = q.wc[k + 1];
+    }
+}
+
+template <int ND>
+__global__ void __launch_bounds__(CD2_NT(ND), 1) k_cd_tile2(FlowP P, CdT T, const float* __restrict__ w, const float* __restrict__ u0,
+                                                            const float* __restrict__ mu0, float* __restrict__ out,
+                                                            const DevScal* __restrict__ ds, int corrector)
+{
+    extern __shared__ float4 cd_smem[];
+    float* ring = reinterpret_cast<float*>(cd_smem);
+    const Grid& g = P.g;
+    const float dt = ds->dt;
+    constexpr int NP = ND == 3 ? CD_NP : 1;
+    constexpr int SLOT = ND * CD_PLANE;            // floats per ring slot
+    float4* ex = reinterpret_cast<float4*>(ring + NP * SLOT);      // [ND][CD_TY][CD_TX] lower-y-face fluxes of the plane
+    const int comp = threadIdx.x / CD_NT, t2 = threadIdx.x - comp * CD_NT;
+    const float Vi = ds->vel[comp];
+    CdView v;
+    v.tx = t2 & (CD_TX - 1);
+    v.ty = t2 / CD_TX;
+    const bool top = v.ty == CD_TY - 1;
+    for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
+        const int tix = tile % T.ntx, rem = tile / T.ntx;
+        const int tiy = rem % T.nty, tiz = rem / T.nty;
+        const int bx = 1 + 4 * CD_TX * tix, by = 1 + CD_TY * tiy;
+        const int z0 = ND == 3 ? 1 + T.zc * tiz : 0;
+        const int z1 = ND == 3 ? min(z0 + T.zc - 1, g.n[2]) : 0;
+        const int gx = bx + 4 * v.tx, gy = by + v.ty;
+        int nv = g.n[0] - gx + 1;
+        nv = nv > 4 ? 4 : nv;
+        if (gy > g.n[1]) nv = 0;
+        __syncthreads();                           // the previous tile's reads are done
+        {
+            float4 st[CD2_STAGE(ND)];
+#pragma unroll 1
+            for (int d = 0; d < NP; ++d) {
+                const int cz = ND == 3 ? src_coord(z0 - 2 + d, g.n[2], g.per[2]) : 0;
+                cd2_load_regs<ND>(g, w, bx, by, cz, st);
+                cd2_store_regs<ND>(ring + d * SLOT, st);
+            }
+        }
+        __syncthreads();
+        int s0 = 0;                                // ring slot of plane z-2
+        float fz[4] = { 0.f, 0.f, 0.f, 0.f };      // flux through the upper z face of the previous plane
+#pragma unroll 1
+        for (int z = z0; z <= z1; ++z) {
+            float4 st[CD2_STAGE(ND)];
+            const bool more = ND == 3 && z < z1;
+            if (more) cd2_load_regs<ND>(g, w, bx, by, src_coord(z + 3, g.n[2], g.per[2]), st);
+#pragma unroll
+            for (int d = 0; d < NP; ++d) {
+                int s = s0 + d;
+                if (s >= NP) s -= NP;
+#pragma unroll
+                for (int c = 0; c < ND; ++c) v.p[c][ND == 3 ? d : 2] = ring + s * SLOT + c * CD_PLANE;
+            }
+            Cd2Part q;
+            const bool first = z == z0;
+            if (comp == 0)      cd2_fluxes<ND, 0>(P, v, gx, gy, z, top, first, fz, q);
+            else if (comp == 1) cd2_fluxes<ND, 1>(P, v, gx, gy, z, top, first, fz, q);
+            else if (ND == 3)   cd2_fluxes<ND, 2>(P, v, gx, gy, z, top, first, fz, q);
+            ex[(comp * CD_TY + v.ty) * CD_TX + v.tx] = make_float4(q.fyl[0], q.fyl[1], q.fyl[2], q.fyl[3]);
+            __syncthreads();                       // every lower-y-face flux of the plane is in shared memory
+            float fyu[4];
+            if (top) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) fyu[k] = q.fyu[k];
+            } else {
+                unpack4(ex[(comp * CD_TY + v.ty + 1) * CD_TX + v.tx], fyu);
+            }
+            if (comp == 0)      cd2_output<ND, 0>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
+            else if (comp == 1) cd2_output<ND, 1>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
+            else if (ND == 3)   cd2_output<ND, 2>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
+            if (more) {
+                __syncthreads();
+                cd2_store_regs<ND>(ring + s0 * SLOT, st);
+                s0 = s0 + 1 == NP ? 0 : s0 + 1;
+                __syncthreads();
+            }
+        }
+    }
+}
+
 // ====================================================================== the band kernel
 template <int ND, int I>
 __device__ __forceinline__ void band_face(const FlowP& P, const float* __restrict__ w, const float* __restrict__ u0,
@@ -488,15 +768,27 @@ void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out,
     FlowP P = wl_flowp(s);
     CdT T = cd_tiling(s, P.g);
     const size_t smem = sizeof(float) * (size_t)(s->nd == 3 ? CD_NP : 1) * s->nd * CD_PLANE;
-    if (!s->cd_attr_set) {
+    if (!(s->cd_attr_set & 1)) {
         cudaFuncSetAttribute(k_cd_tile<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * CD_NP * 3 * CD_PLANE));
         cudaFuncSetAttribute(k_cd_tile<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * 2 * CD_PLANE));
-        s->cd_attr_set = 1;
+        s->cd_attr_set |= 1;
+    }
+    static const int cd2 = getenv("WL_CD2") ? atoi(getenv("WL_CD2")) : 1;     // 0: the one-thread-per-three-components kernel
+    const size_t smem2 = smem + sizeof(float4) * (size_t)s->nd * CD_NT;
+    if (cd2 && !(s->cd_attr_set & 2)) {
+        cudaFuncSetAttribute(k_cd_tile2<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * CD_NP * 3 * CD_PLANE + sizeof(float4) * 3 * CD_NT));
+        cudaFuncSetAttribute(k_cd_tile2<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * 2 * CD_PLANE + sizeof(float4) * 2 * CD_NT));
+        s->cd_attr_set |= 2;
     }
     {
         ProfScope ps(s, WLK_CONVDIFF);
-        if (s->nd == 3) k_cd_tile<3><<<T.ntiles, CD_NT, smem, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
-        else            k_cd_tile<2><<<T.ntiles, CD_NT, smem, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
+        if (cd2) {
+            if (s->nd == 3) k_cd_tile2<3><<<T.ntiles, CD2_NT(3), smem2, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
+            else            k_cd_tile2<2><<<T.ntiles, CD2_NT(2), smem2, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
+        } else {
+            if (s->nd == 3) k_cd_tile<3><<<T.ntiles, CD_NT, smem, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
+            else            k_cd_tile<2><<<T.ntiles, CD_NT, smem, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
+        }
     }
     if (s->cfg.body.kind != WL_BODY_NONE) {
         ProfScope ps(s, WLK_CONVDIFF_BAND);

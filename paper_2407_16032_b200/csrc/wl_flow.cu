@@ -49,13 +49,15 @@ __global__ void __launch_bounds__(512) k_measure(Grid g, Tiling T, BodyP b, cons
         for (int i = 0; i < ND; ++i) {
             float m0 = 1.0f, m1 = 0.0f, nrm[3] = { 0.f, 0.f, 0.f };
             if (b.kind != WLB_NONE) {
-                float xi[3];
+                double xi[3], nd[3];
 #pragma unroll
                 for (int k = 0; k < 3; ++k) {
                     double xf = (double)xc[k] - (k == i ? 0.5 : 0.0);
-                    xi[k] = k < ND ? (float)(xf - ctr[k]) : 0.0f;
+                    xi[k] = k < ND ? xf - ctr[k] : 0.0;
                 }
-                float d = body_sdf<ND>(b, xi, nrm);
+                const float d = (float)body_sdf<ND, double>(b, xi, nd);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) nrm[k] = (float)nd[k];
                 m0 = bdim_mu0(d, b.eps);
                 m1 = bdim_mu1(d, b.eps);
             }
@@ -241,7 +243,7 @@ __global__ void __launch_bounds__(512) k_force(Grid g, Tiling T, BodyP b, const 
             float xi[3], nrm[3];
 #pragma unroll
             for (int k = 0; k < 3; ++k) xi[k] = k < ND ? (float)(((double)c[k] - 0.5) - ctr[k]) : 0.0f;
-            float d = body_sdf<ND>(b, xi, nrm);
+            float d = body_sdf<ND, float>(b, xi, nrm);
             float kk = bdim_K(d, 1.0f);
             if (kk == 0.0f) continue;
             float pk = p[gidx(g, c[0], c[1], c[2])] * kk;

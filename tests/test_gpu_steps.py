@@ -58,10 +58,9 @@ SCALED = [
     ("C2_tgv3d_32", lambda: wi.baseline_config(1, scale=4), dict(tgv=True)),
     ("C3_sphere_64x32x32", lambda: wi.baseline_config(2, scale=4), dict()),
     ("C4_torus_128x64x64", lambda: wi.baseline_config(3, scale=4), dict()),
-    # C5 at 1/2 scale: at 1/4 scale (D = 12 cells) the METHOD itself amplifies a 1e-7 perturbation of u to 1.3e-4 in
-    # ten steps (oracle against oracle), which no fp32 implementation can stay under; at 1/2
-    # scale the same measurement gives 2.5e-5
-    ("C5_heaving_192x128x128", lambda: wi.baseline_config(4, scale=2), dict()),
+    # the most sensitive case: the method itself amplifies a 1e-7 perturbation of u to 1.3e-4 in these ten steps (oracle
+    # against oracle); the CUDA path stays at 2.8e-5 because k_measure evaluates the SDF in fp64
+    ("C5_heaving_96x64x64", lambda: wi.baseline_config(4, scale=4), dict()),
     ("2D_cylinder_exit_96x64", lambda: wi.make(ndim=2, dims=(96, 64), exit_bc=1, nu=0.05, body_kind=wi.BODY_SPHERE,
                                                centre=(24.3, 32.2), R=6.0), dict()),
 ]
@@ -84,7 +83,7 @@ def test_ten_steps_velocity(name, mk, opts):
     po = O(o, "p")[0]; pg = p.astype(np.float64)
     po = po - po[fluid].mean(); pg = pg - pg[fluid].mean()
     assert np.abs(pg - po)[fluid].max() <= 2e-3 * max(np.abs(po[fluid]).max(), 1e-30)
-    assert g.stats()["vcycles"] == [2, 2]
+    assert g.stats()["vcycles"] == [cfg["fixed_vcycles"]] * 2
     o.close(); g.close()
 
 
