@@ -412,6 +412,18 @@ __global__ void __launch_bounds__(CD_NT, 2) k_cd_tile(FlowP P, CdT T, const floa
 // it, and handed down through shared memory, (c) the flux through the upper z face is kept for the next plane of the
 // march, where it is the lower one.  41 instead of 63 fluxes per four cells of the three components, identical
 // values (a flux is the same expression of the same operands whichever thread evaluates it).
+// view of the ring for one thread: b[dz + 2] points at the thread's own float4 of component 0 in plane z+dz, so that
+// every stencil read is one shared load at a compile-time offset (component, row and group offsets are immediates)
+struct CdView2 { const float* b[CD_NP]; };
+__device__ __forceinline__ void v4(const CdView2& v, int comp, int dz, int dy, int dg, float* o)
+{
+    const float4 t = *reinterpret_cast<const float4*>(v.b[dz + 2] + comp * CD_PLANE + dy * CD_W + 4 * dg);
+    o[0] = t.x; o[1] = t.y; o[2] = t.z; o[3] = t.w;
+}
+__device__ __forceinline__ float v1(const CdView2& v, int comp, int dz, int dy, int col)
+{
+    return v.b[dz + 2][comp * CD_PLANE + dy * CD_W + col];
+}
 #define CD2_NT(ND) (CD_NT * (ND))
 #define CD2_STAGE(ND) ((CD_ITEMS(ND) + CD2_NT(ND) - 1) / CD2_NT(ND))
 
@@ -446,7 +458,7 @@ struct Cd2Part {
 // fluxes of component I at the thread's four cells of plane gz.  fz: in (unless `first`) the flux through the lower z
 // face left by the previous plane; out the flux through the upper z face.
 template <int ND, int I>
-__device__ __forceinline__ void cd2_fluxes(const FlowP& P, const CdView& v, int gx, int gy, int gz, bool top, bool first, float (&fz)[4], Cd2Part& o)
+__device__ __forceinline__ void cd2_fluxes(const FlowP& P, const CdView2& v, int gx, int gy, int gz, bool top, bool first, float (&fz)[4], Cd2Part& o)
 {
     const Grid& g = P.g;
     const float nu = P.nu;
@@ -617,17 +629,17 @@ __global__ void __launch_bounds__(CD2_NT(ND), 1) k_cd_tile2(FlowP P, CdT T, cons
     float4* ex = reinterpret_cast<float4*>(ring + NP * SLOT);      // [ND][CD_TY][CD_TX] lower-y-face fluxes of the plane
     const int comp = threadIdx.x / CD_NT, t2 = threadIdx.x - comp * CD_NT;
     const float Vi = ds->vel[comp];
-    CdView v;
-    v.tx = t2 & (CD_TX - 1);
-    v.ty = t2 / CD_TX;
-    const bool top = v.ty == CD_TY - 1;
+    CdView2 v;
+    const int tx = t2 & (CD_TX - 1), ty = t2 / CD_TX;
+    const int tofs = (ty + 2) * CD_W + 4 * (tx + 1);          // the thread's own group inside a plane
+    const bool top = ty == CD_TY - 1;
     for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
         const int tix = tile % T.ntx, rem = tile / T.ntx;
         const int tiy = rem % T.nty, tiz = rem / T.nty;
         const int bx = 1 + 4 * CD_TX * tix, by = 1 + CD_TY * tiy;
         const int z0 = ND == 3 ? 1 + T.zc * tiz : 0;
         const int z1 = ND == 3 ? min(z0 + T.zc - 1, g.n[2]) : 0;
-        const int gx = bx + 4 * v.tx, gy = by + v.ty;
+        const int gx = bx + 4 * tx, gy = by + ty;
         int nv = g.n[0] - gx + 1;
         nv = nv > 4 ? 4 : nv;
         if (gy > g.n[1]) nv = 0;
@@ -653,22 +665,21 @@ __global__ void __launch_bounds__(CD2_NT(ND), 1) k_cd_tile2(FlowP P, CdT T, cons
             for (int d = 0; d < NP; ++d) {
                 int s = s0 + d;
                 if (s >= NP) s -= NP;
-#pragma unroll
-                for (int c = 0; c < ND; ++c) v.p[c][ND == 3 ? d : 2] = ring + s * SLOT + c * CD_PLANE;
+                v.b[ND == 3 ? d : 2] = ring + s * SLOT + tofs;
             }
             Cd2Part q;
             const bool first = z == z0;
             if (comp == 0)      cd2_fluxes<ND, 0>(P, v, gx, gy, z, top, first, fz, q);
             else if (comp == 1) cd2_fluxes<ND, 1>(P, v, gx, gy, z, top, first, fz, q);
             else if (ND == 3)   cd2_fluxes<ND, 2>(P, v, gx, gy, z, top, first, fz, q);
-            ex[(comp * CD_TY + v.ty) * CD_TX + v.tx] = make_float4(q.fyl[0], q.fyl[1], q.fyl[2], q.fyl[3]);
+            ex[(comp * CD_TY + ty) * CD_TX + tx] = make_float4(q.fyl[0], q.fyl[1], q.fyl[2], q.fyl[3]);
             __syncthreads();                       // every lower-y-face flux of the plane is in shared memory
             float fyu[4];
             if (top) {
 #pragma unroll
                 for (int k = 0; k < 4; ++k) fyu[k] = q.fyu[k];
             } else {
-                unpack4(ex[(comp * CD_TY + v.ty + 1) * CD_TX + v.tx], fyu);
+                unpack4(ex[(comp * CD_TY + ty + 1) * CD_TX + tx], fyu);
             }
             if (comp == 0)      cd2_output<ND, 0>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
             else if (comp == 1) cd2_output<ND, 1>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);

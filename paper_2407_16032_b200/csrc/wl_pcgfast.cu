@@ -135,12 +135,6 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
         const float* st = raw + slot * SP;
         float* eb = ebuf + (p & 1) * PL;
         const bool bz = PLB && fa_bnd(p, g.n[2], g.per[2]);     // block-uniform
-        const int zo = GEN ? fa_src(p, g.n[2], g.per[2]) * sz : 0;
-        if (GEN) {                            // a tile cut by a body: 1/D is loaded, at the positions the operands came from
-            if (own) unpack4(ld4(iD, off_own + zo), d_in);
-            if (full && hrow) unpack4(ld4(iD, off_h + zo), dh_in);
-            if (full && hcol) dx_in = ld1(iD, off_x + zo);
-        }
         if (!own) {
 #pragma unroll
             for (int k = 0; k < 4; ++k) { ep[k] = 0.0f; rm[k] = 0.0f; }
@@ -169,14 +163,25 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
         }
     };
 
+    // a tile cut by a body (GEN): 1/D of plane p is loaded, at the positions the operands come from, BEFORE the wait for
+    // the plane's operands, so that its latency hides behind that wait
+    auto load_iD = [&](int p, bool full) {
+        const int zo = fa_src(p, g.n[2], g.per[2]) * sz;
+        if (own) unpack4(ld4(iD, off_own + zo), d_in);
+        if (full && hrow) unpack4(ld4(iD, off_h + zo), dh_in);
+        if (full && hcol) dx_in = ld1(iD, off_x + zo);
+    };
+
     __syncthreads();                          // the previous tile's shared planes are no longer read
     // ---- prologue: planes z0-1 (own column only) in slot FA_S-1, z0 (full) in slot 0, then FA_S-1 planes ahead
     float zm[4], zc[4], zp[4], rmc[4] = { 0.f, 0.f, 0.f, 0.f }, rmp[4] = { 0.f, 0.f, 0.f, 0.f }, dummy[4];
     issue(z0 - 1, FA_S - 1);
     issue(z0, 0);
+    if (GEN) load_iD(z0 - 1, false);
     cp_wait<0>();
     __syncthreads();
     form(z0 - 1, FA_S - 1, zm, dummy, false);
+    if (GEN) load_iD(z0, true);
     form(z0, 0, zc, rmc, true);
     __syncthreads();                          // slot FA_S-1 is free again
 #pragma unroll
@@ -185,6 +190,18 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
     // ---- march
     for (int z = z0; z <= z1; ++z) {
         const int sn = sl + 1 == FA_S ? 0 : sl + 1;       // slot of plane z+1
+        float lx[5] = { 0.f, 0.f, 0.f, 0.f, 0.f }, ly[4] = { 0.f, 0.f, 0.f, 0.f }, lyp[4] = { 0.f, 0.f, 0.f, 0.f };
+        float lz[4] = { 0.f, 0.f, 0.f, 0.f }, lzp[4] = { 0.f, 0.f, 0.f, 0.f };
+        if (GEN) {                            // 1/D of plane z+1 and the face coefficients of the own cells of plane z (L = mu0 on level 0)
+            load_iD(z + 1, true);
+            if (valid) {
+                const int i = off_own + z * sz;
+                const float4 a = ld4(L, i);
+                lx[0] = a.x; lx[1] = a.y; lx[2] = a.z; lx[3] = a.w; lx[4] = ld1(L, i + 4);
+                unpack4(ld4(L + g.nalloc, i), ly); unpack4(ld4(L + g.nalloc, i + sy), lyp);
+                unpack4(ld4(L + 2 * g.nalloc, i), lz); unpack4(ld4(L + 2 * g.nalloc, i + sz), lzp);
+            }
+        }
         cp_wait<FA_S - 2>();                  // plane z+1 has landed (this thread's copies) ...
         __syncthreads();                      // ... and everybody's; e'(z) in shared is complete; the slot of plane z is free
         issue(z + FA_S, sl);
@@ -201,16 +218,7 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
         const float w[6] = { xm, zc[0], zc[1], zc[2], zc[3], xp };
         const float ymv[4] = { ym.x, ym.y, ym.z, ym.w }, ypv[4] = { yp.x, yp.y, yp.z, yp.w };
         float qq[4];
-        if (GEN) {                            // face coefficients of the own cells from L (= mu0 on level 0)
-            float lx[5] = { 0.f, 0.f, 0.f, 0.f, 0.f }, ly[4] = { 0.f, 0.f, 0.f, 0.f }, lyp[4] = { 0.f, 0.f, 0.f, 0.f };
-            float lz[4] = { 0.f, 0.f, 0.f, 0.f }, lzp[4] = { 0.f, 0.f, 0.f, 0.f };
-            if (valid) {
-                const int i = off_own + z * sz;
-                const float4 a = ld4(L, i);
-                lx[0] = a.x; lx[1] = a.y; lx[2] = a.z; lx[3] = a.w; lx[4] = ld1(L, i + 4);
-                unpack4(ld4(L + g.nalloc, i), ly); unpack4(ld4(L + g.nalloc, i + sy), lyp);
-                unpack4(ld4(L + 2 * g.nalloc, i), lz); unpack4(ld4(L + 2 * g.nalloc, i + sz), lzp);
-            }
+        if (GEN) {
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const float ec = w[k + 1];
