@@ -15,6 +15,10 @@
 // one-cell neighbourhood, a few per cent of a level) take the same route; they load 1/D where e' is
 // formed and the face coefficients of their own cells where the stencil is applied, unprefetched.
 #include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <cuda.h>
+#include <cudaTypedefs.h>
 #include "wl_internal.h"
 
 #ifndef WL_FA_MINB
@@ -34,6 +38,34 @@ __device__ __forceinline__ void cp4(unsigned d, const float* gsrc)
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// ---- bulk asynchronous copies (TMA engine, cp.async.bulk) completing on an mbarrier
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "FA_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra FA_DONE;\n"
+        "bra FA_WAIT;\n"
+        "FA_DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// one box of a 3-D tensor map (x fastest) into shared memory; completes `bytes of the box` on the mbarrier
+__device__ __forceinline__ void tma_box3(unsigned dst, const CUtensorMap* tm, int c0, int c1, int c2, unsigned bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
 
 // source coordinate of a (possibly halo) coordinate c of a direction with n cells: periodic wrap,
 // otherwise the ghost cells 0 and n+1 of the padded array (never written: zero); anything further out
@@ -58,15 +90,23 @@ __device__ __forceinline__ float fa_dir(float ee, float rr, float d, float beta,
 // One tile.  MODE (static): TM_PLB, the tile touches a non-periodic domain boundary and coefficients and 1/D
 // depend on the cell position; TM_PLI, they are the constants Lc and iDc; TM_GEN, they are loaded.  Everything that does not depend on the plane is
 // computed once per tile; the stage of a plane rotates through FA_S slots without a division.
-template <int FIRST, int MODE, int LXL>
+// BULK (static): an operand plane of the tile (cells x0-4 .. x0+4LX+3 of rows y0-1 .. y0+LY: both halos included) arrives as
+// ONE TMA box per array (cp.async.bulk.tensor.3d on a tensor map of the padded array), issued by one thread and completing
+// on one mbarrier per stage, instead of one to three cp.async per thread: no per-thread copy instructions or address
+// arithmetic.  Requires non-periodic x and y (a box cannot wrap; z wraps through the plane coordinate) and tiles that do not
+// stick out of the row.
+template <int FIRST, int MODE, int LXL, int BULK>
 __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, float Lc, float iDc, const FaTab& T, float beta, float m,
                                         const float* __restrict__ ein, const float* __restrict__ r, const float* __restrict__ L, const float* __restrict__ iD,
-                                        float* __restrict__ eout, float* __restrict__ q, float* raw, float* ebuf, double (&acc)[2])
+                                        float* __restrict__ eout, float* __restrict__ q, float* raw, float* ebuf, double (&acc)[2],
+                                        unsigned mbar, unsigned& phases, const CUtensorMap* tm_r, const CUtensorMap* tm_e)
 {
     constexpr bool PLB = MODE == TM_PLB, GEN = MODE == TM_GEN;
     constexpr int NA = FIRST ? 1 : 2;
     constexpr int LX = 1 << LXL, LY = WL_VB >> LXL;
-    constexpr int RW = 4 * LX + 8, PL = RW * (LY + 2), SP = NA * PL;
+    constexpr int RW = 4 * LX + 8, PL = RW * (LY + 2);
+    constexpr int PLR = BULK ? (PL + 31) / 32 * 32 : PL;      // raw planes of the TMA path start on 128-byte boundaries
+    constexpr int SP = NA * PLR;
     const int tid = threadIdx.x, tx = tid & (LX - 1), ty = tid >> LXL;
     const int tix = tile % vt.ntx, rem = tile / vt.ntx, tiy = rem % vt.nty, tiz = rem / vt.nty;
     const int x0 = 1 + 4 * LX * tix, y0 = 1 + LY * tiy;
@@ -100,12 +140,23 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
     const unsigned sraw = (unsigned)__cvta_generic_to_shared(raw);
     // plane p into stage slot `slot`
     auto issue = [&](int p, int slot) {
+        if (BULK) {
+            if (p <= z1 + 1 && tid == 0) {
+                const unsigned bar = mbar + 8u * (unsigned)slot;
+                const unsigned dst = sraw + 4u * (unsigned)(slot * SP);
+                const int zc_ = fa_src(p, g.n[2], g.per[2]);
+                mbar_expect_tx(bar, (unsigned)(NA * PL * 4));
+                tma_box3(dst, tm_r, WL_OFF + x0 - 4, y0 - 1, zc_, bar);
+                if (!FIRST) tma_box3(dst + 4u * PLR, tm_e, WL_OFF + x0 - 4, y0 - 1, zc_, bar);
+            }
+            return;
+        }
         if (p <= z1 + 1) {
             const unsigned st = sraw + 4u * (unsigned)(slot * SP);
             const int zo = fa_src(p, g.n[2], g.per[2]) * sz;
-            if (own) { cp16(st + 4u * idx_own, r + (off_own + zo)); if (!FIRST) cp16(st + 4u * (PL + idx_own), ein + (off_own + zo)); }
-            if (hrow) { cp16(st + 4u * idx_h, r + (off_h + zo)); if (!FIRST) cp16(st + 4u * (PL + idx_h), ein + (off_h + zo)); }
-            if (hcol) { cp4(st + 4u * idx_x, r + (off_x + zo)); if (!FIRST) cp4(st + 4u * (PL + idx_x), ein + (off_x + zo)); }
+            if (own) { cp16(st + 4u * idx_own, r + (off_own + zo)); if (!FIRST) cp16(st + 4u * (PLR + idx_own), ein + (off_own + zo)); }
+            if (hrow) { cp16(st + 4u * idx_h, r + (off_h + zo)); if (!FIRST) cp16(st + 4u * (PLR + idx_h), ein + (off_h + zo)); }
+            if (hcol) { cp4(st + 4u * idx_x, r + (off_x + zo)); if (!FIRST) cp4(st + 4u * (PLR + idx_x), ein + (off_x + zo)); }
         }
         cp_commit();                          // one group per plane, empty past the end: the wait counts stay fixed
     };
@@ -141,7 +192,7 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
         } else {
             const float4 rr = *reinterpret_cast<const float4*>(st + idx_own);
             float4 ee = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (!FIRST) ee = *reinterpret_cast<const float4*>(st + PL + idx_own);
+            if (!FIRST) ee = *reinterpret_cast<const float4*>(st + PLR + idx_own);
             ep[0] = fa_dir<FIRST>(ee.x, rr.x, bz ? d_bz[0] : d_in[0], beta, m); ep[1] = fa_dir<FIRST>(ee.y, rr.y, bz ? d_bz[1] : d_in[1], beta, m);
             ep[2] = fa_dir<FIRST>(ee.z, rr.z, bz ? d_bz[2] : d_in[2], beta, m); ep[3] = fa_dir<FIRST>(ee.w, rr.w, bz ? d_bz[3] : d_in[3], beta, m);
             if (FIRST) { rm[0] = rr.x - m; rm[1] = rr.y - m; rm[2] = rr.z - m; rm[3] = rr.w - m; }
@@ -151,14 +202,14 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
         if (hrow) {
             const float4 rr = *reinterpret_cast<const float4*>(st + idx_h);
             float4 ee = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (!FIRST) ee = *reinterpret_cast<const float4*>(st + PL + idx_h);
+            if (!FIRST) ee = *reinterpret_cast<const float4*>(st + PLR + idx_h);
             *reinterpret_cast<float4*>(eb + idx_h) =
                 make_float4(fa_dir<FIRST>(ee.x, rr.x, bz ? dh_bz[0] : dh_in[0], beta, m), fa_dir<FIRST>(ee.y, rr.y, bz ? dh_bz[1] : dh_in[1], beta, m),
                             fa_dir<FIRST>(ee.z, rr.z, bz ? dh_bz[2] : dh_in[2], beta, m), fa_dir<FIRST>(ee.w, rr.w, bz ? dh_bz[3] : dh_in[3], beta, m));
         }
         if (hcol) {
             const float rr = st[idx_x];
-            const float ee = FIRST ? 0.0f : st[PL + idx_x];
+            const float ee = FIRST ? 0.0f : st[PLR + idx_x];
             eb[idx_x] = fa_dir<FIRST>(ee, rr, bz ? dx_bz : dx_in, beta, m);
         }
     };
@@ -175,11 +226,15 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
     __syncthreads();                          // the previous tile's shared planes are no longer read
     // ---- prologue: planes z0-1 (own column only) in slot FA_S-1, z0 (full) in slot 0, then FA_S-1 planes ahead
     float zm[4], zc[4], zp[4], rmc[4] = { 0.f, 0.f, 0.f, 0.f }, rmp[4] = { 0.f, 0.f, 0.f, 0.f }, dummy[4];
+    auto arrived = [&](int slot) {            // BULK: the plane in `slot` has landed (all threads wait on its barrier)
+        mbar_wait(mbar + 8u * (unsigned)slot, (phases >> slot) & 1u);
+        phases ^= 1u << slot;
+    };
     issue(z0 - 1, FA_S - 1);
     issue(z0, 0);
     if (GEN) load_iD(z0 - 1, false);
-    cp_wait<0>();
-    __syncthreads();
+    if (BULK) { arrived(FA_S - 1); arrived(0); }
+    else { cp_wait<0>(); __syncthreads(); }
     form(z0 - 1, FA_S - 1, zm, dummy, false);
     if (GEN) load_iD(z0, true);
     form(z0, 0, zc, rmc, true);
@@ -202,7 +257,8 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
                 unpack4(ld4(L + 2 * g.nalloc, i), lz); unpack4(ld4(L + 2 * g.nalloc, i + sz), lzp);
             }
         }
-        cp_wait<FA_S - 2>();                  // plane z+1 has landed (this thread's copies) ...
+        if (BULK) arrived(sn);
+        else cp_wait<FA_S - 2>();             // plane z+1 has landed (this thread's copies) ...
         __syncthreads();                      // ... and everybody's; e'(z) in shared is complete; the slot of plane z is free
         issue(z + FA_S, sl);
         form(z + 1, sn, zp, rmp, true);
@@ -257,16 +313,17 @@ __device__ __forceinline__ void fa_tile(const Grid& g, const VT& vt, int tile, f
         for (int k = 0; k < 4; ++k) { zm[k] = zc[k]; zc[k] = zp[k]; rmc[k] = rmp[k]; }
         sl = sn;
     }
-    cp_wait<0>();                             // drain the (empty) tail groups before the stages are reused
+    if (!BULK) cp_wait<0>();                  // drain the (empty) tail groups before the stages are reused
 }
 
-template <int FIRST, int LXL>
+template <int FIRST, int LXL, int BULK>
 __global__ void __launch_bounds__(WL_VB, WL_FA_MINB) k_pcg_A_fast(Grid g, VT vt, const int* __restrict__ plain, float Lc, float iDc,
                                                           const float* __restrict__ ein, const float* __restrict__ r,
                                                           const float* __restrict__ L, const float* __restrict__ iD,
-                                                          float* __restrict__ eout, float* __restrict__ q, PcgScal* sc, RedBuf rb)
+                                                          float* __restrict__ eout, float* __restrict__ q, PcgScal* sc, RedBuf rb,
+                                                          const __grid_constant__ CUtensorMap tm_r, const __grid_constant__ CUtensorMap tm_e)
 {
-    extern __shared__ float4 fa_smem4[];
+    extern __shared__ __align__(128) float4 fa_smem4[];
     float* sm = reinterpret_cast<float*>(fa_smem4);
     if (!FIRST && !sc->live) return;          // uniform across the grid: written by an earlier kernel
     const float beta = FIRST ? 0.0f : (float)sc->beta;
@@ -275,15 +332,26 @@ __global__ void __launch_bounds__(WL_VB, WL_FA_MINB) k_pcg_A_fast(Grid g, VT vt,
     constexpr int LX = 1 << LXL, LY = WL_VB >> LXL;
     constexpr int PL = (4 * LX + 8) * (LY + 2);   // floats per shared plane: rows y0-1 .. y0+LY of [3 pad][x0-1][4 LX cells][x0+4LX][3 pad]
     float* raw = sm;                          // [FA_S][NA][PL]
-    float* ebuf = sm + FA_S * NA * PL;        // [2][PL]   e' of the plane being computed / the next one
+    constexpr int PLR = BULK ? (PL + 31) / 32 * 32 : PL;
+    float* ebuf = sm + FA_S * NA * PLR;       // [2][PL]   e' of the plane being computed / the next one
+    const unsigned mbar = (unsigned)__cvta_generic_to_shared(sm + FA_S * NA * PLR + 2 * PL);     // [FA_S] stage barriers (BULK)
+    unsigned phases = 0;                      // parity of the next completion of each stage barrier
+    if (BULK) {
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int k = 0; k < FA_S; ++k) mbar_init(mbar + 8u * k, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncthreads();
+    }
     FaTab T;
     T.t0 = 1.0f / (-6.0f * Lc); T.t1 = 1.0f / (-5.0f * Lc); T.t2 = 1.0f / (-4.0f * Lc); T.t3 = 1.0f / (-3.0f * Lc);
     double acc[2] = { 0.0, 0.0 };
     for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
         const int mode = plain[tile];         // block-uniform
-        if (mode == TM_PLI)      fa_tile<FIRST, TM_PLI, LXL>(g, vt, tile, Lc, iDc, T, beta, m, ein, r, L, iD, eout, q, raw, ebuf, acc);
-        else if (mode == TM_PLB) fa_tile<FIRST, TM_PLB, LXL>(g, vt, tile, Lc, iDc, T, beta, m, ein, r, L, iD, eout, q, raw, ebuf, acc);
-        else                     fa_tile<FIRST, TM_GEN, LXL>(g, vt, tile, Lc, iDc, T, beta, m, ein, r, L, iD, eout, q, raw, ebuf, acc);
+        if (mode == TM_PLI)      fa_tile<FIRST, TM_PLI, LXL, BULK>(g, vt, tile, Lc, iDc, T, beta, m, ein, r, L, iD, eout, q, raw, ebuf, acc, mbar, phases, &tm_r, &tm_e);
+        else if (mode == TM_PLB) fa_tile<FIRST, TM_PLB, LXL, BULK>(g, vt, tile, Lc, iDc, T, beta, m, ein, r, L, iD, eout, q, raw, ebuf, acc, mbar, phases, &tm_r, &tm_e);
+        else                     fa_tile<FIRST, TM_GEN, LXL, BULK>(g, vt, tile, Lc, iDc, T, beta, m, ein, r, L, iD, eout, q, raw, ebuf, acc, mbar, phases, &tm_r, &tm_e);
     }
     if (grid_reduce<2, OpSum>(acc, rb)) {
         if (threadIdx.x == 0) {
@@ -300,11 +368,29 @@ __global__ void __launch_bounds__(WL_VB, WL_FA_MINB) k_pcg_A_fast(Grid g, VT vt,
     }
 }
 
-size_t wl_pcg_fast_smem(const VT& vt, int first)
+size_t wl_pcg_fast_smem(const VT& vt, int first, int bulk)
 {
     const int LX = 1 << vt.lxl, LY = WL_VB >> vt.lxl;
-    const size_t PL = (size_t)(4 * LX + 8) * (LY + 2);
-    return sizeof(float) * PL * (FA_S * (first ? 1 : 2) + 2);
+    const size_t PL = (size_t)(4 * LX + 8) * (LY + 2), PLR = bulk ? (PL + 31) / 32 * 32 : PL;
+    return sizeof(float) * (PLR * FA_S * (first ? 1 : 2) + 2 * PL) + 8 * FA_S + 8;      // + the stage barriers
+}
+
+// tensor map of one padded scalar array of a level: dims (P, S1, S2), box = one tile plane with its halos
+static int fa_tensor_map(CUtensorMap* tm, const float* base, const Grid& g, int LX, int LY)
+{
+    static PFN_cuTensorMapEncodeTiled_v12000 enc = nullptr;
+    if (!enc) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn) return 0;
+        enc = (PFN_cuTensorMapEncodeTiled_v12000)fn;
+    }
+    const cuuint64_t dims[3] = { (cuuint64_t)g.P, (cuuint64_t)g.S[1], (cuuint64_t)g.S[2] };
+    const cuuint64_t strides[2] = { (cuuint64_t)g.sy * 4, (cuuint64_t)g.sz * 4 };
+    const cuuint32_t box[3] = { (cuuint32_t)(4 * LX + 8), (cuuint32_t)(LY + 2), 1 };
+    const cuuint32_t es[3] = { 1, 1, 1 };
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // levels the shared-memory kernel takes: 3-D, whole float4 groups per row, 32-bit element offsets, 8..32 threads along x
@@ -319,15 +405,24 @@ void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout)
 {
     Level& lv = s->lev[l];
     PcgScal* sc = &s->ds->pcg[l];
-    const size_t smem = wl_pcg_fast_smem(lv.vt, first);
     int grid = lv.vt.ntiles < s->sm_count * 4 ? lv.vt.ntiles : s->sm_count * 4;
     if (grid > WL_MAX_PARTIALS) grid = WL_MAX_PARTIALS;
     ProfScope ps_(s, WLK_PCG_MATVEC, l > 0);
-#define FA_LAUNCH(F, X) k_pcg_A_fast<F, X><<<grid, WL_VB, smem, s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, ein, lv.r, lv.L, lv.iD, eout, lv.q, sc, s->rb)
+#define FA_LAUNCH(F, X, B) k_pcg_A_fast<F, X, B><<<grid, WL_VB, smem, s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, ein, lv.r, lv.L, lv.iD, eout, lv.q, sc, s->rb, tm_r, tm_e)
+    // TMA boxes where one box is all a plane needs: 32 threads along x, no wrap in x or y, tiles that fill their rows
+    static const int bulk_on = getenv("WL_BULK") ? atoi(getenv("WL_BULK")) : 1;
+    int bulk = bulk_on && lv.vt.lxl == 5 && !lv.g.per[0] && !lv.g.per[1] && lv.vt.ngx % 32 == 0;
+    CUtensorMap tm_r, tm_e;
+    memset(&tm_r, 0, sizeof(tm_r)); memset(&tm_e, 0, sizeof(tm_e));
+    if (bulk) bulk = fa_tensor_map(&tm_r, lv.r, lv.g, 32, 8) && (first || fa_tensor_map(&tm_e, ein, lv.g, 32, 8));
+    const size_t smem = wl_pcg_fast_smem(lv.vt, first, bulk);
     switch (lv.vt.lxl) {
-    case 5: if (first) FA_LAUNCH(1, 5); else FA_LAUNCH(0, 5); break;
-    case 4: if (first) FA_LAUNCH(1, 4); else FA_LAUNCH(0, 4); break;
-    default: if (first) FA_LAUNCH(1, 3); else FA_LAUNCH(0, 3); break;    // wl_pcg_fast_ok() admits lxl 3..5 only
+    case 5:
+        if (bulk) { if (first) FA_LAUNCH(1, 5, 1); else FA_LAUNCH(0, 5, 1); }
+        else      { if (first) FA_LAUNCH(1, 5, 0); else FA_LAUNCH(0, 5, 0); }
+        break;
+    case 4: if (first) FA_LAUNCH(1, 4, 0); else FA_LAUNCH(0, 4, 0); break;
+    default: if (first) FA_LAUNCH(1, 3, 0); else FA_LAUNCH(0, 3, 0); break;    // wl_pcg_fast_ok() admits lxl 3..5 only
     }
 #undef FA_LAUNCH
 }
