@@ -107,7 +107,9 @@ static VT make_vt(int nd, const Grid& g, int level)
     const int lx = 1 << t.lxl, ly = WL_VB >> t.lxl;
     t.ntx = (t.ngx + lx - 1) / lx;
     t.nty = (g.n[1] + ly - 1) / ly;
-    t.zc = nd == 3 ? (g.n[2] < 8 ? g.n[2] : 8) : 1;
+    int zc0 = 8;
+    if (const char* e = getenv("WL_ZC")) { int v = atoi(e); if (v >= 1 && v <= 64) zc0 = v; }     // planes per tile (tuning)
+    t.zc = nd == 3 ? (g.n[2] < zc0 ? g.n[2] : zc0) : 1;
     if (level > 0 && (long long)g.n[0] * g.n[1] * g.n[2] <= pk_max_cells())
         while (t.zc > 1 && (int64_t)t.ntx * t.nty * ((g.n[2] + t.zc - 1) / t.zc) < 592) t.zc = (t.zc + 1) / 2;
     t.ntz = nd == 3 ? (g.n[2] + t.zc - 1) / t.zc : 1;
@@ -306,6 +308,8 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     }
     s->fast_A = 1;
     s->tiny_on = 1;
+    s->bulk_A = 1;
+    if (const char* e = getenv("WL_BULK")) s->bulk_A = atoi(e) != 0;
     if (const char* e = getenv("WL_TINY")) s->tiny_on = atoi(e) != 0;
     if (const char* e = getenv("WL_FAST_A")) s->fast_A = atoi(e) != 0;
     s->body.kind = cfg->body.kind; s->body.axis = cfg->body.axis;

@@ -7,13 +7,16 @@
 // flops.  What limits the register-marching kernel of wl_poisson.cu is not traffic but latency: 125
 // registers, two blocks per SM, every plane waits for its own loads.  Here the operands of a tile
 // (128 x 8 cells for 32 x 8 threads, one plane at a time, one halo row / column around it) are
-// brought in by cp.async three planes ahead of their use, so ~3 planes x 11 KB per block are in flight
-// without holding registers; e' is formed once per cell (and once per halo cell) into a shared plane,
-// and the seven-point stencil reads its y neighbours from there, its x neighbours by shuffle and its z
-// neighbours from the thread's own registers.  Face coefficients and 1/D are analytic (tile modes
-// TM_PLI / TM_PLB, wl_vec.cuh): nothing but e and r is loaded.  General tiles (TM_GEN: a body or its
-// one-cell neighbourhood, a few per cent of a level) take the same route; they load 1/D where e' is
-// formed and the face coefficients of their own cells where the stencil is applied, unprefetched.
+// brought into shared memory three planes ahead of their use -- as ONE TMA box per array and plane
+// (cp.async.bulk.tensor.3d on a tensor map of the padded array, completing on an mbarrier per stage)
+// where a box is all a plane needs, by per-thread cp.async otherwise (periodic x or y, ragged rows) --
+// so ~3 planes x 11 KB per block are in flight without holding registers; e' is formed once per cell
+// (and once per halo cell) into a shared plane, and the seven-point stencil reads its y neighbours
+// from there, its x neighbours by shuffle and its z neighbours from the thread's own registers.
+// Face coefficients and 1/D are analytic (tile modes TM_PLI / TM_PLB, wl_vec.cuh): nothing but e and
+// r is loaded.  General tiles (TM_GEN: a body or its one-cell neighbourhood, a few per cent of a
+// level) take the same route; they load 1/D and the face coefficients of their own cells before the
+// wait for the plane's operands.
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -24,7 +27,10 @@
 #ifndef WL_FA_MINB
 #define WL_FA_MINB 4
 #endif
-#define FA_S 3                    // raw stages: planes z+1 .. z+3 in flight while plane z is computed
+#ifndef FA_S
+#define FA_S 3
+#endif
+                                    // raw stages: planes z+1 .. z+3 in flight while plane z is computed
 
 // cp.async of 16 / 4 bytes; the destination is a 32-bit shared-window address
 __device__ __forceinline__ void cp16(unsigned d, const float* gsrc)
@@ -408,10 +414,14 @@ void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout)
     int grid = lv.vt.ntiles < s->sm_count * 4 ? lv.vt.ntiles : s->sm_count * 4;
     if (grid > WL_MAX_PARTIALS) grid = WL_MAX_PARTIALS;
     ProfScope ps_(s, WLK_PCG_MATVEC, l > 0);
-#define FA_LAUNCH(F, X, B) k_pcg_A_fast<F, X, B><<<grid, WL_VB, smem, s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, ein, lv.r, lv.L, lv.iD, eout, lv.q, sc, s->rb, tm_r, tm_e)
+#define FA_LAUNCH(F, X, B)                                                                                                          \
+    do {                                                                                                                           \
+        if (smem > 48 * 1024) cudaFuncSetAttribute(k_pcg_A_fast<F, X, B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+        k_pcg_A_fast<F, X, B><<<grid, WL_VB, smem, s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, ein, lv.r, lv.L, lv.iD, eout,     \
+                                                            lv.q, sc, s->rb, tm_r, tm_e);                                          \
+    } while (0)
     // TMA boxes where one box is all a plane needs: 32 threads along x, no wrap in x or y, tiles that fill their rows
-    static const int bulk_on = getenv("WL_BULK") ? atoi(getenv("WL_BULK")) : 1;
-    int bulk = bulk_on && lv.vt.lxl == 5 && !lv.g.per[0] && !lv.g.per[1] && lv.vt.ngx % 32 == 0;
+    int bulk = s->bulk_A && lv.vt.lxl == 5 && !lv.g.per[0] && !lv.g.per[1] && lv.vt.ngx % 32 == 0;
     CUtensorMap tm_r, tm_e;
     memset(&tm_r, 0, sizeof(tm_r)); memset(&tm_e, 0, sizeof(tm_e));
     if (bulk) bulk = fa_tensor_map(&tm_r, lv.r, lv.g, 32, 8) && (first || fa_tensor_map(&tm_e, ein, lv.g, 32, 8));

@@ -2,7 +2,7 @@
 (`k_pcg_A_fast`) against the register-marching one, the persistent coarse-level kernels (`k_coarse`, cooperative;
 `k_tiny`, one thread-block cluster) against stand-alone launches, a fused chain of coarse passes against the same
 passes launched one by one -- each against the fp64 oracle, and against one another.  The environment switches
-(WL_FAST_A, WL_TINY, WL_PK_MAX_CELLS) are read when a simulation is created."""
+(WL_FAST_A, WL_TINY, WL_PK_MAX_CELLS, WL_BULK) are read when a simulation is created."""
 import os
 
 import numpy as np
@@ -18,6 +18,7 @@ SWITCHES = [
     {"WL_FAST_A": "0"},                     # register-marching pass A everywhere
     {"WL_TINY": "0"},                       # tiny levels inside the cooperative kernel
     {"WL_PK_MAX_CELLS": "0"},               # every level by stand-alone kernels
+    {"WL_BULK": "0"},                       # pass A copies its planes with per-thread cp.async instead of TMA boxes
 ]
 
 
@@ -37,7 +38,10 @@ class _env:
                 os.environ[k] = v
 
 
-WIDE = [c for c in CASES if len(c[0]) == 3 and c[0][0] >= 136] + [((64, 64, 64), (0, 1, 0), 1, "sphere", False)]
+# the last two take the TMA path of pass A (rows of whole 128-cell tiles, no wrap in x and y)
+WIDE = [c for c in CASES if len(c[0]) == 3 and c[0][0] >= 136] + [((64, 64, 64), (0, 1, 0), 1, "sphere", False),
+                                                                   ((128, 40, 24), (0, 0, 0), 1, "sphere", False),
+                                                                   ((256, 24, 20), (0, 0, 1), 1, "torus", False)]
 
 
 @pytest.mark.parametrize("case", WIDE, ids=_ids)
