@@ -62,9 +62,9 @@ ALG_BYTES = {
 
 
 # DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the fine-level kernels on C4, from the
-# ncu --set full capture summarised in profiles/r1b_stages_c4_ncu.md (bytes; other workloads: not captured)
-NCU_TRAFFIC_C4 = {"pcg_update": 793e6, "pcg_matvec": 596e6, "residual": 919e6, "prolong": 572e6,
-                  "apply_gradient": 1085e6, "cfl": 442e6, "restrict": 159e6, "conv_diff_bdim": 1478e6}
+# ncu --set full capture summarised in profiles/r1c_stages_c4_ncu.md (bytes; other workloads: not captured)
+NCU_TRAFFIC_C4 = {"pcg_update": 793e6, "pcg_matvec": 593e6, "residual": 882e6, "prolong": 577e6,
+                  "apply_gradient": 1088e6, "cfl": 420e6, "restrict": 160e6, "conv_diff_bdim": 1430e6}
 
 
 def conv_alg_bytes(cfg) -> float:
@@ -344,7 +344,7 @@ def run_gpu(args) -> None:
                 "frac": (achieved / hbm_peak) if achieved else None, "frac_of_nominal_8TBs": (achieved / 8000.0) if achieved else None,
                 "peak_source": peak_src,
                 "traffic": NCU_TRAFFIC_C4.get(base) if args.workload == "C4" else None,
-                "traffic_source": "profiles/r1b_stages_c4_ncu.md (ncu --set full, one launch)" if args.workload == "C4" else None,
+                "traffic_source": "profiles/r1c_stages_c4_ncu.md (ncu --set full, one launch)" if args.workload == "C4" else None,
                 "alg_bytes_per_cell_per_launch": alg.get(base), "avg_launch_us": dom_ms / dom_n * 1e3,
                 "share_of_step": dom_ms / tot_prof,
                 "step": {"alg_bytes_per_cell_per_step": step_bytes / cells,
