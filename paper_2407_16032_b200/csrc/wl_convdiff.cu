@@ -17,6 +17,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include "wl_internal.h"
+#include "wl_tma.cuh"
 
 __device__ __forceinline__ float med3(float a, float b, float c)
 {
@@ -694,6 +695,104 @@ __global__ void __launch_bounds__(CD2_NT(ND), 1) k_cd_tile2(FlowP P, CdT T, cons
     }
 }
 
+// ---- k_cd_tile3: k_cd_tile2 with the ring filled by the TMA engine (3-D, non-periodic x and y).
+// A ring of SIX plane slots: while plane z is computed from the planes z-2 .. z+2, the box copies of plane z+3 (one
+// per component: cells bx-4 .. bx+131 of rows by-2 .. by+9, out-of-range parts zero-filled; z wraps through the plane
+// coordinate) land in the sixth slot, issued by one thread a whole plane ahead and completing on the slot's mbarrier.
+// No thread touches a global load for the ring, no register staging, and ONE block barrier per plane (the hand-over
+// of the y-face fluxes, double-buffered) instead of three.
+#define CD3_NP 6
+__global__ void __launch_bounds__(CD2_NT(3), 1) k_cd_tile3(FlowP P, CdT T, const float* __restrict__ u0, const float* __restrict__ mu0,
+                                                           float* __restrict__ out, const DevScal* __restrict__ ds, int corrector,
+                                                           const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1,
+                                                           const __grid_constant__ CUtensorMap tm2)
+{
+    constexpr int ND = 3;
+    extern __shared__ __align__(128) float4 cd_smem[];
+    float* ring = reinterpret_cast<float*>(cd_smem);
+    const Grid& g = P.g;
+    const float dt = ds->dt;
+    constexpr int SLOT = ND * CD_PLANE;            // floats per ring slot (a multiple of 32: slots stay 128-byte aligned)
+    float4* ex = reinterpret_cast<float4*>(ring + CD3_NP * SLOT);          // [2][ND][CD_TY][CD_TX] lower-y-face fluxes
+    const unsigned sring = (unsigned)__cvta_generic_to_shared(ring);
+    const unsigned mbar = (unsigned)__cvta_generic_to_shared(ex + 2 * ND * CD_NT);     // [CD3_NP] slot barriers
+    const int comp = threadIdx.x / CD_NT, t2 = threadIdx.x - comp * CD_NT;
+    const float Vi = ds->vel[comp];
+    CdView2 v;
+    const int tx = t2 & (CD_TX - 1), ty = t2 / CD_TX;
+    const int tofs = (ty + 2) * CD_W + 4 * (tx + 1);          // the thread's own group inside a plane
+    const bool top = ty == CD_TY - 1;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < CD3_NP; ++k) mbar_init(mbar + 8u * k, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    unsigned phases = 0;                           // parity of the next completion of each slot barrier
+    for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
+        const int tix = tile % T.ntx, rem = tile / T.ntx;
+        const int tiy = rem % T.nty, tiz = rem / T.nty;
+        const int bx = 1 + 4 * CD_TX * tix, by = 1 + CD_TY * tiy;
+        const int z0 = 1 + T.zc * tiz, z1 = min(z0 + T.zc - 1, g.n[2]);
+        const int gx = bx + 4 * tx, gy = by + ty;
+        int nv = g.n[0] - gx + 1;
+        nv = nv > 4 ? 4 : nv;
+        if (gy > g.n[1]) nv = 0;
+        // plane p of the tile (z0-2 <= p <= z1+2) lives in slot (p - z0 + 2) % CD3_NP
+        auto issue = [&](int p, int slot) {
+            const unsigned bar = mbar + 8u * (unsigned)slot, dst = sring + 4u * (unsigned)(slot * SLOT);
+            const int cz = src_coord(p, g.n[2], g.per[2]);
+            mbar_expect_tx(bar, (unsigned)(SLOT * 4));
+            tma_box3(dst, &tm0, WL_OFF + bx - 4, by - 2, cz, bar);
+            tma_box3(dst + 4u * CD_PLANE, &tm1, WL_OFF + bx - 4, by - 2, cz, bar);
+            tma_box3(dst + 8u * CD_PLANE, &tm2, WL_OFF + bx - 4, by - 2, cz, bar);
+        };
+        auto arrived = [&](int slot) {
+            mbar_wait(mbar + 8u * (unsigned)slot, (phases >> slot) & 1u);
+            phases ^= 1u << slot;
+        };
+        __syncthreads();                           // the previous tile's reads are done (and the barriers are initialised)
+        if (threadIdx.x == 0)
+            for (int d = 0; d < CD3_NP && z0 - 2 + d <= z1 + 2; ++d) issue(z0 - 2 + d, d);
+        for (int d = 0; d < 4; ++d) arrived(d);    // planes z0-2 .. z0+1; plane z+2 is awaited at the top of every step
+        int s0 = 0;                                // ring slot of plane z-2
+        float fz[4] = { 0.f, 0.f, 0.f, 0.f };      // flux through the upper z face of the previous plane
+#pragma unroll 1
+        for (int z = z0; z <= z1; ++z) {
+            {
+                int s = s0 + 4;
+                if (s >= CD3_NP) s -= CD3_NP;
+                arrived(s);                        // plane z+2
+            }
+#pragma unroll
+            for (int d = 0; d < CD_NP; ++d) {
+                int s = s0 + d;
+                if (s >= CD3_NP) s -= CD3_NP;
+                v.b[d] = ring + s * SLOT + tofs;
+            }
+            Cd2Part q;
+            const bool first = z == z0;
+            if (comp == 0)      cd2_fluxes<ND, 0>(P, v, gx, gy, z, top, first, fz, q);
+            else if (comp == 1) cd2_fluxes<ND, 1>(P, v, gx, gy, z, top, first, fz, q);
+            else                cd2_fluxes<ND, 2>(P, v, gx, gy, z, top, first, fz, q);
+            float4* exz = ex + (z & 1) * ND * CD_NT;
+            exz[(comp * CD_TY + ty) * CD_TX + tx] = make_float4(q.fyl[0], q.fyl[1], q.fyl[2], q.fyl[3]);
+            __syncthreads();                       // the lower-y-face fluxes of the plane are in shared memory; the ring reads of the plane are done
+            if (threadIdx.x == 0 && z + 4 <= z1 + 2) issue(z + 4, s0);     // into the slot plane z-2 occupied; needed two steps from now
+            float fyu[4];
+            if (top) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) fyu[k] = q.fyu[k];
+            } else {
+                unpack4(exz[(comp * CD_TY + ty + 1) * CD_TX + tx], fyu);
+            }
+            if (comp == 0)      cd2_output<ND, 0>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
+            else if (comp == 1) cd2_output<ND, 1>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
+            else                cd2_output<ND, 2>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
+            s0 = s0 + 1 == CD3_NP ? 0 : s0 + 1;
+        }
+    }
+}
+
 // ====================================================================== the band kernel
 template <int ND, int I>
 __device__ __forceinline__ void band_face(const FlowP& P, const float* __restrict__ w, const float* __restrict__ u0,
@@ -791,7 +890,21 @@ void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out,
         cudaFuncSetAttribute(k_cd_tile2<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * 2 * CD_PLANE + sizeof(float4) * 2 * CD_NT));
         s->cd_attr_set |= 2;
     }
-    {
+    // the TMA-fed kernel where a box never has to wrap in x or y (WL_CD3=0 switches it off)
+    static const int cd3_on = getenv("WL_CD3") ? atoi(getenv("WL_CD3")) : 1;
+    int cd3 = cd2 && cd3_on && s->nd == 3 && !P.g.per[0] && !P.g.per[1];
+    CUtensorMap tm[3];
+    if (cd3)
+        for (int c = 0; c < 3 && cd3; ++c) cd3 = wl_tensor_map3(&tm[c], w + c * P.g.nalloc, P.g, CD_W, CD_R);
+    if (cd3) {
+        const size_t smem3 = sizeof(float) * CD3_NP * 3 * CD_PLANE + sizeof(float4) * 2 * 3 * CD_NT + 8 * CD3_NP + 16;
+        if (!(s->cd_attr_set & 4)) {
+            cudaFuncSetAttribute(k_cd_tile3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3);
+            s->cd_attr_set |= 4;
+        }
+        ProfScope ps(s, WLK_CONVDIFF);
+        k_cd_tile3<<<T.ntiles, CD2_NT(3), smem3, s->st>>>(P, T, u0, s->mu0, out, s->ds, corrector, tm[0], tm[1], tm[2]);
+    } else {
         ProfScope ps(s, WLK_CONVDIFF);
         if (cd2) {
             if (s->nd == 3) k_cd_tile2<3><<<T.ntiles, CD2_NT(3), smem2, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);

@@ -20,9 +20,8 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
-#include <cuda.h>
-#include <cudaTypedefs.h>
 #include "wl_internal.h"
+#include "wl_tma.cuh"
 
 #ifndef WL_FA_MINB
 #define WL_FA_MINB 4
@@ -44,34 +43,6 @@ __device__ __forceinline__ void cp4(unsigned d, const float* gsrc)
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-// ---- bulk asynchronous copies (TMA engine, cp.async.bulk) completing on an mbarrier
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "FA_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra FA_DONE;\n"
-        "bra FA_WAIT;\n"
-        "FA_DONE:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-// one box of a 3-D tensor map (x fastest) into shared memory; completes `bytes of the box` on the mbarrier
-__device__ __forceinline__ void tma_box3(unsigned dst, const CUtensorMap* tm, int c0, int c1, int c2, unsigned bar)
-{
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                 ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
-}
 
 // source coordinate of a (possibly halo) coordinate c of a direction with n cells: periodic wrap,
 // otherwise the ghost cells 0 and n+1 of the padded array (never written: zero); anything further out
@@ -381,24 +352,6 @@ size_t wl_pcg_fast_smem(const VT& vt, int first, int bulk)
     return sizeof(float) * (PLR * FA_S * (first ? 1 : 2) + 2 * PL) + 8 * FA_S + 8;      // + the stage barriers
 }
 
-// tensor map of one padded scalar array of a level: dims (P, S1, S2), box = one tile plane with its halos
-static int fa_tensor_map(CUtensorMap* tm, const float* base, const Grid& g, int LX, int LY)
-{
-    static PFN_cuTensorMapEncodeTiled_v12000 enc = nullptr;
-    if (!enc) {
-        void* fn = nullptr;
-        cudaDriverEntryPointQueryResult qr;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn) return 0;
-        enc = (PFN_cuTensorMapEncodeTiled_v12000)fn;
-    }
-    const cuuint64_t dims[3] = { (cuuint64_t)g.P, (cuuint64_t)g.S[1], (cuuint64_t)g.S[2] };
-    const cuuint64_t strides[2] = { (cuuint64_t)g.sy * 4, (cuuint64_t)g.sz * 4 };
-    const cuuint32_t box[3] = { (cuuint32_t)(4 * LX + 8), (cuuint32_t)(LY + 2), 1 };
-    const cuuint32_t es[3] = { 1, 1, 1 };
-    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
 // levels the shared-memory kernel takes: 3-D, whole float4 groups per row, 32-bit element offsets, 8..32 threads along x
 int wl_pcg_fast_ok(const wl_sim* s, int l)
 {
@@ -424,7 +377,7 @@ void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout)
     int bulk = s->bulk_A && lv.vt.lxl == 5 && !lv.g.per[0] && !lv.g.per[1] && lv.vt.ngx % 32 == 0;
     CUtensorMap tm_r, tm_e;
     memset(&tm_r, 0, sizeof(tm_r)); memset(&tm_e, 0, sizeof(tm_e));
-    if (bulk) bulk = fa_tensor_map(&tm_r, lv.r, lv.g, 32, 8) && (first || fa_tensor_map(&tm_e, ein, lv.g, 32, 8));
+    if (bulk) bulk = wl_tensor_map3(&tm_r, lv.r, lv.g, 4 * 32 + 8, 8 + 2) && (first || wl_tensor_map3(&tm_e, ein, lv.g, 4 * 32 + 8, 8 + 2));
     const size_t smem = wl_pcg_fast_smem(lv.vt, first, bulk);
     switch (lv.vt.lxl) {
     case 5:
