@@ -309,6 +309,8 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     s->fast_A = 1;
     s->tiny_on = 1;
     s->bulk_A = 1;
+    s->cd_kernel = 3;
+    if (const char* e = getenv("WL_CD")) { int v = atoi(e); if (v >= 1 && v <= 3) s->cd_kernel = v; }
     if (const char* e = getenv("WL_BULK")) s->bulk_A = atoi(e) != 0;
     if (const char* e = getenv("WL_TINY")) s->tiny_on = atoi(e) != 0;
     if (const char* e = getenv("WL_FAST_A")) s->fast_A = atoi(e) != 0;

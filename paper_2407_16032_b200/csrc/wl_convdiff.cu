@@ -883,16 +883,15 @@ void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out,
         cudaFuncSetAttribute(k_cd_tile<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * 2 * CD_PLANE));
         s->cd_attr_set |= 1;
     }
-    static const int cd2 = getenv("WL_CD2") ? atoi(getenv("WL_CD2")) : 1;     // 0: the one-thread-per-three-components kernel
+    const int cd2 = s->cd_kernel >= 2;        // 1: k_cd_tile (three components per thread), 2: k_cd_tile2, 3: k_cd_tile3 where it applies
     const size_t smem2 = smem + sizeof(float4) * (size_t)s->nd * CD_NT;
     if (cd2 && !(s->cd_attr_set & 2)) {
         cudaFuncSetAttribute(k_cd_tile2<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * CD_NP * 3 * CD_PLANE + sizeof(float4) * 3 * CD_NT));
         cudaFuncSetAttribute(k_cd_tile2<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * 2 * CD_PLANE + sizeof(float4) * 2 * CD_NT));
         s->cd_attr_set |= 2;
     }
-    // the TMA-fed kernel where a box never has to wrap in x or y (WL_CD3=0 switches it off)
-    static const int cd3_on = getenv("WL_CD3") ? atoi(getenv("WL_CD3")) : 1;
-    int cd3 = cd2 && cd3_on && s->nd == 3 && !P.g.per[0] && !P.g.per[1];
+    // the TMA-fed kernel where a box never has to wrap in x or y
+    int cd3 = s->cd_kernel >= 3 && s->nd == 3 && !P.g.per[0] && !P.g.per[1];
     CUtensorMap tm[3];
     if (cd3)
         for (int c = 0; c < 3 && cd3; ++c) cd3 = wl_tensor_map3(&tm[c], w + c * P.g.nalloc, P.g, CD_W, CD_R);

@@ -2,7 +2,7 @@
 (`k_pcg_A_fast`) against the register-marching one, the persistent coarse-level kernels (`k_coarse`, cooperative;
 `k_tiny`, one thread-block cluster) against stand-alone launches, a fused chain of coarse passes against the same
 passes launched one by one -- each against the fp64 oracle, and against one another.  The environment switches
-(WL_FAST_A, WL_TINY, WL_PK_MAX_CELLS, WL_BULK) are read when a simulation is created."""
+(WL_FAST_A, WL_TINY, WL_PK_MAX_CELLS, WL_BULK, WL_CD) are read when a simulation is created."""
 import os
 
 import numpy as np
@@ -19,6 +19,8 @@ SWITCHES = [
     {"WL_TINY": "0"},                       # tiny levels inside the cooperative kernel
     {"WL_PK_MAX_CELLS": "0"},               # every level by stand-alone kernels
     {"WL_BULK": "0"},                       # pass A copies its planes with per-thread cp.async instead of TMA boxes
+    {"WL_CD": "2"},                         # conv_diff from the register-staged ring (k_cd_tile2) instead of the TMA-fed one
+    {"WL_CD": "1"},                         # conv_diff with three components per thread (k_cd_tile)
 ]
 
 
@@ -121,6 +123,30 @@ def test_fused_coarse_chain_equals_single_passes(case):
         o.close(); g.close()
     for (xa, ra), (xb, rb) in zip(*res):
         assert np.array_equal(xa, xb) and np.array_equal(ra, rb)       # same kernels, same order: bit-identical
+
+
+@pytest.mark.parametrize("kernel", ["1", "2", "3"])
+@pytest.mark.parametrize("case", [c for c in WIDE if not c[1][0] and not c[1][1]] + [CASES[1], CASES[4]], ids=_ids)
+def test_conv_diff_kernels_agree(case, kernel):
+    """conv_diff + BDIM + Heun through each of the three tile kernels (k_cd_tile, k_cd_tile2, the TMA-fed k_cd_tile3 where x and
+    y do not wrap): predictor and corrector against the oracle at the per-kernel tolerance."""
+    from paper_2407_16032_b200 import wl
+    cfg = _cfg(case)
+    for corrector in (0, 1):
+        o, _g = _sims(cfg)
+        _g.close()
+        with _env({"WL_CD": kernel}):
+            g = wl.Sim(cfg)
+        _load_state(o, g, case[0], seed=wi.SEED, p_too=False)
+        o.arr("u0")[...] = o.arr("u"); g.dbg_save_u0()
+        if corrector:
+            _load_state(o, g, case[0], seed=wi.SEED + 11, p_too=False)
+            o.conv_diff("u")
+        else:
+            o.conv_diff("u0")
+        o.bdim(0.31, corrector); g.dbg_conv_diff_bdim(0.31, corrector)
+        assert relerr(g.dbg_get("u"), O(o, "u")) <= TOL
+        o.close(); g.close()
 
 
 def test_smoother_removes_residual_mean_on_the_gpu():
