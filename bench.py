@@ -391,6 +391,18 @@ def run_gpu(args) -> None:
                                            "ms_per_step": ms / args.steps}
             s2.close()
             torch.cuda.empty_cache()
+        # the shape of the paper's headline figure (TGV 512^3, 134 M cells; here fully periodic and with
+        # the fixed two V-cycles of the BASELINE configs): context beside the paper's 1.57 ns on an H100, not a config
+        try:
+            c2 = wi.tgv3d(512)
+            s2, d0 = make_sim(c2, device)
+            ms = time_steps(torch, s2, d0, min(args.steps, 10), 3, None)
+            also["TGV3D_512_paper_headline_shape"] = {"cells": ncells(c2), "ns_per_cell_step": ms * 1e6 / (ncells(c2) * min(args.steps, 10)),
+                                                      "ms_per_step": ms / min(args.steps, 10)}
+            s2.close()
+        except Exception as e:                       # not enough free memory on a shared box: skip the context line
+            also["TGV3D_512_paper_headline_shape"] = {"skipped": str(e)[:120]}
+        torch.cuda.empty_cache()
 
     if rank != 0:
         if dist is not None:

@@ -27,7 +27,7 @@
 #define WL_B_MINB 4
 #endif
 #ifndef WL_TINY_CLUSTER
-#define WL_TINY_CLUSTER 8     // blocks of the k_tiny cluster (8 = portable maximum)
+#define WL_TINY_CLUSTER 16    // blocks of the k_tiny cluster (16 = the opt-in maximum on B200; 8 is the portable one)
 #endif
 #ifndef WL_TINY_TILES
 #define WL_TINY_TILES 16      // levels with at most this many tiles run in k_tiny
@@ -1026,6 +1026,11 @@ static void coarse_launch_one(wl_sim* s, const CoarseProg& prog, int tiny)
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = WL_TINY_CLUSTER; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
+        if (WL_TINY_CLUSTER > 8 && !(s->cd_attr_set & 8)) {     // cluster sizes above 8 are opt-in
+            cudaFuncSetAttribute(k_tiny<3>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            cudaFuncSetAttribute(k_tiny<2>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            s->cd_attr_set |= 8;
+        }
         if (s->nd == 3) cudaLaunchKernelEx(&cfg, k_tiny<3>, levs, prog, ds, part);
         else            cudaLaunchKernelEx(&cfg, k_tiny<2>, levs, prog, ds, part);
         return;
