@@ -316,10 +316,31 @@ void wl_k_set_time(wl_sim* s, double t, float dt, int t_mode, int dt_mode)
     k_set_time<<<1, 1, 0, s->st>>>(s->ds, s->cfg.body, t, dt, t_mode, dt_mode);
 }
 
+// measure! over the whole padded grid the first time; afterwards only over the box the body can reach: mu0 = 1 and
+// mu1 = 0 further than eps from the surface never change (the boundary-face zeros of mu0 neither), and the supported
+// motion is a sinusoidal translation of known amplitude, so the box is known on the host although t is device-resident.
 void wl_k_measure(wl_sim* s)
 {
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_padded(s, g);
+    const wl_body& b = s->cfg.body;
+    if (s->measured && b.kind != WL_BODY_NONE) {
+        int o[3] = { 0, 0, 0 }, e[3] = { g.S[0], g.S[1], g.S[2] };
+        for (int d = 0; d < s->nd; ++d) {
+            float ext = b.R;                                          // sphere / circle
+            if (b.kind == WL_BODY_TORUS) ext = d == b.axis ? b.r : b.R + b.r;
+            float reach = ext + s->cfg.eps + 2.0f;                    // the face positions are half a cell off the centres
+            if (b.motion == WL_MOTION_HEAVE_SIN && d == b.heave_dir) reach += fabsf(b.amp);
+            int lo = (int)floorf(b.centre[d] - reach), hi = (int)ceilf(b.centre[d] + reach) + 1;      // padded coordinates c = x + 1/2
+            if (lo < 0) lo = 0;
+            if (hi > g.n[d] + 1) hi = g.n[d] + 1;
+            if (g.per[d] && (lo <= 2 || hi >= g.n[d] - 1)) { lo = 0; hi = g.n[d] + 1; }   // ghosts mirror the far side: whole direction
+            if (hi < lo) { lo = 0; hi = g.n[d] + 1; }
+            o[d] = lo; e[d] = hi - lo + 1;
+        }
+        T = wl_tiling(s->nd, o, e);
+    }
+    s->measured = 1;
     cudaMemsetAsync(&s->ds->band_count, 0, sizeof(int), s->st);
     {
         ProfScope ps(s, WLK_MEASURE);

@@ -64,6 +64,7 @@ struct wl_sim {
     int pk_level;            // levels >= pk_level run inside k_coarse (nlev: none)
     int pk_blocks;           // co-resident grid of k_coarse (0: not yet queried)
     int tiny_on;             // tiny levels run in the one-cluster kernel k_tiny (env WL_TINY=0 switches it off)
+    int measured;            // measure! has run over the whole grid once: later calls only visit the box the body can reach
     int cd_kernel;           // conv_diff kernel: 3 (default) k_cd_tile3 (TMA) where it applies, 2 k_cd_tile2, 1 k_cd_tile (env WL_CD)
     int bulk_A;              // k_pcg_A_fast takes its operand planes as TMA boxes where it can (env WL_BULK=0 switches it off)
     int fast_A;              // uniform tiles of PCG pass A go through k_pcg_A_fast (env WL_FAST_A=0 switches it off)
