@@ -88,6 +88,9 @@ static Grid make_grid(int nd, const int* n, const int* per)
     return g;
 }
 
+#ifndef WL_PK_MIN_TILES
+#define WL_PK_MIN_TILES 256     // the persistent-kernel levels take fewer planes per tile until they have this many tiles
+#endif
 // levels with at most this many cells run inside the persistent coarse-level kernels (k_coarse / k_tiny)
 static long long pk_max_cells()
 {
@@ -111,7 +114,7 @@ static VT make_vt(int nd, const Grid& g, int level)
     if (const char* e = getenv("WL_ZC")) { int v = atoi(e); if (v >= 1 && v <= 64) zc0 = v; }     // planes per tile (tuning)
     t.zc = nd == 3 ? (g.n[2] < zc0 ? g.n[2] : zc0) : 1;
     if (level > 0 && (long long)g.n[0] * g.n[1] * g.n[2] <= pk_max_cells())
-        while (t.zc > 1 && (int64_t)t.ntx * t.nty * ((g.n[2] + t.zc - 1) / t.zc) < 592) t.zc = (t.zc + 1) / 2;
+        while (t.zc > 1 && (int64_t)t.ntx * t.nty * ((g.n[2] + t.zc - 1) / t.zc) < WL_PK_MIN_TILES) t.zc = (t.zc + 1) / 2;
     t.ntz = nd == 3 ? (g.n[2] + t.zc - 1) / t.zc : 1;
     t.ntiles = t.ntx * t.nty * t.ntz;
     return t;
