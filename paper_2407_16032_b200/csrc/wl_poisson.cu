@@ -7,12 +7,15 @@
 // values never contribute.  Dot products stay on the device (PcgScal).
 //
 // Kernel shapes (wl_vec.cuh): float4 per thread along x, 256-thread blocks, z-marching with the
-// z-neighbours in registers.  One PCG iteration is TWO passes over the level (DESIGN.md 6.1):
+// z-neighbours in registers.  One PCG iteration is TWO passes over the level (DESIGN.md 6.2):
 //   A: e' = beta e + iD r   (recomputed at the six neighbours instead of stored and re-read);
-//      q = A e' ; gamma = q.e'                      [first iteration: e' = iD r, rho = r.e']
+//      q = A e' ; gamma = q.e'       [first iteration: e' = iD (r - m), rho = (r - m).e'; R-T2]
 //   B: x += alpha e' ; r -= alpha q ; rho' = r.(iD r)
-// z = iD r is never stored.  Tiles flagged "plain" (all face coefficients equal the level
-// constant) skip the L and iD loads altogether.
+// z = iD r is never stored.  Every tile carries a mode (wl_vec.cuh): TM_GEN loads L and iD, the
+// uniform modes TM_PLB / TM_PLI take them from the cell position / as constants.  On 3-D levels
+// pass A runs in wl_pcgfast.cu (shared memory, TMA); k_pcg_A here serves 2-D and ragged levels and
+// the persistent kernels.  Levels of at most 1 M cells run as chains of passes inside k_coarse
+// (cooperative launch, grid barrier between passes) and k_tiny (one thread-block cluster).
 #include <cstdio>
 #include <cstdlib>
 #include "wl_internal.h"

@@ -8,9 +8,8 @@
 // reads 512 contiguous bytes per row.  y-neighbours come from L1 (the rows of the adjacent
 // threads of the same block), x-neighbours from two scalar loads.
 //
-// Tiles also carry the "plain" flag: a tile is plain when every face
-// coefficient of every cell in it equals the level constant Lc (no body, no domain boundary
-// nearby).  Plain tiles never load L or iD.
+// Tiles also carry a mode (TM_GEN / TM_PLB / TM_PLI below): uniform tiles
+// (no body within one cell) never load L or iD.
 #pragma once
 #include "wl_common.cuh"
 
