@@ -187,11 +187,15 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
         float* e2 = (float*)cv.take(scl);
         float* q = (float*)cv.take(scl);
         VT vt = make_vt(nd, g, l);
+        // the one-sweep PCG form (wl_pcgfused.cu) ping-pongs r and q: two more arrays on the levels that take it
+        const bool fused = wl_pcg_fused_shape(nd, g, vt) && (l == 0 || (long long)g.n[0] * g.n[1] * g.n[2] > pk_max_cells());
+        float* r2 = fused ? (float*)cv.take(scl) : nullptr;
+        float* q2 = fused ? (float*)cv.take(scl) : nullptr;
         int* plain = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
         int* uniform = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
         if (s) {
             Level& lv = s->lev[l];
-            lv.g = g; lv.L = L; lv.iD = iD; lv.x = x; lv.r = r; lv.e = e; lv.e2 = e2; lv.q = q;
+            lv.g = g; lv.L = L; lv.iD = iD; lv.x = x; lv.r = r; lv.e = e; lv.e2 = e2; lv.q = q; lv.r2 = r2; lv.q2 = q2;
             lv.vt = vt; lv.plain = plain; lv.uniform = uniform;
             lv.Lc = nd == 3 ? (float)(1 << l) : 1.0f;
             lv.iDc = 1.0f / (-(2.0f * nd) * lv.Lc);
@@ -310,6 +314,8 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
         }
     }
     s->fast_A = 1;
+    s->fused = 1;
+    if (const char* e = getenv("WL_FUSED")) s->fused = atoi(e) != 0;
     s->tiny_on = 1;
     s->bulk_A = 1;
     s->cd_kernel = 3;
@@ -506,7 +512,7 @@ extern "C" int wl_level_dims(const wl_sim* s, int level, int dims_out[3])
 // ---- per-kernel-class timing (CUDA events on the handle's stream)
 static const char* const kern_names[WLK_COUNT] = {
     "set_time", "measure", "poisson_update", "conv_diff_bdim", "bc", "exit_bc", "residual", "restrict", "prolong",
-    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc", "conv_diff_band", "vcycle"
+    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc", "conv_diff_band", "vcycle", "pcg_fused"
 };
 
 extern "C" int wl_prof_enable(wl_sim* s, int enable)

@@ -49,7 +49,7 @@ struct PcgScal {
     double rsum;    // sum of r over the coupled cells (iD != 0), left by the kernel that last wrote r (R-T2)
     double nlive;   // number of coupled cells of the level (k_diag_flags)
     int live;   // 0 once a guard of DESIGN.md R-T has fired: later kernels of this smoother call are no-ops
-    int pad;
+    int stop_k; // one-sweep form (wl_pcgfused.cu): the iteration whose stopping criterion fired with its update still owed (0: none)
 };
 
 struct DevScal {

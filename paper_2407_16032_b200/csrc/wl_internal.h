@@ -11,7 +11,7 @@
 enum WlKern {
     WLK_SET_TIME, WLK_MEASURE, WLK_POISSON_UPDATE, WLK_CONVDIFF, WLK_BC, WLK_EXIT_BC, WLK_RESIDUAL,
     WLK_RESTRICT, WLK_PROLONG, WLK_PCG_INIT, WLK_PCG_MATVEC, WLK_PCG_UPDATE, WLK_PCG_DIR,
-    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_CONVDIFF_BAND, WLK_COARSE, WLK_COUNT
+    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_CONVDIFF_BAND, WLK_COARSE, WLK_PCG_FUSED, WLK_COUNT
 };
 struct ProfRec { cudaEvent_t a, b; int cls; };
 
@@ -24,6 +24,8 @@ struct Level {
     float* e;    // CG direction (ping)
     float* e2;   // CG direction (pong): pass A reads one and writes the other
     float* q;    // A e
+    float* r2;   // second residual and A e buffers of the one-sweep PCG form (wl_pcgfused.cu); null on levels that do not take it
+    float* q2;
     VT vt;       // vector tiling of this level
     int* uniform; // per-tile flag: every face coefficient of every cell of the tile equals Lc
     int* plain;  // per-tile flag: the tile and its face-neighbour tiles are uniform (kernels skip L and iD loads)
@@ -67,6 +69,7 @@ struct wl_sim {
     int measured;            // measure! has run over the whole grid once: later calls only visit the box the body can reach
     int cd_kernel;           // conv_diff kernel: 3 (default) k_cd_tile3 (TMA) where it applies, 2 k_cd_tile2, 1 k_cd_tile (env WL_CD)
     int bulk_A;              // k_pcg_A_fast takes its operand planes as TMA boxes where it can (env WL_BULK=0 switches it off)
+    int fused;               // PCG smoother in its one-sweep form where the level allows (env WL_FUSED=0 switches it off)
     int fast_A;              // uniform tiles of PCG pass A go through k_pcg_A_fast (env WL_FAST_A=0 switches it off)
     BodyP body;
     cudaStream_t st;
@@ -137,6 +140,9 @@ void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out,
 // wl_pcgfast.cu
 int wl_pcg_fast_ok(const wl_sim* s, int l);
 void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout);
+// wl_pcgfused.cu
+int wl_pcg_fused_shape(int nd, const Grid& g, const VT& vt);    // the one-sweep form can take a level of this shape
+int wl_k_smooth_fused(wl_sim* s, int l, int iters);              // 0: not taken (the caller runs the two-pass form)
 // wl_poisson.cu
 void wl_k_poisson_update(wl_sim* s);                 // iD on level 0, coarse L and iD
 void wl_k_residual(wl_sim* s, const float* u, float w);   // pscale = w*dt; x = pscale*p; r = div u - A x

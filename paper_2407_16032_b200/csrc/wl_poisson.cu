@@ -1091,6 +1091,7 @@ void wl_k_smooth(wl_sim* s, int l, int iters)
 {
     Level& lv = s->lev[l];
     if (l >= s->pk_level) { CoarseProg P; P.n = 0; prog_add(P, COP_SMOOTH, l, iters); coarse_launch(s, P); return; }
+    if (s->fused && s->fast_A && s->bulk_A && wl_k_smooth_fused(s, l, iters)) return;
     PcgScal* sc = &s->ds->pcg[l];
     float* ea = lv.e;      // direction written by the running A pass
     float* eb = lv.e2;     // previous direction

@@ -15,6 +15,7 @@ pytestmark = pytest.mark.gpu
 
 SWITCHES = [
     {},                                     # default: fast pass A, k_coarse for levels <= 1 M cells, k_tiny below
+    {"WL_FUSED": "0"},                      # two-pass PCG iterations (wl_pcgfast.cu pass A + k_pcg_B) instead of the one-sweep form
     {"WL_FAST_A": "0"},                     # register-marching pass A everywhere
     {"WL_TINY": "0"},                       # tiny levels inside the cooperative kernel
     {"WL_PK_MAX_CELLS": "0"},               # every level by stand-alone kernels
