@@ -52,7 +52,8 @@ ALG_BYTES = {
     "conv_diff_bdim": None,   # mean of predictor and corrector: computed below
     "residual": 4 * (3 + 1 + 2),            # u, p -> x, r
     "pcg_matvec": 4 * (2 + 2),              # pass A: e, r -> e', q (first iteration: r -> e', q)
-    "pcg_update": 4 * (4 + 2),              # pass B: x, r, e', q -> x, r
+    "pcg_update": 4 * (4 + 2),              # pass B / the last sweep of the one-sweep form: x, r, e', q -> x, r
+    "pcg_fused": 4 * (4 + 4),               # one-sweep iteration (wl_pcgfused.cu): x, r, e, q -> x, r', e', q'
     "restrict": 4 * (1 + 2 / 8),            # r -> r_c, x_c
     "prolong": 4 * (2 + 1 / 8 + 2),         # x, r, x_c -> x, r
     "apply_gradient": 4 * (3 + 1 + 3 + 1),  # u, x -> u, p
@@ -62,8 +63,9 @@ ALG_BYTES = {
 
 
 # DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the fine-level kernels on C4, from the
-# ncu --set full capture summarised in profiles/r1c_stages_c4_ncu.md (bytes; other workloads: not captured)
-NCU_TRAFFIC_C4 = {"pcg_update": 793e6, "pcg_matvec": 593e6, "residual": 882e6, "prolong": 577e6,
+# ncu --set full captures summarised in profiles/r1c_stages_c4_ncu.md and (pcg_fused) profiles/r1e_pcg_fused_c4_ncu.md
+# (bytes; other workloads: not captured)
+NCU_TRAFFIC_C4 = {"pcg_fused": 1200e6, "pcg_update": 793e6, "pcg_matvec": 593e6, "residual": 882e6, "prolong": 577e6,
                   "apply_gradient": 1088e6, "cfl": 420e6, "restrict": 160e6, "conv_diff_bdim": 1430e6}
 
 
@@ -327,6 +329,8 @@ def run_gpu(args) -> None:
     tot_prof = sum(v[0] for v in prof.values())
     alg = dict(ALG_BYTES)
     alg["conv_diff_bdim"] = conv_alg_bytes(cfg)
+    if "pcg_fused" in prof:                           # one-sweep form: every fine-level pcg_matvec launch is a first sweep, r -> e', q
+        alg["pcg_matvec"] = 4 * (1 + 2)
     breakdown = {}
     for name, (ms, n) in sorted(prof.items(), key=lambda kv: -kv[1][0]):
         ent = {"ms_per_step": ms / args.steps, "launches_per_step": n / args.steps, "share": ms / tot_prof}
@@ -344,7 +348,8 @@ def run_gpu(args) -> None:
                 "frac": (achieved / hbm_peak) if achieved else None, "frac_of_nominal_8TBs": (achieved / 8000.0) if achieved else None,
                 "peak_source": peak_src,
                 "traffic": NCU_TRAFFIC_C4.get(base) if args.workload == "C4" else None,
-                "traffic_source": "profiles/r1c_stages_c4_ncu.md (ncu --set full, one launch)" if args.workload == "C4" else None,
+                "traffic_source": (("profiles/r1e_pcg_fused_c4_ncu.md" if base == "pcg_fused" else "profiles/r1c_stages_c4_ncu.md")
+                                   + " (ncu --set full, one launch)") if args.workload == "C4" else None,
                 "alg_bytes_per_cell_per_launch": alg.get(base), "avg_launch_us": dom_ms / dom_n * 1e3,
                 "share_of_step": dom_ms / tot_prof,
                 "step": {"alg_bytes_per_cell_per_step": step_bytes / cells,

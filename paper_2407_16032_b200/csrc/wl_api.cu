@@ -187,10 +187,12 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
         float* e2 = (float*)cv.take(scl);
         float* q = (float*)cv.take(scl);
         VT vt = make_vt(nd, g, l);
-        // the one-sweep PCG form (wl_pcgfused.cu) ping-pongs r and q: two more arrays on the levels that take it
+        // the one-sweep PCG form (wl_pcgfused.cu) ping-pongs r and q: two more arrays on the levels that take it.  Level 0
+        // borrows them from the velocity buffer that is dead during the projection (solver_scratch()).
         const bool fused = wl_pcg_fused_shape(nd, g, vt) && (l == 0 || (long long)g.n[0] * g.n[1] * g.n[2] > pk_max_cells());
-        float* r2 = fused ? (float*)cv.take(scl) : nullptr;
-        float* q2 = fused ? (float*)cv.take(scl) : nullptr;
+        float* r2 = fused && l > 0 ? (float*)cv.take(scl) : nullptr;
+        float* q2 = fused && l > 0 ? (float*)cv.take(scl) : nullptr;
+        if (s && l == 0) s->fused0 = fused ? 1 : 0;
         int* plain = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
         int* uniform = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
         if (s) {
@@ -241,9 +243,22 @@ static int solve(wl_sim* s)
     return WL_OK;
 }
 
+// Two level-0 scalar arrays the solver may scribble on: the first two components of a velocity buffer whose content is dead
+// while `u` is being projected.  In mom_step the predictor's projection runs before ut is written, and the corrector's
+// (u == ut) after the last use of u0; their ghost cells hold boundary values, which the stencil multiplies by the zero
+// coefficient of a boundary face.
+static void solver_scratch(wl_sim* s, const float* u)
+{
+    if (!s->fused0) return;
+    float* b = (u == s->ut) ? s->u0 : s->ut;
+    s->lev[0].r2 = b;
+    s->lev[0].q2 = b + s->lev[0].g.nalloc;
+}
+
 // project!: z = div u; x = (w dt) p; solve A x = z; u -= L grad x; p = x/(w dt)
 static int project(wl_sim* s, float* u, float w)
 {
+    solver_scratch(s, u);
     wl_k_residual(s, u, w);
     int rc = solve(s);
     wl_k_apply_gradient(s, u);
@@ -305,6 +320,7 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     s->st = (cudaStream_t)cuda_stream;
     layout(s, cfg, dev_ws);
     s->u = s->ubuf[0]; s->u0 = s->ubuf[1]; s->ut = s->ubuf[2];
+    solver_scratch(s, s->u);
     {   // levels that run inside the persistent coarse-level kernel: from the first level >= 1 small enough
         const long long maxc = pk_max_cells();
         s->pk_level = s->nlev;

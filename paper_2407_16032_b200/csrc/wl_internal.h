@@ -69,6 +69,7 @@ struct wl_sim {
     int measured;            // measure! has run over the whole grid once: later calls only visit the box the body can reach
     int cd_kernel;           // conv_diff kernel: 3 (default) k_cd_tile3 (TMA) where it applies, 2 k_cd_tile2, 1 k_cd_tile (env WL_CD)
     int bulk_A;              // k_pcg_A_fast takes its operand planes as TMA boxes where it can (env WL_BULK=0 switches it off)
+    int fused0;              // level 0 takes the one-sweep PCG form; its r2, q2 live in a dead velocity buffer (wl_api.cu solver_scratch)
     int fused;               // PCG smoother in its one-sweep form where the level allows (env WL_FUSED=0 switches it off)
     int fast_A;              // uniform tiles of PCG pass A go through k_pcg_A_fast (env WL_FAST_A=0 switches it off)
     BodyP body;

@@ -57,11 +57,12 @@ def test_alg_bytes_table_matches_design():
     sys.path.insert(0, str(ROOT))
     import bench
     import wl_inputs as wi
-    assert bench.ALG_BYTES["pcg_matvec"] == 16 and bench.ALG_BYTES["pcg_update"] == 24
+    assert bench.ALG_BYTES["pcg_matvec"] == 16 and bench.ALG_BYTES["pcg_update"] == 24 and bench.ALG_BYTES["pcg_fused"] == 32
     assert bench.ALG_BYTES["residual"] == 24 and bench.ALG_BYTES["apply_gradient"] == 32
     assert bench.conv_alg_bytes(wi.baseline_config(3)) == (36 + 48) / 2
     text = (ROOT / "DESIGN.md").read_text()
-    for tok in ("| `pcg_matvec` (pass A) | e, r → e′, q | 16 |", "| `pcg_update` (pass B) | x, r, e′, q → x, r | 24 |", "| `apply_gradient` |"):
+    for tok in ("| `pcg_matvec` (pass A) | e, r → e′, q | 16 |", "| `pcg_update` (pass B) | x, r, e′, q → x, r | 24 |",
+                "| `pcg_fused` (one-sweep iteration, §6.2) | x, r, e, q → x, r′, e′, q′ | 32 |", "| `apply_gradient` |"):
         assert tok in text
 
 

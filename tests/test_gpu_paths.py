@@ -173,3 +173,112 @@ def test_smoother_removes_residual_mean_on_the_gpu():
         assert np.abs(xb - xa).max() <= 1e-4 * max(np.abs(xa).max(), 1e-30)
         assert abs(rb[0][live].mean()) <= 1e-6
     o.close(); g.close()
+
+
+# levels the one-sweep smoother (wl_pcgfused.cu) takes: rows of whole 128-cell tiles, no wrap in x and y; with
+# WL_PK_MAX_CELLS=0 level 1 of the second case (128 x 16 x 12) is a stand-alone level too and takes it as well
+FUSED = [((128, 40, 24), (0, 0, 0), 1, "sphere", False), ((256, 32, 24), (0, 0, 1), 1, "torus", False)]
+
+
+def _fused_levels(case):
+    return (0, 1) if case[0][0] == 256 else (0,)
+
+
+def _smoother_inputs(o, g, l):
+    ld = g.level_dims(l)
+    r0 = wi.random_scalar(ld, seed=700 + l)
+    r0 -= r0.mean()
+    r0 = r0 * np.minimum(1.0, np.abs(diag(O(o, "iD", l)[0])))
+    g.dbg_set("L", O(o, "L", l), l)
+    g.dbg_set("iD", O(o, "iD", l), l)
+    return r0
+
+
+def _run_smoother(o, g, l, r0, iters):
+    o.interior("r", l)[0][...] = r0
+    o.arr("x", l)[...] = 0.0
+    g.dbg_set("r", r0[None].astype(np.float32), l)
+    g.dbg_set("x", np.zeros_like(r0)[None].astype(np.float32), l)
+    o.smooth(l, iters)
+    g.dbg_smooth(l, iters)
+    return g.dbg_get("x", l), g.dbg_get("r", l)
+
+
+@pytest.mark.parametrize("iters", [1, 2, 3, 6])
+@pytest.mark.parametrize("case", FUSED, ids=_ids)
+def test_one_sweep_smoother_matches_the_oracle_and_the_two_pass_form(case, iters):
+    """The recurrence form of the PCG iteration (one sweep per iteration, r and q ping-pong: odd and even numbers of
+    swaps) against the oracle and against the two-pass kernels, on levels 0 and 1."""
+    from paper_2407_16032_b200 import wl
+    cfg = _cfg(case)
+    outs = []
+    for sw in ({"WL_PK_MAX_CELLS": "0"}, {"WL_PK_MAX_CELLS": "0", "WL_FUSED": "0"}):
+        o, g0 = _sims(cfg)
+        g0.close()
+        with _env(sw):
+            g = wl.Sim(cfg)
+        res = []
+        for l in _fused_levels(case):
+            r0 = _smoother_inputs(o, g, l)
+            xg, rg = _run_smoother(o, g, l, r0, iters)
+            tol = TOL if iters == 1 else 1e-4
+            assert relerr(xg, O(o, "x", l)) <= tol, (sw, l)
+            assert np.abs(rg - O(o, "r", l)).max() <= tol * np.abs(r0).max(), (sw, l)
+            res.append((xg.astype(np.float64), rg.astype(np.float64), np.abs(r0).max()))
+        outs.append(res)
+        o.close(); g.close()
+    for (xa, ra, s), (xb, rb, _s) in zip(*outs):
+        assert np.abs(xa - xb).max() <= 1e-4 * np.abs(xb).max()
+        assert np.abs(ra - rb).max() <= 1e-4 * s
+
+
+@pytest.mark.parametrize("case", FUSED, ids=_ids)
+def test_one_sweep_smoother_stops_like_the_oracle(case):
+    """R-T guards in the one-sweep form.  A zero residual changes nothing.  A residual scaled so that |rho| falls below
+    tau = 1e-30 after the first iteration stops the oracle there; the device evaluates the criterion on the recurrence
+    value of rho', applies the update still owed in the next sweep and carries r across the remaining ones: x and r
+    as the oracle's."""
+    from paper_2407_16032_b200 import wl
+    cfg = _cfg(case)
+    o, g0 = _sims(cfg)
+    g0.close()
+    with _env({"WL_PK_MAX_CELLS": "0"}):
+        g = wl.Sim(cfg)
+    for l in _fused_levels(case):
+        r0 = _smoother_inputs(o, g, l)
+        iD = O(o, "iD", l)[0]
+        # zero residual
+        x1 = wi.random_scalar(g.level_dims(l), seed=800 + l).astype(np.float32)
+        g.dbg_set("r", np.zeros_like(r0)[None].astype(np.float32), l)
+        g.dbg_set("x", x1[None], l)
+        g.dbg_smooth(l, 6)
+        assert np.array_equal(g.dbg_get("x", l)[0], x1) and not g.dbg_get("r", l).any()
+        assert g.dbg_pcg_scalars(l)["live"] == 0.0
+        # a checkerboard is (away from boundaries and the body) an eigenvector of iD A: one iteration takes |rho| = |r . iD r|
+        # down by ~1e3.  |rho_k| of the unscaled problem after k iterations, from the oracle's residuals:
+        shp = o.interior("r", l)[0].shape
+        k3, j3, i3 = np.indices(shp)
+        rc = (1.0 - 2.0 * ((i3 + j3 + k3) & 1)) * np.minimum(1.0, np.abs(diag(iD))) + 0.02 * r0
+        rc -= rc.mean()
+        rho = []
+        for k in range(3):
+            o.interior("r", l)[0][...] = rc
+            o.arr("x", l)[...] = 0.0
+            if k:
+                o.smooth(l, k)
+            rk = O(o, "r", l)[0]
+            rho.append(abs(float((rk * iD * rk).sum())))
+        assert rho[1] <= rho[0] / 64.0
+        scale = np.sqrt(1e-30 * 8.0 / rho[0])                 # rho_0 = 8 tau, rho_1 <= tau / 8: the smoother stops after one iteration
+        for iters in (1, 2, 3, 6):                            # the update still owed is applied by the last sweep / a fused sweep
+            xg, rg = _run_smoother(o, g, l, rc * scale, iters)
+            xo, ro = O(o, "x", l).copy(), O(o, "r", l).copy()
+            o.interior("r", l)[0][...] = rc * scale
+            o.arr("x", l)[...] = 0.0
+            o.smooth(l, 1)
+            # the oracle did stop after the first iteration (its OpenMP sums may differ in the last bit from run to run)
+            assert np.allclose(O(o, "x", l), xo, rtol=1e-10, atol=0.0)
+            assert g.dbg_pcg_scalars(l)["live"] == 0.0
+            assert relerr(xg, xo) <= 1e-4, (l, iters)
+            assert np.abs(rg - ro).max() <= 1e-4 * np.abs(rc * scale).max(), (l, iters)
+    o.close(); g.close()
