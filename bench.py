@@ -331,6 +331,8 @@ def run_gpu(args) -> None:
     alg["conv_diff_bdim"] = conv_alg_bytes(cfg)
     if "pcg_fused" in prof:                           # one-sweep form: every fine-level pcg_matvec launch is a first sweep, r -> e', q
         alg["pcg_matvec"] = 4 * (1 + 2)
+        # ... and of the two last sweeps of a solve (fixed two V-cycles) the second leaves r alone (x, e' -> x): mean of 24 and 12
+        alg["pcg_update"] = (4 * (4 + 2) + 4 * (2 + 1)) / 2
     breakdown = {}
     for name, (ms, n) in sorted(prof.items(), key=lambda kv: -kv[1][0]):
         ent = {"ms_per_step": ms / args.steps, "launches_per_step": n / args.steps, "share": ms / tot_prof}

@@ -222,7 +222,7 @@ static int solve(wl_sim* s)
     const wl_mg& mg = s->cfg.mg;
     int nv = 0;
     if (mg.fixed_vcycles > 0) {
-        for (; nv < mg.fixed_vcycles; ++nv) { wl_k_vcycle(s, 0); wl_k_smooth(s, 0, mg.smooth_iters); }
+        for (; nv < mg.fixed_vcycles; ++nv) { wl_k_vcycle(s, 0); wl_k_smooth(s, 0, mg.smooth_iters, nv + 1 < mg.fixed_vcycles); }
         s->res[s->solve_slot] = -1.0;
     } else {
         double res = 0.0;

@@ -143,13 +143,15 @@ int wl_pcg_fast_ok(const wl_sim* s, int l);
 void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout);
 // wl_pcgfused.cu
 int wl_pcg_fused_shape(int nd, const Grid& g, const VT& vt);    // the one-sweep form can take a level of this shape
-int wl_k_smooth_fused(wl_sim* s, int l, int iters);              // 0: not taken (the caller runs the two-pass form)
+int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r);              // 0: not taken (the caller runs the two-pass form)
 // wl_poisson.cu
 void wl_k_poisson_update(wl_sim* s);                 // iD on level 0, coarse L and iD
 void wl_k_residual(wl_sim* s, const float* u, float w);   // pscale = w*dt; x = pscale*p; r = div u - A x
 void wl_k_restrict(wl_sim* s, int l);                // r_{l+1} = sum children r_l ; x_{l+1} = 0
 void wl_k_prolong(wl_sim* s, int l);                 // x_l += P x_{l+1}; r_l -= A_l P x_{l+1}
-void wl_k_smooth(wl_sim* s, int l, int iters);
+// need_r = 0: nobody reads the residual of this level before it is rewritten (a coarse level before its prolongation, the
+// last smoother call of a solve with a fixed number of V-cycles): the one-sweep form then leaves r one update behind
+void wl_k_smooth(wl_sim* s, int l, int iters, int need_r = 1);
 void wl_k_coarse_prog(wl_sim* s, const CoarseProg& P);   // one k_coarse launch
 void wl_k_rsum(wl_sim* s, int l);                    // pcg[l].rsum = sum of r over the coupled cells (stage hooks)
 void wl_k_vcycle(wl_sim* s, int l);

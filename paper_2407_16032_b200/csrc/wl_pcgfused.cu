@@ -263,7 +263,7 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
 }
 
 // The update of one iteration alone, on one tile: x += alpha e; rout = (rin - m) - alpha q  (UPDATE), or rout = rin (the
-// smoother has stopped and r only has to change buffers).  Pointwise: no halos, plain loads.
+// smoother has stopped and r only has to change buffers), or (UPDATE == 2) x += alpha e alone.  Pointwise: no halos, plain loads.
 template <int UPDATE>
 __device__ __forceinline__ void ff_pointwise(const Grid& g, const VT& vt, int tile, int mode, float alpha, float m, const float* __restrict__ iD,
                                              float* __restrict__ x, const float* rin, float* rout,
@@ -277,6 +277,13 @@ __device__ __forceinline__ void ff_pointwise(const Grid& g, const VT& vt, int ti
     const int off = WL_OFF + c0 + c1 * (int)g.sy;
     for (int z = z0; z <= z1; ++z) {
         const int i = off + z * (int)g.sz;
+        if (UPDATE == 2) {
+            float xv[4], ee[4];
+            unpack4(*reinterpret_cast<const float4*>(x + i), xv);
+            unpack4(ld4(e, i), ee);
+            *reinterpret_cast<float4*>(x + i) = make_float4(xv[0] + alpha * ee[0], xv[1] + alpha * ee[1], xv[2] + alpha * ee[2], xv[3] + alpha * ee[3]);
+            continue;
+        }
         float rr[4];
         unpack4(*reinterpret_cast<const float4*>(rin + i), rr);
         if (UPDATE) {
@@ -366,15 +373,16 @@ __global__ void __launch_bounds__(WL_VB, 3) k_pcg_fused(Grid g, VT vt, const int
 // the update of the last iteration (kprev), or what a stopped smoother still owes
 __global__ void __launch_bounds__(WL_VB, 4) k_pcg_last(Grid g, VT vt, const int* __restrict__ plain, int kprev, const float* __restrict__ iD, float* __restrict__ x,
                                                        const float* rin, float* rout, const float* __restrict__ e,
-                                                       const float* __restrict__ q, const PcgScal* sc)
+                                                       const float* __restrict__ q, const PcgScal* sc, int need_r)
 {
     const float m = kprev == 1 && sc->nlive > 0.0 ? (float)(sc->rsum / sc->nlive) : 0.0f;
     const float alpha = (float)sc->alpha;
     const bool update = sc->live || sc->stop_k == kprev;
-    if (!update && rin == rout) return;
+    if (!update && (rin == rout || !need_r)) return;
     for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
-        if (update) ff_pointwise<1>(g, vt, tile, plain[tile], alpha, m, iD, x, rin, rout, e, q);
-        else        ff_pointwise<0>(g, vt, tile, plain[tile], alpha, m, iD, x, rin, rout, e, q);
+        if (update && need_r) ff_pointwise<1>(g, vt, tile, plain[tile], alpha, m, iD, x, rin, rout, e, q);
+        else if (update)      ff_pointwise<2>(g, vt, tile, plain[tile], alpha, m, iD, x, rin, rout, e, q);
+        else                  ff_pointwise<0>(g, vt, tile, plain[tile], alpha, m, iD, x, rin, rout, e, q);
     }
 }
 
@@ -387,7 +395,7 @@ int wl_pcg_fused_shape(int nd, const Grid& g, const VT& vt)
 }
 
 // The smoother on level l as iters + 1 sweeps (see the head of this file).  Returns 0 when the level does not take this form.
-int wl_k_smooth_fused(wl_sim* s, int l, int iters)
+int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
 {
     Level& lv = s->lev[l];
     if (!lv.r2 || !lv.q2 || iters < 1) return 0;
@@ -427,7 +435,7 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters)
         float* rout = lv.r;
         int g2 = lv.vt.ntiles < s->sm_count * 8 ? lv.vt.ntiles : s->sm_count * 8;
         ProfScope ps_(s, WLK_PCG_UPDATE, l > 0);
-        k_pcg_last<<<g2, WL_VB, 0, s->st>>>(lv.g, lv.vt, lv.plain, iters, lv.iD, lv.x, ra, rout, eb, qb, sc);
+        k_pcg_last<<<g2, WL_VB, 0, s->st>>>(lv.g, lv.vt, lv.plain, iters, lv.iD, lv.x, ra, rout, eb, qb, sc, need_r);
     }
     cudaMemsetAsync(&sc->rsum, 0, sizeof(double), s->st);    // the mean of r has been removed (R-T2)
     return 1;

@@ -1087,11 +1087,11 @@ void wl_k_rsum(wl_sim* s, int l)
     VDISPATCH(s, WLK_MISC, l > 0, lv.vt, k_rsum<2>, k_rsum<3>, lv.g, lv.vt, lv.plain, lv.r, lv.iD, &s->ds->pcg[l], s->rb);
 }
 
-void wl_k_smooth(wl_sim* s, int l, int iters)
+void wl_k_smooth(wl_sim* s, int l, int iters, int need_r)
 {
     Level& lv = s->lev[l];
     if (l >= s->pk_level) { CoarseProg P; P.n = 0; prog_add(P, COP_SMOOTH, l, iters); coarse_launch(s, P); return; }
-    if (s->fused && s->fast_A && s->bulk_A && wl_k_smooth_fused(s, l, iters)) return;
+    if (s->fused && s->fast_A && s->bulk_A && wl_k_smooth_fused(s, l, iters, need_r)) return;
     PcgScal* sc = &s->ds->pcg[l];
     float* ea = lv.e;      // direction written by the running A pass
     float* eb = lv.e2;     // previous direction
@@ -1134,7 +1134,7 @@ void wl_k_vcycle(wl_sim* s, int l)
         coarse_launch(s, P);
     } else {
         if (l + 1 < s->nlev - 1) wl_k_vcycle(s, l + 1);
-        wl_k_smooth(s, l + 1, it);
+        wl_k_smooth(s, l + 1, it, 0);       // the prolongation reads x of the coarse level only
     }
     wl_k_prolong(s, l);
 }
