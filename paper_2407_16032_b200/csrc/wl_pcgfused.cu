@@ -63,14 +63,16 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
     // same time (both at their start, or both at their end), and the second reader finds them in L2
     const int dir = (tiz & 1) ? -1 : 1, zs = dir > 0 ? z0 : z1;
     const int gx = tix * LX + tx, c0 = 1 + 4 * gx, c1 = y0 + ty;
-    const bool valid = c1 <= g.n[1];          // tiles fill their rows (host check); the last tile row may stick out in y
+    // the last tile of a row may stick out in x and y: positions past the row read zeros (the pad of the array, or the zero
+    // fill of the TMA box), form finite values nobody uses, and store nothing; n0 % 4 == 0: whole groups only
+    const bool own = gx < vt.ngx, valid = own && c1 <= g.n[1];
     const int sy = (int)g.sy, sz = (int)g.sz;
     const int off_own = WL_OFF + c0 + ff_src(c1, g.n[1], 0) * sy;
     const int idx_own = (ty + 1) * RW + 4 + 4 * tx;
-    bool hrow = false; int off_h = 0, idx_h = 0, hc0 = 0, hc1 = 0;
+    bool hrow = false, hrow_ld = false; int off_h = 0, idx_h = 0, hc0 = 0, hc1 = 0;
     if (tid < 2 * LX) {
         const int hr = tid >> 5, hx = tid & (LX - 1);
-        hrow = true;
+        hrow = true; hrow_ld = tix * LX + hx < vt.ngx;
         hc0 = 1 + 4 * (tix * LX + hx); hc1 = hr ? y0 + LY : y0 - 1;
         off_h = WL_OFF + hc0 + ff_src(hc1, g.n[1], 0) * sy;
         idx_h = (hr ? LY + 1 : 0) * RW + 4 + 4 * hx;
@@ -125,8 +127,8 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
     }
     auto load_iD = [&](int p, bool full) {    // GEN: 1/D of plane p at the positions the operands come from
         const int zo = ff_src(p, g.n[2], g.per[2]) * sz;
-        unpack4(ld4(iD, off_own + zo), d_in);
-        if (full && hrow) unpack4(ld4(iD, off_h + zo), dh_in);
+        if (own) unpack4(ld4(iD, off_own + zo), d_in);
+        if (full && hrow_ld) unpack4(ld4(iD, off_h + zo), dh_in);
         if (full && hcol) dx_in = ld1(iD, off_x + zo);
     };
     // plane p from stage slot `slot`: r' and x stored for the own cells, e' -> registers and shared, iD r' and iD -> registers
@@ -273,7 +275,7 @@ __device__ __forceinline__ void ff_pointwise(const Grid& g, const VT& vt, int ti
     const int tix = tile % vt.ntx, rem = tile / vt.ntx, tiy = rem % vt.nty, tiz = rem / vt.nty;
     const int c0 = 1 + 4 * (tix * 32 + tx), c1 = 1 + 8 * tiy + ty;
     const int z0 = 1 + tiz * vt.zc, z1 = min(z0 + vt.zc - 1, g.n[2]);
-    if (c1 > g.n[1]) return;
+    if (c1 > g.n[1] || c0 > g.n[0]) return;
     const int off = WL_OFF + c0 + c1 * (int)g.sy;
     for (int z = z0; z <= z1; ++z) {
         const int i = off + z * (int)g.sz;
@@ -388,10 +390,10 @@ __global__ void __launch_bounds__(WL_VB, 4) k_pcg_last(Grid g, VT vt, const int*
 
 static size_t ff_smem(int first) { return sizeof(float) * ((size_t)FF_S * (first ? FF_PLR : 3 * FF_PLR + FF_XB) + 2 * FF_PL) + 8 * FF_S + 8; }
 
-// 3-D, no wrap in x or y (a TMA box cannot wrap), 32 float4 groups per tile row and rows made of whole tiles, 32-bit offsets
+// 3-D, no wrap in x or y (a TMA box cannot wrap), whole float4 groups and at least 17 of them per row (32 threads along x), 32-bit offsets
 int wl_pcg_fused_shape(int nd, const Grid& g, const VT& vt)
 {
-    return nd == 3 && !g.per[0] && !g.per[1] && g.n[0] % 4 == 0 && vt.lxl == 5 && vt.ngx % 32 == 0 && g.nalloc < ((int64_t)1 << 31);
+    return nd == 3 && !g.per[0] && !g.per[1] && g.n[0] % 4 == 0 && vt.lxl == 5 && g.nalloc < ((int64_t)1 << 31);
 }
 
 // The smoother on level l as iters + 1 sweeps (see the head of this file).  Returns 0 when the level does not take this form.

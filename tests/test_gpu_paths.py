@@ -175,9 +175,10 @@ def test_smoother_removes_residual_mean_on_the_gpu():
     o.close(); g.close()
 
 
-# levels the one-sweep smoother (wl_pcgfused.cu) takes: rows of whole 128-cell tiles, no wrap in x and y; with
+# levels the one-sweep smoother (wl_pcgfused.cu) takes: 3-D, at least 68 cells along x, no wrap in x and y; with
 # WL_PK_MAX_CELLS=0 level 1 of the second case (128 x 16 x 12) is a stand-alone level too and takes it as well
-FUSED = [((128, 40, 24), (0, 0, 0), 1, "sphere", False), ((256, 32, 24), (0, 0, 1), 1, "torus", False)]
+FUSED = [((128, 40, 24), (0, 0, 0), 1, "sphere", False), ((256, 32, 24), (0, 0, 1), 1, "torus", False),
+         ((160, 44, 24), (0, 0, 0), 1, "sphere", False)]          # the last: rows of 1.25 tiles, 5.5 tiles along y
 
 
 def _fused_levels(case):
