@@ -57,7 +57,7 @@ struct wl_sim {
     float* mu1;              // nd*nd comps
     long long* band_list;    // faces with mu1 != 0, written by measure!: (array offset << 2) | component
     int band_cap;            // capacity of band_list (entries)
-    int cd_attr_set;         // dynamic shared-memory attribute of the conv_diff kernels is set
+    int cd_attr_set;         // dynamic shared-memory attributes set: bits 1, 2, 4 conv_diff kernels, 8 cluster size of k_tiny, 16 k_pcg_fused
     DevScal* ds;             // device-resident scalars
     DevScal* hs;             // pinned host mirror for read-back
     RedBuf rb;

@@ -404,11 +404,10 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
     PcgScal* sc = &s->ds->pcg[l];
     int grid = lv.vt.ntiles < s->sm_count * 3 ? lv.vt.ntiles : s->sm_count * 3;
     if (grid > WL_MAX_PARTIALS) grid = WL_MAX_PARTIALS;
-    static bool attr = false;
-    if (!attr) {
+    if (!(s->cd_attr_set & 16)) {         // per handle: a process may hold handles on several devices
         cudaFuncSetAttribute(k_pcg_fused<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ff_smem(1));
         cudaFuncSetAttribute(k_pcg_fused<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ff_smem(0));
-        attr = true;
+        s->cd_attr_set |= 16;
     }
     float *ra = lv.r, *rb = lv.r2;            // ra: the residual as it stands
     float *ea = lv.e2, *eb = lv.e;            // ea: the direction of the previous iteration, eb: the one being written
