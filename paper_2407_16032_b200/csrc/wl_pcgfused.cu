@@ -5,14 +5,15 @@
 //     rho' = rho - 2 alpha (q . iD r) + alpha^2 (q . iD q),
 // so a sweep that also accumulates q.iD r and q.iD q knows alpha AND beta when it ends, and the update of iteration k
 // can ride on the sweep of iteration k+1:
-//     first sweep  (k_pcg_A_fast<1>, extended):  e' = iD (r - m); q = A e'; gamma, rho, q.iD(r-m), q.iD q
-//     fused sweep  (k_pcg_fused, iterations 2..n): r' = (r - m) - alpha q [r and q with halos]; x += alpha e;
+//     first sweep  (k_pcg_fused<1>):             e' = iD (r - m); q = A e'; gamma, rho, q.iD(r-m), q.iD q
+//     fused sweep  (k_pcg_fused<0>, iterations 2..n): r' = (r - m) - alpha q [r and q with halos]; x += alpha e;
 //                                                  e' = beta e + iD r'; q' = A e'; gamma, q'.iD r', q'.iD q'
-//     last sweep   (k_pcg_last, pointwise):       x += alpha e; r' = r - alpha q
+//     last sweep   (k_pcg_last, pointwise):       x += alpha e; r' = r - alpha q  (x alone where nobody reads r' any more)
 // 12 + 32 (n-1) + 24 bytes per cell instead of 12 + 16 (n-1) + 24 n, n + 1 launches instead of 2 n.  r and q ping-pong
-// between two buffers (a block reads the OLD r and q of its neighbours' cells); n - 1 fused sweeps and the last one make
-// an even number of swaps for n = 6, and a sweep that finds the smoother stopped still copies r across, so after the call
-// r is where it was.  Levels this form does not take (periodic x or y, ragged rows, 2-D) keep the two-pass form.
+// between two buffers (a block reads the OLD r and q of its neighbours' cells); the last sweep writes r back to where it
+// was, and a sweep that finds the smoother stopped applies the update still owed or copies r across, so after the call r
+// is where it was.  The planes of r, e, q (with halos) and x (own cells) arrive as TMA boxes, three planes ahead of use.
+// Levels this form does not take (periodic x or y, fewer than 68 cells along x, 2-D) keep the two-pass form.
 #include <cstdio>
 #include <cstring>
 #include "wl_internal.h"
