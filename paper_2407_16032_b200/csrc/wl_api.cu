@@ -195,10 +195,11 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
         if (s && l == 0) s->fused0 = fused ? 1 : 0;
         int* plain = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
         int* uniform = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
+        int* tile_live = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
         if (s) {
             Level& lv = s->lev[l];
             lv.g = g; lv.L = L; lv.iD = iD; lv.x = x; lv.r = r; lv.e = e; lv.e2 = e2; lv.q = q; lv.r2 = r2; lv.q2 = q2;
-            lv.vt = vt; lv.plain = plain; lv.uniform = uniform;
+            lv.vt = vt; lv.plain = plain; lv.uniform = uniform; lv.tile_live = tile_live;
             lv.Lc = nd == 3 ? (float)(1 << l) : 1.0f;
             lv.iDc = 1.0f / (-(2.0f * nd) * lv.Lc);
         }
@@ -703,5 +704,6 @@ extern "C" int wl_dbg_set(wl_sim* s, const char* name, int level, const float* i
     if (rc != WL_OK) return rc;
     if (in_floats < (size_t)(interior_count(*g) * nc) || arr == s->lev[0].q) return WL_EINVAL;
     rc = copy_in(s, *g, arr, nc, in, 0);
+    s->measured = 0;        // the next measure! takes nothing for unchanged
     return rc != WL_OK ? rc : nc;
 }

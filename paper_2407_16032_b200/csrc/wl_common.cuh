@@ -70,6 +70,8 @@ struct DevScal {
 };
 
 // reduction scratch: partial sums of up to 4 values per block + the arrival counter
+struct CellBox { int lo[3], hi[3]; };     // inclusive range of cell coordinates (both 0 in an unused direction)
+
 struct RedBuf {
     double* partial;     // [4][WL_MAX_PARTIALS]
     unsigned int* counter;

@@ -340,6 +340,7 @@ void wl_k_measure(wl_sim* s)
         }
         T = wl_tiling(s->nd, o, e);
     }
+    for (int d = 0; d < 3; ++d) { s->mbox_lo[d] = T.o[d]; s->mbox_hi[d] = T.o[d] + T.e[d] - 1; }
     s->measured = 1;
     cudaMemsetAsync(&s->ds->band_count, 0, sizeof(int), s->st);
     {

@@ -27,6 +27,7 @@ struct Level {
     float* r2;   // second residual and A e buffers of the one-sweep PCG form (wl_pcgfused.cu); null on levels that do not take it
     float* q2;
     VT vt;       // vector tiling of this level
+    int* tile_live; // per tile: number of coupled cells (iD != 0) in it, kept so that k_diag_flags can skip tiles the body cannot reach
     int* uniform; // per-tile flag: every face coefficient of every cell of the tile equals Lc
     int* plain;  // per-tile flag: the tile and its face-neighbour tiles are uniform (kernels skip L and iD loads)
     float Lc;    // face coefficient of a body-free, boundary-free cell on this level (R-S: 1, or 2^l in 3-D)
@@ -69,6 +70,7 @@ struct wl_sim {
     int measured;            // measure! has run over the whole grid once: later calls only visit the box the body can reach
     int cd_kernel;           // conv_diff kernel: 3 (default) k_cd_tile3 (TMA) where it applies, 2 k_cd_tile2, 1 k_cd_tile (env WL_CD)
     int bulk_A;              // k_pcg_A_fast takes its operand planes as TMA boxes where it can (env WL_BULK=0 switches it off)
+    int mbox_lo[3], mbox_hi[3]; // padded coordinates of the box the last measure! rewrote (the whole array the first time)
     int fused0;              // level 0 takes the one-sweep PCG form; its r2, q2 live in a dead velocity buffer (wl_api.cu solver_scratch)
     int fused;               // PCG smoother in its one-sweep form where the level allows (env WL_FUSED=0 switches it off)
     int fast_A;              // uniform tiles of PCG pass A go through k_pcg_A_fast (env WL_FAST_A=0 switches it off)

@@ -248,12 +248,25 @@ __device__ __forceinline__ void march(const Grid& g, const VPos& p, const Src& S
 // when every face coefficient of every cell in it has its body-free value.
 template <int ND>
 __global__ void __launch_bounds__(WL_VB) k_diag_flags(Grid g, VT vt, const float* __restrict__ L, float Lc, float* __restrict__ iD, int* __restrict__ uniform,
-                                                      PcgScal* sc, RedBuf rb)
+                                                      int* __restrict__ tile_live, CellBox B, PcgScal* sc, RedBuf rb)
 {
+    __shared__ int live_s;
     double v[1] = { 0.0 };
     for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
         VPos p = vt_pos(g, vt, tile);
-        int ok = 1;
+        {   // a tile no cell of which lies in the box where L may have changed keeps its 1/D, its flag and its count
+            const int lx4 = 4 << vt.lxl, ly = WL_VB >> vt.lxl;
+            const int tix = tile % vt.ntx, tiy = (tile / vt.ntx) % vt.nty;
+            const bool in = 1 + lx4 * tix <= B.hi[0] && lx4 * (tix + 1) >= B.lo[0] && 1 + ly * tiy <= B.hi[1] && ly * (tiy + 1) >= B.lo[1]
+                            && p.z0 <= B.hi[2] && p.z1 >= B.lo[2];
+            if (!in) {
+                if (threadIdx.x == 0) v[0] += (double)tile_live[tile];
+                continue;
+            }
+        }
+        if (threadIdx.x == 0) live_s = 0;
+        __syncthreads();
+        int ok = 1, cnt = 0;
         if (p.nv > 0) {
             const int64_t rc = (int64_t)WL_OFF + (int64_t)p.c1 * g.sy;
             Coef C, R;
@@ -269,7 +282,7 @@ __global__ void __launch_bounds__(WL_VB) k_diag_flags(Grid g, VT vt, const float
                     D -= C.y[k] + C.yp[k];
                     if (ND == 3) D -= C.z[k] + C.zp[k];
                     d[k] = fabsf(D) > 2.0f * ND * 1e-6f ? 1.0f / D : 0.0f;
-                    if (k < p.nv && d[k] != 0.0f) v[0] += 1.0;
+                    if (k < p.nv && d[k] != 0.0f) ++cnt;
                     if (k < p.nv) {
                         bool same = C.x[k] == R.x[k] && C.x[k + 1] == R.x[k + 1] && C.y[k] == R.y[k] && C.yp[k] == R.yp[k];
                         if (ND == 3) same = same && C.z[k] == R.z[k] && C.zp[k] == R.zp[k];
@@ -279,8 +292,11 @@ __global__ void __launch_bounds__(WL_VB) k_diag_flags(Grid g, VT vt, const float
                 st4(iD, i, d, p.nv);
             }
         }
+        v[0] += (double)cnt;
+        if (cnt) atomicAdd(&live_s, cnt);
         ok = __syncthreads_and(ok);
-        if (threadIdx.x == 0) uniform[tile] = ok;
+        if (threadIdx.x == 0) { uniform[tile] = ok; tile_live[tile] = live_s; }
+        __syncthreads();
     }
     if (grid_reduce<1, OpSum>(v, rb)) {
         if (threadIdx.x == 0) sc->nlive = v[0];
@@ -971,18 +987,32 @@ __global__ void __launch_bounds__(WL_VB, WL_PK_MINB) k_tiny(const LevDev* levs, 
         else              kern2<<<wl_vgrid(s, vt), WL_VB, 0, (s)->st>>>(__VA_ARGS__);        \
     } while (0)
 
+// After a measure! that rewrote only the box the body can reach (wl_k_measure), L, 1/D and the tile flags change only in
+// that box grown by one cell, halved and grown by one cell again from level to level.
 void wl_k_poisson_update(wl_sim* s)
 {
+    CellBox B;
+    for (int d = 0; d < 3; ++d) {
+        const int n = s->lev[0].g.n[d];
+        B.lo[d] = s->mbox_lo[d] - 1 < 1 ? 1 : s->mbox_lo[d] - 1;
+        B.hi[d] = s->mbox_hi[d] + 1 > n ? n : s->mbox_hi[d] + 1;
+        if (d >= s->nd) { B.lo[d] = 0; B.hi[d] = 0; }
+    }
     for (int l = 0; l < s->nlev; ++l) {
         Level& lv = s->lev[l];
         if (l > 0) {
             Level& lf = s->lev[l - 1];
-            int o[3] = { 1, 1, s->nd == 3 ? 1 : 0 };
-            int e[3] = { lv.g.n[0] + 1, lv.g.n[1] + 1, s->nd == 3 ? lv.g.n[2] + 1 : 1 };
+            for (int d = 0; d < s->nd; ++d) {
+                const int lo = (B.lo[d] + 1) / 2 - 1, hi = (B.hi[d] + 1) / 2 + 1;
+                B.lo[d] = lo < 1 ? 1 : lo;
+                B.hi[d] = hi > lv.g.n[d] ? lv.g.n[d] : hi;
+            }
+            int o[3] = { B.lo[0], B.lo[1], s->nd == 3 ? B.lo[2] : 0 };
+            int e[3] = { B.hi[0] - B.lo[0] + 2, B.hi[1] - B.lo[1] + 2, s->nd == 3 ? B.hi[2] - B.lo[2] + 2 : 1 };      // faces lo .. hi + 1
             Tiling T = wl_tiling(s->nd, o, e);
             DISPATCH(s, WLK_POISSON_UPDATE, l > 1, k_restrict_L, T, lf.g, lv.g, T, lf.L, lv.L);
         }
-        VDISPATCH(s, WLK_POISSON_UPDATE, l > 0, lv.vt, k_diag_flags<2>, k_diag_flags<3>, lv.g, lv.vt, lv.L, lv.Lc, lv.iD, lv.uniform, &s->ds->pcg[l], s->rb);
+        VDISPATCH(s, WLK_POISSON_UPDATE, l > 0, lv.vt, k_diag_flags<2>, k_diag_flags<3>, lv.g, lv.vt, lv.L, lv.Lc, lv.iD, lv.uniform, lv.tile_live, B, &s->ds->pcg[l], s->rb);
         {
             ProfScope ps_(s, WLK_POISSON_UPDATE, l > 0);
             int nb = (lv.vt.ntiles + 255) / 256;
