@@ -25,7 +25,9 @@
  * convergence order, Laplacian special case vs a textbook kron Laplacian, operator
  * symmetry / null space, multigrid vs dense direct solve on 16x16, divergence after
  * projection, free-stream preservation, 2-D Taylor-Green closed-form decay, CFL closed
- * forms, force vs divergence theorem.  No function here is "parity unpinned" except
+ * forms, force vs divergence theorem; the two constants the readings add (the decoupling
+ * threshold of level_diag, the relative stop of wlo_smooth) by hand-set coefficients and by a
+ * two-eigenmode residual with closed-form iterates.  No function here is "parity unpinned" except
  * whole-run physical values (C_D etc.), which need the paper's run lengths and data.
  */
 #include <math.h>

@@ -323,3 +323,101 @@ def test_projection_identities(which):
     if not cfg["periodic"][0]:                                   # L = 0 on the inflow face
         assert np.all(s.arr("u")[0][..., 1] == cfg["U"][0])
     s.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# Pins for the two constants of DESIGN.md R-O and R-T that the paper does not state (P:76, P:149 name the
+# solver only): the decoupling threshold |D| > 2n * 1e-6 of level_diag and the relative stop
+# |rho'| < 1e-8 |rho0| of wlo_smooth.  Each test fails if the constant is changed by 100x either way.
+
+@pytest.mark.parametrize("nd", [2, 3])
+def test_level_diag_threshold_is_2n_times_1e_minus_6(nd):
+    """R-O: iD = 1/D where |D| > 2n * 1e-6, else 0.  Hand-set face coefficients give cells with
+    |D| = 0 (-> 0), 0.5x the threshold (-> 0), 2x the threshold (-> 1/D), 5e-6 (between the 2-D threshold
+    4e-6 and the 3-D one 6e-6: coupled in 2-D, decoupled in 3-D, which pins the factor 2n), and an
+    ordinary fluid cell (-> -1/2n)."""
+    dims = (12, 8) if nd == 2 else (12, 8, 8)
+    s = wo.OracleSim(wi.make(ndim=nd, dims=dims, periodic=(0,) * 3, U=(0.0,) * 3))
+    L = s.arr("L", 0)
+    thr = 2 * nd * 1e-6
+
+    def set_cell(c0, total):
+        """all 2n faces of cell (c0, 4[, 4]) get total / 2n, so that D = -total"""
+        c = (4, 4, c0) if nd == 3 else (0, 4, c0)           # (c2, c1, c0)
+        for i in range(nd):
+            up = list(c)
+            up[2 - i] += 1
+            L[i][c] = total / (2 * nd)
+            L[i][tuple(up)] = total / (2 * nd)
+        return c
+
+    cells = {                                                # well separated: no shared faces
+        "zero": set_cell(2, 0.0), "below": set_cell(4, 0.5 * thr), "above": set_cell(6, 2.0 * thr),
+        "five": set_cell(8, 5e-6),
+    }
+    s.poisson_update()
+    iD = s.arr("iD", 0)[0]
+    assert iD[cells["zero"]] == 0.0
+    assert iD[cells["below"]] == 0.0                          # a threshold 100x smaller would couple it
+    assert iD[cells["above"]] == pytest.approx(-1.0 / (2.0 * thr), rel=1e-12)   # 100x larger would decouple it
+    if nd == 2:
+        assert iD[cells["five"]] == pytest.approx(-1.0 / 5e-6, rel=1e-12)
+    else:
+        assert iD[cells["five"]] == 0.0
+    far = (4, 6, 10) if nd == 3 else (0, 6, 10)
+    assert iD[far] == pytest.approx(-1.0 / (2 * nd), rel=1e-14)
+    s.close()
+
+
+def _periodic_laplacian_8x8():
+    T = _lap1d(8, True)
+    I = sp.identity(8)
+    return (sp.kron(I, T) + sp.kron(T, I)).tocsr()            # x fastest
+
+
+@pytest.mark.parametrize("delta,stops_after", [(1.3e-5, 1), (1.3e-4, 2)])
+def test_smoother_relative_stop_is_1e_minus_8(delta, stops_after):
+    """R-T on the 8x8 periodic level of the 2-D Taylor-Green case: no body, so iD = -1/4 everywhere and the
+    smoother is plain CG on the textbook Laplacian.  The residual is one eigenmode of amplitude 1 plus a
+    second one of amplitude delta (eigenvalues l1 = -4 sin^2(pi/8), l2 = -2: closed forms).  One CG
+    iteration removes the first mode and leaves rho'/rho0 = 5.83 delta^2 (1 + O(delta^2)):
+      delta = 1.3e-5 -> 9.9e-10 < 1e-8: the call must STOP after iteration 1, leaving x off the exact solution by
+                        delta |1/l1 - 1/l2| max|phi2| in the second mode (a stop at 1e-10 would go on and converge);
+      delta = 1.3e-4 -> 9.9e-8 > 1e-8: the call must go ON, and iteration 2 (two eigenmodes: CG is exact after
+                        two) lands on the exact solution (a stop at 1e-6 would leave it 1.6e-4 off).
+    The expected iterates come from an unguarded CG written here in numpy on scipy's kron Laplacian."""
+    n = 8
+    s = wo.OracleSim(wi.tgv2d(n, max_levels=1))
+    y, x = np.meshgrid(np.arange(n) + 0.5, np.arange(n) + 0.5, indexing="ij")
+    phi1, phi2 = np.cos(2 * np.pi * x / n), np.cos(2 * np.pi * 2 * y / n)
+    l1, l2 = -4 * np.sin(np.pi / n) ** 2, -4 * np.sin(2 * np.pi / n) ** 2
+    assert l2 == pytest.approx(-2.0, abs=1e-15)
+    r0 = phi1 + delta * phi2
+    s.interior("r")[0, 0][...] = r0
+    s.arr("x")[...] = 0.0
+    s.smooth(0, 6)
+    xo = s.interior("x")[0, 0].copy()
+    # unguarded Jacobi-PCG in numpy (iD = -1/4), keeping every iterate
+    A = _periodic_laplacian_8x8()
+    r = r0.ravel().copy(); xk = np.zeros(n * n); iD = -0.25
+    e = iD * r; rho = r @ e; rho0 = rho
+    iterates, ratios = [], []
+    for k in range(3):
+        q = A @ e; alpha = rho / (q @ e)
+        xk = xk + alpha * e; r = r - alpha * q
+        iterates.append(xk.reshape(n, n).copy())
+        z = iD * r; rho2 = r @ z
+        ratios.append(abs(rho2 / rho0))
+        e = (rho2 / rho) * e + z; rho = rho2
+    assert ratios[0] == pytest.approx(delta ** 2 * (1 - l2 / l1) ** 2, rel=1e-3)
+    assert (ratios[0] < 1e-8) == (stops_after == 1)
+    exact = phi1 / l1 + delta * phi2 / l2
+    assert np.abs(iterates[1] - exact).max() < 1e-13           # two modes: CG is exact after two iterations
+    assert np.abs(xo - iterates[stops_after - 1]).max() < 1e-13
+    off = np.abs(xo - exact).max()
+    if stops_after == 1:
+        assert off == pytest.approx(delta * abs(1 / l1 - 1 / l2) * np.abs(phi2).max(), rel=1e-3)   # stopped: second mode unsolved
+        assert np.abs(xo - iterates[1]).max() > 0.5 * off                      # going on WOULD have changed x
+    else:
+        assert off < 1e-13
+    s.close()
