@@ -41,8 +41,8 @@
 #define WLO_MAXLEV 16
 #define WLO_PI 3.14159265358979323846
 
-enum { WLO_BODY_NONE = 0, WLO_BODY_SPHERE = 1, WLO_BODY_TORUS = 2 };
-enum { WLO_MOTION_STATIC = 0, WLO_MOTION_HEAVE_SIN = 1 };
+enum { WLO_BODY_NONE = 0, WLO_BODY_SPHERE = 1, WLO_BODY_TORUS = 2, WLO_BODY_CYLINDER = 3 };
+enum { WLO_MOTION_STATIC = 0, WLO_MOTION_SIN = 1 };
 
 typedef struct {
     int ndim;
@@ -57,10 +57,10 @@ typedef struct {
     /* body: SDF + translation map */
     int body_kind;
     double centre[3];
-    double R, r;        /* sphere radius R; torus major R, minor r */
-    int axis;           /* torus axis */
-    int motion, heave_dir;
-    double amp, freq, phase;
+    double R, r;        /* sphere / cylinder radius R; torus major R, minor r */
+    int axis;           /* torus / cylinder axis */
+    int motion;
+    double amp[3], freq[3], phase[3];   /* c_d(t) = centre[d] + amp[d] sin(2 pi freq[d] t + phase[d]) */
     /* multigrid */
     int max_levels, smooth_iters, max_vcycles, fixed_vcycles;
     double tol;
@@ -155,8 +155,11 @@ double wlo_kernel_mu1(double d, double eps)
  * P:104 "AutoBody type holds the signed-distance function as well as the coordinates
  * mapping"; "signed-distance d and normal n from any point in space".  Reading R-E:
  * analytic gradients of the parametric SDFs (same values the paper gets by AD).
- * Maps are translations xi = x - c(t), c(t) = c0 + amp*sin(2 pi f t + phase) e_heave, so
- * J = I and V = dc/dt (uniform).  |grad| < 1e-12 => n = 0.
+ * Maps are translations xi = x - c(t), sinusoidal in every direction,
+ *   c_d(t) = c0_d + amp_d sin(2 pi f_d t + phase_d)
+ * (the heaving sphere of BASELINE configs[4]: one direction; the two-degree-of-freedom cylinder of P:181,
+ * y = A_y sin(w t), x = A_x sin(2 w t + theta): two), so J = I and V = dc/dt (uniform).  |grad| < 1e-12 => n = 0.
+ * The circular cylinder of P:121 (radius R, axis e_a, spanning a periodic direction): d = |xi - (xi.e_a) e_a| - R.
  * Returns d; fills nrm[3], vel[3].
  */
 double wlo_body_eval(const wlo_config *cf, const double *xpt, double t, double *nrm, double *vel)
@@ -166,10 +169,12 @@ double wlo_body_eval(const wlo_config *cf, const double *xpt, double t, double *
     nrm[0] = nrm[1] = nrm[2] = 0.0;
     vel[0] = vel[1] = vel[2] = 0.0;
     if (cf->body_kind == WLO_BODY_NONE) return 1e30;
-    if (cf->motion == WLO_MOTION_HEAVE_SIN) {
-        double ph = 2.0 * WLO_PI * cf->freq * t + cf->phase;
-        c[cf->heave_dir] += cf->amp * sin(ph);
-        vel[cf->heave_dir] = cf->amp * 2.0 * WLO_PI * cf->freq * cos(ph);
+    if (cf->motion == WLO_MOTION_SIN) {
+        for (int k = 0; k < nd; ++k) {
+            double ph = 2.0 * WLO_PI * cf->freq[k] * t + cf->phase[k];
+            c[k] += cf->amp[k] * sin(ph);
+            vel[k] = cf->amp[k] * 2.0 * WLO_PI * cf->freq[k] * cos(ph);
+        }
     }
     double xi[3] = { 0, 0, 0 };
     for (int k = 0; k < nd; ++k) xi[k] = xpt[k] - c[k];
@@ -180,9 +185,13 @@ double wlo_body_eval(const wlo_config *cf, const double *xpt, double t, double *
         if (rr >= 1e-12) for (int k = 0; k < nd; ++k) nrm[k] = xi[k] / rr;
         return rr - cf->R;
     }
-    /* torus (3-D): axis a; rho = distance from the axis in the (b,c) plane */
+    /* torus and cylinder (3-D): axis a; rho = distance from the axis in the (b,c) plane */
     int a = cf->axis, b = (a + 1) % 3, cc = (a + 2) % 3;
     double rho = sqrt(xi[b] * xi[b] + xi[cc] * xi[cc]);
+    if (cf->body_kind == WLO_BODY_CYLINDER) {
+        if (rho >= 1e-12) { nrm[b] = xi[b] / rho; nrm[cc] = xi[cc] / rho; }
+        return rho - cf->R;
+    }
     double w = rho - cf->R;
     double g = sqrt(w * w + xi[a] * xi[a]);
     if (g >= 1e-12 && rho >= 1e-12) {
@@ -866,17 +875,52 @@ void wlo_pressure_force(wlo_sim *s, double t, double *F)
     F[0] = F0; F[1] = F1; F[2] = F2;
 }
 
+/* -------------------------------------------------- kinetic energy and enstrophy
+ * P:169-173 (Fig. 4) follow the Taylor-Green vortex by its kinetic energy and enstrophy; the paper gives no
+ * discrete formula.  Reading R-E2, the plain staggered-grid sums over the interior cells c (h = 1):
+ *   KE = 1/2 sum_c sum_i u_i[c]^2                              (every face once: the lower faces of the cells)
+ *   Z  = 1/2 sum_c |w[c]|^2,  w_k[c] = (u_j[c] - u_j[c - d_i]) - (u_i[c] - u_i[c - d_j]),  (i, j, k) cyclic,
+ * the circulation around the cell edge along k through the lower-i, lower-j corner of cell c (2-D: w_z only).
+ * Ghost values come from the BC fill.  out[0] = KE, out[1] = Z. */
+void wlo_energy(wlo_sim *s, double *out)
+{
+    const wlo_level *g = &s->lev[0];
+    int nd = s->nd;
+    long nc = g->ncell;
+    double ke = 0, ens = 0;
+#pragma omp parallel for collapse(2) reduction(+ : ke, ens)
+    for (int c2 = ZLO(g, nd); c2 <= ZHI(g, nd); ++c2)
+        for (int c1 = 1; c1 <= g->n[1]; ++c1)
+            for (int c0 = 1; c0 <= g->n[0]; ++c0) {
+                long id = IDX(g, c0, c1, c2);
+                for (int i = 0; i < nd; ++i) ke += 0.5 * s->u[i * nc + id] * s->u[i * nc + id];
+                for (int k = (nd == 3 ? 0 : 2); k < 3; ++k) {
+                    int i = (k + 1) % 3, j = (k + 2) % 3;
+                    double w = (s->u[j * nc + id] - s->u[j * nc + id - g->st[i]])
+                             - (s->u[i * nc + id] - s->u[i * nc + id - g->st[j]]);
+                    ens += 0.5 * w * w;
+                }
+            }
+    out[0] = ke; out[1] = ens;
+}
+
 /* -------------------------------------------------- set-up */
 
 /* TGV initial condition (Eq. 3-5 with the sign of BASELINE configs[0],[1];
  * reading R-W): u = s sin(kx)cos(ky)[cos(kz)], v = -s cos(kx)sin(ky)[cos(kz)], w = 0,
- * k_d = 2 pi/N_d, sampled at the staggered face positions; then BC fill. */
+ * sampled at the staggered face positions; then BC fill.  k_d = 2 pi/N_d in a periodic direction (one
+ * period in the box); k_d = pi/N_d in a non-periodic one: the box is then the half-period [0, pi] between
+ * two symmetry planes of the vortex ("computational domain is the half-domain with symmetry boundary
+ * conditions"), where the normal component vanishes and the tangential ones are even -- exactly what the
+ * slip wall of reading R-M imposes when U = 0. */
 void wlo_init_tgv(wlo_sim *s, int sign)
 {
     const wlo_level *g = &s->lev[0];
     int nd = s->nd;
     long nc = g->ncell;
-    double k0 = 2 * WLO_PI / g->n[0], k1 = 2 * WLO_PI / g->n[1], k2 = nd == 3 ? 2 * WLO_PI / g->n[2] : 0;
+    const int *per = s->cfg.periodic;
+    double k0 = (per[0] ? 2 : 1) * WLO_PI / g->n[0], k1 = (per[1] ? 2 : 1) * WLO_PI / g->n[1];
+    double k2 = nd == 3 ? (per[2] ? 2 : 1) * WLO_PI / g->n[2] : 0;
     for (int c2 = 0; c2 < g->S[2]; ++c2)
         for (int c1 = 0; c1 < g->S[1]; ++c1)
             for (int c0 = 0; c0 < g->S[0]; ++c0) {
@@ -896,8 +940,8 @@ static int config_ok(const wlo_config *cf)
     if (cf->ndim != 2 && cf->ndim != 3) return 0;
     for (int d = 0; d < cf->ndim; ++d) if (cf->dims[d] < 4) return 0;
     if (cf->nu < 0 || !(cf->eps > 0)) return 0;
-    if (cf->body_kind < 0 || cf->body_kind > 2) return 0;
-    if (cf->body_kind == WLO_BODY_TORUS && cf->ndim != 3) return 0;
+    if (cf->body_kind < 0 || cf->body_kind > 3) return 0;
+    if ((cf->body_kind == WLO_BODY_TORUS || cf->body_kind == WLO_BODY_CYLINDER) && (cf->ndim != 3 || cf->axis < 0 || cf->axis > 2)) return 0;
     return 1;
 }
 

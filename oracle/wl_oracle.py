@@ -21,8 +21,8 @@ import numpy as np
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "wl_oracle.c"
 
-BODY_NONE, BODY_SPHERE, BODY_TORUS = 0, 1, 2
-MOTION_STATIC, MOTION_HEAVE_SIN = 0, 1
+BODY_NONE, BODY_SPHERE, BODY_TORUS, BODY_CYLINDER = 0, 1, 2, 3
+MOTION_STATIC, MOTION_SIN = 0, 1
 
 
 class Config(C.Structure):
@@ -33,8 +33,8 @@ class Config(C.Structure):
         ("eps", C.c_double),
         ("dt0", C.c_double), ("dt_max", C.c_double), ("cfl_c", C.c_double), ("cfl_cnu", C.c_double),
         ("body_kind", C.c_int), ("centre", C.c_double * 3), ("R", C.c_double), ("r", C.c_double),
-        ("axis", C.c_int), ("motion", C.c_int), ("heave_dir", C.c_int),
-        ("amp", C.c_double), ("freq", C.c_double), ("phase", C.c_double),
+        ("axis", C.c_int), ("motion", C.c_int),
+        ("amp", C.c_double * 3), ("freq", C.c_double * 3), ("phase", C.c_double * 3),
         ("max_levels", C.c_int), ("smooth_iters", C.c_int), ("max_vcycles", C.c_int),
         ("fixed_vcycles", C.c_int), ("tol", C.c_double),
     ]
@@ -108,6 +108,7 @@ def lib():
         L.wlo_cfl.argtypes = [C.c_void_p]
         L.wlo_pressure_force.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.wlo_init_tgv.argtypes = [C.c_void_p, C.c_int]
+        L.wlo_energy.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.wlo_nlevels.restype = C.c_int
         L.wlo_nlevels.argtypes = [C.c_void_p]
         L.wlo_stats.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_double)]
@@ -117,6 +118,17 @@ def lib():
         L.wlo_num_threads.restype = C.c_int
         _lib = L
     return _lib
+
+
+def wi_motion(cfg: dict):
+    """(amp[3], freq[3], phase[3]) of the sinusoidal translation from the plain dict: either three-vectors under
+    amp3 / freq3 / phase3, or the scalars amp / freq / phase acting along heave_dir (wl_inputs.CONFIG_DEFAULTS)."""
+    if cfg.get("amp3") is not None:
+        return ([float(v) for v in cfg["amp3"]], [float(v) for v in cfg["freq3"]], [float(v) for v in cfg["phase3"]])
+    a, f, p = [0.0] * 3, [0.0] * 3, [0.0] * 3
+    d = int(cfg["heave_dir"])
+    a[d], f[d], p[d] = float(cfg["amp"]), float(cfg["freq"]), float(cfg["phase"])
+    return a, f, p
 
 
 def make_config(cfg: dict) -> Config:
@@ -129,9 +141,12 @@ def make_config(cfg: dict) -> Config:
         c.U[d] = float(cfg["U"][d]) if d < len(cfg["U"]) else 0.0
         c.periodic[d] = int(cfg["periodic"][d]) if d < nd else 0
         c.centre[d] = float(cfg["centre"][d]) if d < len(cfg["centre"]) else 0.0
-    for k in ("L", "nu", "eps", "dt0", "dt_max", "cfl_c", "cfl_cnu", "R", "r", "amp", "freq", "phase", "tol"):
+    for k in ("L", "nu", "eps", "dt0", "dt_max", "cfl_c", "cfl_cnu", "R", "r", "tol"):
         setattr(c, k, float(cfg[k]))
-    for k in ("exit_bc", "body_kind", "axis", "motion", "heave_dir", "max_levels", "smooth_iters",
+    amp, freq, phase = wi_motion(cfg)
+    for d in range(3):
+        c.amp[d], c.freq[d], c.phase[d] = amp[d], freq[d], phase[d]
+    for k in ("exit_bc", "body_kind", "axis", "motion", "max_levels", "smooth_iters",
               "max_vcycles", "fixed_vcycles"):
         setattr(c, k, int(cfg[k]))
     return c
@@ -247,6 +262,12 @@ class OracleSim:
 
     def init_tgv(self, sign=1):
         lib().wlo_init_tgv(self._h, int(sign))
+
+    def energy(self) -> np.ndarray:
+        """(kinetic energy, enstrophy): the staggered-grid sums of reading R-E2"""
+        out = np.zeros(2)
+        lib().wlo_energy(self._h, _dp(out))
+        return out
 
     def matvec(self, level, x: np.ndarray):
         """q = A_level x on padded arrays (ghosts of x are wrapped in place); returns (q, q.x)."""

@@ -85,6 +85,8 @@ def test_quick_bounded_and_consistent():
 SPH = wi.make(ndim=3, dims=(32, 32, 32), body_kind=wi.BODY_SPHERE, centre=(16.0, 15.0, 17.0), R=8.0)
 TOR = wi.make(ndim=3, dims=(48, 48, 48), body_kind=wi.BODY_TORUS, centre=(20.0, 24.0, 24.0), R=12.0, r=4.0, axis=0)
 CIR = wi.make(ndim=2, dims=(32, 32), body_kind=wi.BODY_SPHERE, centre=(16.0, 16.0), R=6.0, periodic=(0, 0))
+CYL = wi.make(ndim=3, dims=(32, 32, 8), body_kind=wi.BODY_CYLINDER, centre=(15.0, 17.0, 0.0), R=5.0, axis=2, periodic=(0, 0, 1))
+CYLX = wi.make(ndim=3, dims=(8, 32, 32), body_kind=wi.BODY_CYLINDER, centre=(0.0, 15.0, 17.0), R=5.0, axis=0, periodic=(1, 0, 0))
 
 
 def test_sdf_known_points():
@@ -104,7 +106,21 @@ def test_sdf_known_points():
     assert wo.body_eval(CIR, c2 + [3, 4], 0)[0] == pytest.approx(-1.0)
 
 
-@pytest.mark.parametrize("cfg", [SPH, TOR, CIR])
+def test_cylinder_sdf_known_points_and_axis_invariance():
+    """PAPER.md:121 'circular cylinder ... periodic boundary condition on the spanwise direction': d = distance from
+    the axis - R, independent of the coordinate along the axis, normal in the cross-plane."""
+    c = np.array(CYL["centre"])
+    for z in (0.0, 3.3, 7.9, -40.0):
+        assert wo.body_eval(CYL, c + [0, 0, z], 0)[0] == pytest.approx(-5.0)
+        assert wo.body_eval(CYL, c + [3, 4, z], 0)[0] == pytest.approx(0.0, abs=1e-14)
+        d, n, _ = wo.body_eval(CYL, c + [6, -8, z], 0)
+        assert d == pytest.approx(5.0) and np.allclose(n, [0.6, -0.8, 0.0], atol=1e-15)
+    cx = np.array(CYLX["centre"])
+    d, n, _ = wo.body_eval(CYLX, cx + [2.5, 0, -13], 0)
+    assert d == pytest.approx(8.0) and np.allclose(n, [0.0, 0.0, -1.0], atol=1e-15)
+
+
+@pytest.mark.parametrize("cfg", [SPH, TOR, CIR, CYL, CYLX])
 def test_normal_is_unit_gradient_of_sdf(cfg):
     g = wi.rng(11)
     nd = cfg["ndim"]
@@ -132,6 +148,68 @@ def test_heave_velocity_is_time_derivative_of_centre():
         fd = (cy(t + 1e-5) - cy(t - 1e-5)) / 2e-5
         assert v[1] == pytest.approx(fd, abs=1e-8)
         assert v[0] == 0.0 and v[2] == 0.0
+
+
+def test_two_dof_motion_is_the_papers_map_and_V_its_time_derivative():
+    """y = A_y sin(w t), x = A_x sin(2 w t + theta); V = dc/dt, uniform in space.  The centre is read
+    back from the SDF at two far points on the axes through the initial centre."""
+    D = 16.0
+    cfg = wi.cylinder_2dof(16)
+    Ax, Ay, th, w = 0.4 * D, 1.6 * D, math.pi / 6, 2 * math.pi / (5.4 * D)
+    assert cfg["amp3"] == (Ax, Ay, 0.0) and cfg["phase3"] == (th, 0.0, 0.0)
+    assert cfg["freq3"][0] == pytest.approx(2 * w / (2 * math.pi)) and cfg["freq3"][1] == pytest.approx(w / (2 * math.pi))
+    c0 = np.array(cfg["centre"])
+    far_x, far_y = c0 + [500.0, 0, 3.0], c0 + [0, 500.0, 5.0]
+
+    def centre(t):
+        # on the x axis through the moving centre d = |x - c_x| - R only if y = c_y: use Pythagoras on both probes
+        dx = wo.body_eval(cfg, far_x, t)[0] + cfg["R"]          # sqrt((500 - ex)^2 + ey^2)
+        dy = wo.body_eval(cfg, far_y, t)[0] + cfg["R"]          # sqrt(ex^2 + (500 - ey)^2)
+        # two circles about the probes: solve for (ex, ey), the displacement of the centre
+        # dx^2 - dy^2 = -1000 ex + 1000 ey  and  dx^2 = (500 - ex)^2 + ey^2
+        k = (dx * dx - dy * dy) / 1000.0                         # ey - ex
+        # (500 - ex)^2 + (ex + k)^2 = dx^2  ->  2 ex^2 + (2k - 1000) ex + 250000 + k^2 - dx^2 = 0, the small root
+        a, b, cc = 2.0, 2 * k - 1000.0, 250000.0 + k * k - dx * dx
+        ex = (-b - math.sqrt(b * b - 4 * a * cc)) / (2 * a)
+        return np.array([ex, ex + k])
+
+    for t in (0.0, 7.3, 21.0, 50.0, 86.4):
+        e = centre(t)
+        assert e[0] == pytest.approx(Ax * math.sin(2 * w * t + th), abs=1e-9)
+        assert e[1] == pytest.approx(Ay * math.sin(w * t), abs=1e-9)
+        _, _, v = wo.body_eval(cfg, c0 + [3.0, -2.0, 1.0], t)
+        _, _, v2 = wo.body_eval(cfg, far_x, t)
+        assert np.array_equal(v, v2)                              # rigid translation: V is uniform
+        fd = (centre(t + 1e-4) - centre(t - 1e-4)) / 2e-4
+        assert v[0] == pytest.approx(fd[0], abs=1e-6) and v[1] == pytest.approx(fd[1], abs=1e-6) and v[2] == 0.0
+        assert v[0] == pytest.approx(2 * w * Ax * math.cos(2 * w * t + th), abs=1e-12)
+        assert v[1] == pytest.approx(w * Ay * math.cos(w * t), abs=1e-12)
+    # the motion closes after one period of the slow component, 5.4 D / U
+    assert np.allclose(centre(5.4 * D), centre(0.0), atol=1e-9)
+
+
+def test_cylinder_measure_is_invariant_along_the_axis_and_has_the_circle_area():
+    """measure! of the spanning cylinder: every field is independent of z (the paper's periodic spanwise direction),
+    and sum(1 - mu0) over the cells of one z-slab, with mu0 evaluated at the cell centres, is the area of the circle plus
+    the kernel's second-moment correction: int (1 - mu0(|x| - R)) dA = pi (R^2 + s2)."""
+    cfg = wi.make(ndim=3, dims=(32, 32, 8), body_kind=wi.BODY_CYLINDER, centre=(15.3, 16.6, 0.0), R=9.0, axis=2,
+                  periodic=(0, 0, 1), U=(1.0, 0.0, 0.0))
+    s = wo.OracleSim(cfg)
+    for name in ("mu0", "mu1", "V", "iD"):
+        a = s.interior(name)
+        assert np.array_equal(a, np.broadcast_to(a[:, :1], a.shape)), name
+    assert np.all(s.interior("mu1")[[2, 5, 8]] == 0.0)                # no normal component along the axis: mu1[i, z] = 0
+    for l in range(1, s.nlevels):
+        a = s.interior("L", l)
+        assert np.array_equal(a, np.broadcast_to(a[:, :1], a.shape))
+    s.close()
+    s2 = 1 / 3 - 2 / math.pi ** 2
+    area = 0.0
+    for x in np.arange(32) + 0.5:
+        for y in np.arange(32) + 0.5:
+            d = wo.body_eval(cfg, [x, y, 0.5], 0.0)[0]
+            area += 1.0 - wo.kernel_mu0(d, 1.0)
+    assert area == pytest.approx(math.pi * (81.0 + s2), rel=1e-3)
 
 
 def _centre_mu0_volume(cfg):

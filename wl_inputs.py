@@ -15,8 +15,9 @@ import numpy as np
 
 SEED = 20240716  # per-kernel parity inputs
 
-BODY_NONE, BODY_SPHERE, BODY_TORUS = 0, 1, 2
-MOTION_STATIC, MOTION_HEAVE_SIN = 0, 1
+BODY_NONE, BODY_SPHERE, BODY_TORUS, BODY_CYLINDER = 0, 1, 2, 3
+MOTION_STATIC, MOTION_SIN = 0, 1
+MOTION_HEAVE_SIN = MOTION_SIN          # one direction of the sinusoidal translation (heave_dir, amp, freq, phase)
 
 CONFIG_DEFAULTS = dict(
     ndim=3, dims=(32, 32, 32), L=1.0, U=(1.0, 0.0, 0.0), nu=0.01,
@@ -24,6 +25,8 @@ CONFIG_DEFAULTS = dict(
     dt0=0.25, dt_max=10.0, cfl_c=1.0, cfl_cnu=5.0,
     body_kind=BODY_NONE, centre=(0.0, 0.0, 0.0), R=0.0, r=0.0, axis=0,
     motion=MOTION_STATIC, heave_dir=1, amp=0.0, freq=0.0, phase=0.0,
+    amp3=None, freq3=None, phase3=None,     # sinusoidal translation in every direction (overrides the four above)
+    tune=None,                              # implementation switches of the CUDA library (wl_tuning), a dict
     max_levels=0, smooth_iters=6, max_vcycles=32, fixed_vcycles=2, tol=1e-4,
 )
 
@@ -78,6 +81,31 @@ def heaving_sphere(dims=(384, 256, 256), D=48.0, Re=1000.0, St=0.2, amp_over_D=0
     base = dict(ndim=3, dims=tuple(dims), L=D, U=(1.0, 0.0, 0.0), nu=D / Re, exit_bc=1,
                 body_kind=BODY_SPHERE, centre=tuple(centre), R=D / 2.0,
                 motion=MOTION_HEAVE_SIN, heave_dir=1, amp=amp_over_D * D, freq=St / D)
+    base.update(kw)
+    return make(**base)
+
+
+def cylinder_2dof(L=64, Re=1000.0, **kw) -> dict:
+    """SURVEY 8(f) NEXT-1, the paper's third benchmark case: circular cylinder of diameter L cells
+    spanning the periodic z direction of a 9L x 6L x 2L box, inflow +x, convective exit, slip in y, Re = U L / nu,
+    with the prescribed two-degree-of-freedom motion of PAPER.md:181: y = A_y sin(w t), x = A_x sin(2 w t + theta),
+    A_y = 1.6 D, A_x = 0.4 D, theta = pi/6, w = (2 pi / 5.4) U / D.  The paper does not say where the cylinder
+    sits in the benchmark box: centre (3L, 3L) here."""
+    D = float(L)
+    f = 1.0 / (5.4 * D)
+    base = dict(ndim=3, dims=(9 * L, 6 * L, 2 * L), L=D, U=(1.0, 0.0, 0.0), nu=D / Re, periodic=(0, 0, 1), exit_bc=1,
+                body_kind=BODY_CYLINDER, axis=2, centre=(3.0 * L, 3.0 * L, 0.0), R=D / 2.0, motion=MOTION_SIN,
+                amp3=(0.4 * D, 1.6 * D, 0.0), freq3=(2.0 * f, f, 0.0), phase3=(math.pi / 6.0, 0.0, 0.0))
+    base.update(kw)
+    return make(**base)
+
+
+def tgv3d_half(n=512, Re=1600.0, **kw) -> dict:
+    """SURVEY 8(f) NEXT-3, the paper's first benchmark case as it states it: the Taylor-Green vortex on
+    the half-domain [0, pi]^3 of n^3 cells between symmetry planes (slip walls with U = 0), kappa = pi / n,
+    Re = U / (kappa nu)."""
+    Lref = n / math.pi
+    base = dict(ndim=3, dims=(n, n, n), L=Lref, U=(0.0, 0.0, 0.0), nu=Lref / Re, periodic=(0, 0, 0))
     base.update(kw)
     return make(**base)
 
