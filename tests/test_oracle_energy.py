@@ -85,7 +85,8 @@ def test_2d_vortex_energy_and_enstrophy_decay_at_the_viscous_rate():
     """C1 (BASELINE configs[0]: 64^2, nu = dt = 0.01 physical, 20 steps): the 2-D Taylor-Green vortex is an exact
     solution whose amplitude decays as exp(-2 nu kappa^2 t), so KE and Z, both quadratic, decay as exp(-4 nu kappa^2 t)
     = exp(-0.008) -- with the DISCRETE Laplacian eigenvalue 2 (2 s)^2 in place of 2 kappa^2 (s = sin(kappa/2)), which at
-    64 cells changes the exponent by 8e-4 relative."""
+    64 cells changes the exponent by 8e-4 relative.  The upwind-biased convective flux adds a little dissipation of its own
+    (third-order: 2.4e-5 of the energy over these 20 steps), hence the tolerance 5e-5."""
     cfg = wi.baseline_config(0)
     s = wo.OracleSim(cfg)
     s.init_tgv(1)
@@ -97,6 +98,7 @@ def test_2d_vortex_energy_and_enstrophy_decay_at_the_viscous_rate():
     rate = 2.0 * nu * 2.0 * (2.0 * math.sin(math.pi / n)) ** 2        # d/dt of a quadratic: twice the amplitude rate
     expect = math.exp(-rate * 20 * cfg["nu"])
     assert expect == pytest.approx(math.exp(-0.008), rel=1e-5)
-    assert e1[0] / e0[0] == pytest.approx(expect, rel=2e-5)
-    assert e1[1] / e0[1] == pytest.approx(expect, rel=2e-5)
+    assert e1[0] / e0[0] == pytest.approx(expect, rel=5e-5)
+    assert e1[1] / e0[1] == pytest.approx(expect, rel=5e-5)
+    assert e1[0] / e0[0] < expect and e1[1] / e0[1] < expect          # the scheme never adds energy
     s.close()
