@@ -42,18 +42,22 @@ extern "C" {
 #define WL_ECUDA    -3   /* CUDA error (sticky); text through wl_last_error */
 #define WL_ENOCONV  -4   /* tolerance-mode Poisson solve hit max_vcycles (result still written) */
 
-/* body kinds and motions: SDF + coordinate map of the paper's AutoBody */
-enum { WL_BODY_NONE = 0, WL_BODY_SPHERE = 1 /* circle in 2-D */, WL_BODY_TORUS = 2 };
-enum { WL_MOTION_STATIC = 0, WL_MOTION_HEAVE_SIN = 1 /* c(t) = c0 + amp sin(2 pi freq t + phase) e_heave */ };
+/* body kinds and motions: SDF + coordinate map of the paper's AutoBody.
+ * WL_BODY_CYLINDER is the circular cylinder of P:121 / P:179 (radius R, infinitely long along `axis`: it spans a
+ * periodic direction).  WL_MOTION_SIN is a rigid translation, sinusoidal in every direction:
+ *     c_d(t) = centre[d] + amp[d] sin(2 pi freq[d] t + phase[d]),   V_d = dc_d/dt  (uniform in space),
+ * which covers the heaving sphere (one non-zero amp) and the two-degree-of-freedom cylinder of P:181,
+ * y = A_y sin(w t), x = A_x sin(2 w t + theta). */
+enum { WL_BODY_NONE = 0, WL_BODY_SPHERE = 1 /* circle in 2-D */, WL_BODY_TORUS = 2, WL_BODY_CYLINDER = 3 };
+enum { WL_MOTION_STATIC = 0, WL_MOTION_SIN = 1 };
 
 typedef struct {
     int   kind;          /* WL_BODY_* */
     float centre[3];     /* c0, grid units */
-    float R, r;          /* sphere radius R; torus major R, minor r */
-    int   axis;          /* torus axis 0..2 */
+    float R, r;          /* sphere / cylinder radius R; torus major R, minor r */
+    int   axis;          /* torus / cylinder axis 0..2 */
     int   motion;        /* WL_MOTION_* */
-    int   heave_dir;     /* 0..2 */
-    float amp, freq, phase;
+    float amp[3], freq[3], phase[3];
 } wl_body;
 
 typedef struct {
@@ -64,6 +68,20 @@ typedef struct {
     float tol;           /* tolerance mode: stop when max|r| <= tol */
 } wl_mg;
 
+/* Implementation switches, for A/B tests of alternative kernel paths (tests/test_gpu_paths.py) and tuning runs.
+ * All zero = the defaults.  Part of the config so that a handle carries no hidden state: the library reads no
+ * environment variable. */
+typedef struct {
+    int no_fused;        /* PCG smoother as two passes per iteration instead of the one-sweep form (wl_pcgfused.cu) */
+    int no_fast_a;       /* register-marching pass A everywhere (no shared-memory kernel) */
+    int no_bulk;         /* pass A stages its planes with per-thread cp.async instead of TMA boxes */
+    int no_block_levels; /* small levels by the cooperative kernel instead of the one-block kernel */
+    int no_tma_cd;       /* conv_diff from the register-staged ring (k_cd_tile2) instead of the TMA-fed one */
+    int zc;              /* planes per tile of the vector kernels (0: 8) */
+    long long pk_max_cells; /* levels >= 1 with at most this many cells run inside the persistent kernels (0: 1 M; < 0: none) */
+    int pk_blocks_per_sm;   /* co-resident blocks per SM of the cooperative kernel (0: 2) */
+} wl_tuning;
+
 /* Problem statement (grid size, boundary velocity, length scale, viscosity, BC type,
  * body).  POD, caller-owned, copied at create. */
 typedef struct {
@@ -72,12 +90,14 @@ typedef struct {
     float L;             /* length scale; only scales reported quantities */
     float U[3];          /* boundary / inflow velocity */
     float nu;            /* kinematic viscosity in grid units */
-    int   periodic[3];   /* per direction */
+    int   periodic[3];   /* per direction; a non-periodic direction is a slip wall with normal velocity U_d: with
+                            U_d = 0 that is the symmetry plane of P:118 (normal component 0, tangential mirrored) */
     int   exit_bc;       /* convective exit on the +x plane */
     float eps;           /* BDIM kernel half-width in cells */
     float dt0, dt_max, cfl_c, cfl_cnu;   /* CFL rule, DESIGN.md R-U */
     wl_body body;
     wl_mg   mg;
+    wl_tuning tune;
 } wl_config;
 
 typedef struct wl_sim wl_sim;
@@ -88,6 +108,8 @@ typedef struct {
     int    nlevels;
     int    kernel_launches;   /* kernels launched by this handle since create */
     int    nan_flag;          /* 1 if the last CFL reduction saw a non-finite velocity */
+    int    noconv;            /* tolerance-mode solves since create that hit max_vcycles (WL_ENOCONV is also
+                                 returned, once, by the next wl_cfl) */
 } wl_stats_t;
 
 /* Pure function: bytes of device workspace wl_sim_create needs; 0 on invalid config. */
@@ -105,9 +127,10 @@ int wl_sim_destroy(wl_sim* s);
  * p: one.  Ghost cells are then filled by the BC rule.  Synchronises when host. */
 int wl_set_fields(wl_sim* s, const float* u, const float* p, int on_device);
 
-/* Taylor-Green initial condition of P:112-116 (Eq. 3-5) on the periodic box, staggered
- * sampling; sign = +1 gives BASELINE.json's u = sin x cos y [cos z], v = -cos x sin y [cos z];
- * sign = -1 gives the paper's.  p = 0. */
+/* Taylor-Green initial condition of P:112-116 (Eq. 3-5), staggered sampling; sign = +1 gives BASELINE.json's
+ * u = sin x cos y [cos z], v = -cos x sin y [cos z]; sign = -1 gives the paper's.  One period of the vortex in every
+ * periodic direction, half a period in every non-periodic one (the half-domain between symmetry planes of P:118:
+ * use U = 0).  p = 0. */
 int wl_init_tgv(wl_sim* s, int sign);
 
 /* measure!: evaluate the SDF and motion map at every face at time t (solver
@@ -125,17 +148,22 @@ int wl_mom_step(wl_sim* s, float dt);
 int wl_cfl(wl_sim* s, float* dt_out);
 
 /* Pressure force ON THE BODY, grid units (rho = 1, h = 1), reading R-Z:
- * F = -sum_cells p n K(d) at cell centres, body placed at time t.  Synchronises. */
+ * F = -sum_cells p n K(d) at cell centres, body placed at time t (NaN: where the last measure! placed it).  Neither
+ * the stored body state nor the simulation time changes.  Synchronises. */
 int wl_pressure_force(wl_sim* s, double t, float F_out[3]);
+
+/* Kinetic energy and enstrophy of the current velocity (Fig. 4 follows the Taylor-Green vortex by them;
+ * reading R-E2): out[0] = 1/2 sum_cells sum_i u_i^2, out[1] = 1/2 sum_cells |w|^2 with w the circulations around the
+ * cell edges through the lower corner of each cell, grid units.  fp64 partial sums, fixed tree.  Synchronises. */
+int wl_energy(wl_sim* s, double out[2]);
 
 /* Copy interior fields out; any pointer may be NULL.  u: ndim arrays; p, mu0 likewise
  * (mu0: ndim arrays).  Synchronises when host. */
 int wl_get_fields(wl_sim* s, float* u, float* p, float* mu0, int on_device);
 
-/* Fused benchmark step: wl_measure(t) (only if the body moves) + wl_mom_step(dt) +
- * the CFL reduction, all asynchronous; the new dt stays on the device and is read by
- * wl_cfl_result.  With `adaptive` != 0 the NEXT call ignores `dt` and uses the device-
- * resident dt (no host round trip).  */
+/* Fused step: wl_measure(t) (only if the body moves) + wl_mom_step(dt) + the CFL reduction, all asynchronous; t is
+ * the time the step ends at (R-R) and becomes the simulation time.  With `adaptive` != 0 the NEXT call ignores `t` and
+ * `dt` and uses the device-resident CFL result and simulation time + dt (no host round trip). */
 int wl_step(wl_sim* s, double t, float dt, int adaptive);
 
 /* ---- stage hooks: each applies one stage once to the current state (parity tests) ---- */
@@ -150,14 +178,10 @@ int wl_dbg_restrict(wl_sim* s, int level);
 int wl_dbg_prolong(wl_sim* s, int level);
 int wl_dbg_smooth(wl_sim* s, int level, int iters);
 int wl_dbg_vcycle(wl_sim* s, int level);
-/* Runs n coarse-level passes as one chain through the persistent kernels (DESIGN.md 6.3): kinds[k] = 0 restrict
- * levels[k] -> levels[k]+1, 1 smooth level levels[k] with iters[k] PCG iterations, 2 prolong levels[k]+1 ->
- * levels[k], 3 one grid-wide reduction only, 4 one barrier only (timing probes).  Consecutive passes of the same
- * kind of launch (whole-GPU cooperative k_coarse / one-cluster k_tiny) share a launch.  n <= 48. */
+/* Runs n coarse-level passes as one chain through the persistent kernels (DESIGN.md 6.4): kinds[k] = 0 restrict
+ * levels[k] -> levels[k]+1, 1 smooth level levels[k] with iters[k] PCG iterations, 2 prolong levels[k]+1 -> levels[k].
+ * Consecutive passes of the same kind of launch share a launch.  n <= 48. */
 int wl_dbg_coarse_prog(wl_sim* s, int n, const int* kinds, const int* levels, const int* iters);
-/* %globaltimer (ns) at the start of every pass of the LAST persistent-kernel launch and at its end: n values
- * (n - 1 passes).  Synchronises. */
-int wl_dbg_coarse_times(wl_sim* s, unsigned long long* out, int n);
 /* Device-resident PCG scalars of a level: rho, gamma, alpha, beta, rho0, sum of r over the coupled cells (R-T2),
  * number of coupled cells, live flag.  Synchronises. */
 int wl_dbg_pcg_scalars(wl_sim* s, int level, double out[8]);

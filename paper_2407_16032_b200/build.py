@@ -23,7 +23,7 @@ HEADERS = ["wl_common.cuh", "wl_body.cuh", "wl_vec.cuh", "wl_tma.cuh", "wl_inter
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr",
-] + os.environ.get("WL_NVCC_EXTRA", "").split()      # e.g. -DWL_A_MINB=3 for tuning experiments
+]
 
 
 def _nvcc() -> str:

@@ -62,10 +62,10 @@ static int config_ok(const wl_config* c)
     if (c->ndim != 2 && c->ndim != 3) return 0;
     for (int d = 0; d < c->ndim; ++d) if (c->dims[d] < 4 || c->dims[d] > 16384) return 0;
     if (!(c->nu >= 0.0f) || !(c->eps > 0.0f)) return 0;
-    if (c->body.kind < 0 || c->body.kind > 2) return 0;
-    if (c->body.kind == WL_BODY_TORUS && (c->ndim != 3 || c->body.axis < 0 || c->body.axis > 2)) return 0;
+    if (c->body.kind < 0 || c->body.kind > 3) return 0;
+    if ((c->body.kind == WL_BODY_TORUS || c->body.kind == WL_BODY_CYLINDER) && (c->ndim != 3 || c->body.axis < 0 || c->body.axis > 2)) return 0;
     if (c->body.motion < 0 || c->body.motion > 1) return 0;
-    if (c->body.motion == WL_MOTION_HEAVE_SIN && (c->body.heave_dir < 0 || c->body.heave_dir >= c->ndim)) return 0;
+    if (c->tune.zc < 0 || c->tune.zc > 64 || c->tune.pk_blocks_per_sm < 0) return 0;
     if (c->exit_bc && c->periodic[0]) return 0;
     if (c->mg.smooth_iters < 1) return 0;
     return 1;
@@ -92,16 +92,15 @@ static Grid make_grid(int nd, const int* n, const int* per)
 #define WL_PK_MIN_TILES 256     // the persistent-kernel levels take fewer planes per tile until they have this many tiles
 #endif
 // levels with at most this many cells run inside the persistent coarse-level kernels (k_coarse / k_tiny)
-static long long pk_max_cells()
+static long long pk_max_cells(const wl_config* c)
 {
-    long long maxc = 1000000;
-    if (const char* e = getenv("WL_PK_MAX_CELLS")) maxc = atoll(e);
-    return maxc;
+    if (c->tune.pk_max_cells < 0) return 0;
+    return c->tune.pk_max_cells > 0 ? c->tune.pk_max_cells : 1000000;
 }
 
 // Vector tiling of a level.  Coarse levels are latency-bound, not bandwidth-bound: they take fewer
 // planes per tile so that enough tiles (>= 4 per SM of a 148-SM B200 where the level allows) are in flight.
-static VT make_vt(int nd, const Grid& g, int level)
+static VT make_vt(const wl_config* c, int nd, const Grid& g, int level)
 {
     VT t;
     t.ngx = (g.n[0] + 3) / 4;
@@ -110,10 +109,9 @@ static VT make_vt(int nd, const Grid& g, int level)
     const int lx = 1 << t.lxl, ly = WL_VB >> t.lxl;
     t.ntx = (t.ngx + lx - 1) / lx;
     t.nty = (g.n[1] + ly - 1) / ly;
-    int zc0 = 8;
-    if (const char* e = getenv("WL_ZC")) { int v = atoi(e); if (v >= 1 && v <= 64) zc0 = v; }     // planes per tile (tuning)
+    const int zc0 = c->tune.zc > 0 ? c->tune.zc : 8;      // planes per tile
     t.zc = nd == 3 ? (g.n[2] < zc0 ? g.n[2] : zc0) : 1;
-    if (level > 0 && (long long)g.n[0] * g.n[1] * g.n[2] <= pk_max_cells())
+    if (level > 0 && (long long)g.n[0] * g.n[1] * g.n[2] <= pk_max_cells(c))
         while (t.zc > 1 && (int64_t)t.ntx * t.nty * ((g.n[2] + t.zc - 1) / t.zc) < WL_PK_MIN_TILES) t.zc = (t.zc + 1) / 2;
     t.ntz = nd == 3 ? (g.n[2] + t.zc - 1) / t.zc : 1;
     t.ntiles = t.ntx * t.nty * t.ntz;
@@ -186,10 +184,10 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
         float* e = (float*)cv.take(scl);
         float* e2 = (float*)cv.take(scl);
         float* q = (float*)cv.take(scl);
-        VT vt = make_vt(nd, g, l);
+        VT vt = make_vt(c, nd, g, l);
         // the one-sweep PCG form (wl_pcgfused.cu) ping-pongs r and q: two more arrays on the levels that take it.  Level 0
         // borrows them from the velocity buffer that is dead during the projection (solver_scratch()).
-        const bool fused = wl_pcg_fused_shape(nd, g, vt) && (l == 0 || (long long)g.n[0] * g.n[1] * g.n[2] > pk_max_cells());
+        const bool fused = wl_pcg_fused_shape(nd, g, vt) && (l == 0 || (long long)g.n[0] * g.n[1] * g.n[2] > pk_max_cells(c));
         float* r2 = fused && l > 0 ? (float*)cv.take(scl) : nullptr;
         float* q2 = fused && l > 0 ? (float*)cv.take(scl) : nullptr;
         if (s && l == 0) s->fused0 = fused ? 1 : 0;
@@ -213,7 +211,7 @@ extern "C" size_t wl_workspace_bytes(const wl_config* cfg)
     return layout(nullptr, cfg, nullptr);
 }
 
-extern "C" int wl_abi_version(void) { return 1; }
+extern "C" int wl_abi_version(void) { return 2; }
 
 // ------------------------------------------------------------------ the step
 static void bc_all(wl_sim* s, float* u) { wl_k_bc(s, u); }
@@ -238,7 +236,7 @@ static int solve(wl_sim* s)
             ++nv;
         }
         s->res[s->solve_slot] = res;
-        if (res > (double)mg.tol) s->noconv = 1;
+        if (res > (double)mg.tol) { s->noconv = 1; s->noconv_total++; }
     }
     s->vcycles[s->solve_slot] = nv;
     return WL_OK;
@@ -323,23 +321,18 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     s->u = s->ubuf[0]; s->u0 = s->ubuf[1]; s->ut = s->ubuf[2];
     solver_scratch(s, s->u);
     {   // levels that run inside the persistent coarse-level kernel: from the first level >= 1 small enough
-        const long long maxc = pk_max_cells();
+        const long long maxc = pk_max_cells(cfg);
         s->pk_level = s->nlev;
         for (int l = s->nlev - 1; l >= 1; --l) {
             const Grid& g = s->lev[l].g;
             if ((long long)g.n[0] * g.n[1] * g.n[2] <= maxc) s->pk_level = l; else break;
         }
     }
-    s->fast_A = 1;
-    s->fused = 1;
-    if (const char* e = getenv("WL_FUSED")) s->fused = atoi(e) != 0;
-    s->tiny_on = 1;
-    s->bulk_A = 1;
-    s->cd_kernel = 3;
-    if (const char* e = getenv("WL_CD")) { int v = atoi(e); if (v >= 1 && v <= 3) s->cd_kernel = v; }
-    if (const char* e = getenv("WL_BULK")) s->bulk_A = atoi(e) != 0;
-    if (const char* e = getenv("WL_TINY")) s->tiny_on = atoi(e) != 0;
-    if (const char* e = getenv("WL_FAST_A")) s->fast_A = atoi(e) != 0;
+    s->fast_A = !cfg->tune.no_fast_a;
+    s->fused = !cfg->tune.no_fused;
+    s->tiny_on = !cfg->tune.no_block_levels;
+    s->bulk_A = !cfg->tune.no_bulk;
+    s->tma_cd = !cfg->tune.no_tma_cd;
     s->body.kind = cfg->body.kind; s->body.axis = cfg->body.axis;
     s->body.R = cfg->body.R; s->body.r = cfg->body.r; s->body.eps = cfg->eps;
     int dev = 0;
@@ -363,7 +356,7 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     if (cudaMemcpyAsync(s->levdev, hl, sizeof(hl), cudaMemcpyHostToDevice, s->st) != cudaSuccess) { cudaFreeHost(s->hs); delete s; return WL_ECUDA; }
     // initial state (R-V): u = U everywhere (all three buffers, so the exit plane is defined), p = 0, measure(0)
     for (int k = 0; k < 3; ++k) wl_k_fill_u(s, s->ubuf[k]);
-    wl_k_set_time(s, 0.0, cfg->dt0, 1, 1);
+    wl_k_set_time(s, 0.0, cfg->dt0, 2, 1);
     wl_k_measure(s);
     bc_all(s, s->u);
     int rc = sync(s);
@@ -474,7 +467,7 @@ extern "C" int wl_step(wl_sim* s, double t, float dt, int adaptive)
     if (!s) return WL_EINVAL;
     int dev = adaptive && s->primed;   // device-resident t and dt are valid
     if (!dev && !(dt > 0.0f)) return WL_EINVAL;
-    wl_k_set_time(s, t, dt, dev ? 0 : 1, dev ? 0 : 1);
+    wl_k_set_time(s, t, dt, dev ? 0 : 2, dev ? 0 : 1);
     if (s->cfg.body.kind != WL_BODY_NONE && s->cfg.body.motion != WL_MOTION_STATIC) wl_k_measure(s);
     int rc = mom_step_body(s);
     if (rc != WL_OK) return rc;
@@ -499,12 +492,22 @@ extern "C" int wl_cfl(wl_sim* s, float* dt_out)
 extern "C" int wl_pressure_force(wl_sim* s, double t, float F_out[3])
 {
     if (!s || !F_out) return WL_EINVAL;
-    if (t == t) wl_k_set_time(s, t, 0.0f, 1, -1);    // NaN: keep the device-resident body state
-    wl_k_force(s);
+    wl_k_force(s, t);                                // NaN: the body where measure! last placed it
     WL_CUDA_CHECK(s, cudaMemcpyAsync(s->hs->force, s->ds->force, 3 * sizeof(double), cudaMemcpyDeviceToHost, s->st));
     int rc = sync(s);
     if (rc != WL_OK) return rc;
     for (int k = 0; k < 3; ++k) F_out[k] = (float)s->hs->force[k];
+    return WL_OK;
+}
+
+extern "C" int wl_energy(wl_sim* s, double out[2])
+{
+    if (!s || !out) return WL_EINVAL;
+    wl_k_energy(s, s->u);
+    WL_CUDA_CHECK(s, cudaMemcpyAsync(s->hs->energy, s->ds->energy, 2 * sizeof(double), cudaMemcpyDeviceToHost, s->st));
+    int rc = sync(s);
+    if (rc != WL_OK) return rc;
+    out[0] = s->hs->energy[0]; out[1] = s->hs->energy[1];
     return WL_OK;
 }
 
@@ -516,6 +519,7 @@ extern "C" int wl_stats(wl_sim* s, wl_stats_t* out)
     out->nlevels = s->nlev;
     out->kernel_launches = s->launches;
     out->nan_flag = s->hs->nan_flag;
+    out->noconv = s->noconv_total;
     return WL_OK;
 }
 
@@ -627,19 +631,11 @@ extern "C" int wl_dbg_coarse_prog(wl_sim* s, int n, const int* kinds, const int*
     CoarseProg P; P.n = n;
     for (int k = 0; k < n; ++k) {
         const int top = kinds[k] == COP_SMOOTH ? s->nlev - 1 : s->nlev - 2;
-        if (kinds[k] < 0 || kinds[k] > 4 || levels[k] < 0 || levels[k] > top || (kinds[k] == COP_SMOOTH && iters[k] < 1)) return WL_EINVAL;
+        if (kinds[k] < 0 || kinds[k] > 2 || levels[k] < 0 || levels[k] > top || (kinds[k] == COP_SMOOTH && iters[k] < 1)) return WL_EINVAL;
         P.op[k].kind = kinds[k]; P.op[k].level = levels[k]; P.op[k].iters = iters[k];
     }
     wl_k_coarse_prog(s, P);
     return check(s);
-}
-
-// pass start times (ns, %globaltimer) of the last k_coarse launch: n+1 values for n passes
-extern "C" int wl_dbg_coarse_times(wl_sim* s, unsigned long long* out, int n)
-{
-    if (!s || !out || n < 1 || n > 3 * WL_MAXLEV + 1) return WL_EINVAL;
-    WL_CUDA_CHECK(s, cudaMemcpyAsync(out, s->ds->pk_t, sizeof(unsigned long long) * n, cudaMemcpyDeviceToHost, s->st));
-    return sync(s);
 }
 
 // PCG scalars of a level: rho, gamma, alpha, beta, rho0, rsum, nlive, live

@@ -7,14 +7,15 @@
 
 struct BodyP {
     int kind;        // WL_BODY_*
-    int axis;        // torus axis
-    float R, r;      // sphere radius R; torus major R / minor r
+    int axis;        // torus / cylinder axis
+    float R, r;      // sphere / cylinder radius R; torus major R / minor r
     float eps;       // BDIM kernel half-width
 };
 
 #define WLB_NONE 0
 #define WLB_SPHERE 1
 #define WLB_TORUS 2
+#define WLB_CYLINDER 3
 
 // cosine kernel K(s) = (1 + cos(pi s/eps)) / (2 eps) on |s| < eps
 __device__ __forceinline__ float bdim_K(float s, float eps)
@@ -69,12 +70,20 @@ __device__ __forceinline__ T body_sdf(const BodyP& b, const T (&xi)[3], T (&nrm)
         }
         return rr - (T)b.R;
     }
-    // torus: axis a, rho = distance from the axis
+    // torus and cylinder: axis a, rho = distance from the axis
     T xa, xb, xc;
     if (b.axis == 0) { xa = xi[0]; xb = xi[1]; xc = xi[2]; }
     else if (b.axis == 1) { xa = xi[1]; xb = xi[2]; xc = xi[0]; }
     else { xa = xi[2]; xb = xi[0]; xc = xi[1]; }
     T rho = sqrt(xb * xb + xc * xc);
+    if (b.kind == WLB_CYLINDER) {          // circular cylinder along the axis: d = rho - R, normal in the cross-plane
+        T nb = T(0), nc = T(0);
+        if (rho >= tiny) { T ir = T(1) / rho; nb = xb * ir; nc = xc * ir; }
+        if (b.axis == 0) { nrm[1] = nb; nrm[2] = nc; }
+        else if (b.axis == 1) { nrm[2] = nb; nrm[0] = nc; }
+        else { nrm[0] = nb; nrm[1] = nc; }
+        return rho - (T)b.R;
+    }
     T w = rho - (T)b.R;
     T gq = sqrt(w * w + xa * xa);
     T na = T(0), nb = T(0), nc = T(0);

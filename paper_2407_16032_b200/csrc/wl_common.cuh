@@ -54,8 +54,10 @@ struct PcgScal {
 
 struct DevScal {
     PcgScal pcg[WL_MAXLEV];
-    double t;            // time at which the body was last measured
-    double centre[3];    // body centre at that time
+    double t;            // time at which the body was last placed (measure!)
+    double t_step;       // simulation time advanced by wl_step (never touched by wl_measure / wl_pressure_force)
+    double centre[3];    // body centre at time t
+    double centre_f[3];  // body centre the pressure-force integral is taken at
     float  vel[3];       // body velocity V (rigid translation: uniform)
     float  dt;           // time step of the running step
     float  dt_next;      // CFL result
@@ -66,7 +68,7 @@ struct DevScal {
     double resmax;
     int    nan_flag;
     int    band_count;   // faces with mu1 != 0 found by the last measure! (may exceed the list capacity)
-    unsigned long long pk_t[3 * WL_MAXLEV + 1];   // %globaltimer at the start of every pass of the last k_coarse launch, and at its end
+    double energy[2];    // kinetic energy, enstrophy (wl_energy)
 };
 
 // reduction scratch: partial sums of up to 4 values per block + the arrival counter

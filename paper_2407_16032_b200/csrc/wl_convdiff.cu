@@ -4,16 +4,18 @@
 //   f   = u0 + dt r - V ;  B_i = V_i + mu0 f_i + sum_j mu1_ij (f_i[c+d_j] - f_i[c-d_j])/2
 //                                          (Eq. 1-2; R-B, R-C)
 //   predictor: u = B ; corrector: u = (u' + B)/2            (P:76, P:139 scale_u!; R-K, R-L)
-// f is never stored.  Two kernels:
-//  * k_cd_tile: the whole grid.  A block owns a 128 x 8 column of cells and marches along z; the
-//    three velocity components of the five planes z-2..z+2 (with a two-cell halo in x and y,
-//    periodic wrap applied while loading) sit in a shared-memory ring, so every value is read from
-//    HBM/L2 once per tile and all stencil reads are conflict-free 16-byte shared loads.  Each
-//    thread owns four consecutive x cells: x-face fluxes are shared inside the thread.  It
-//    writes u = V + mu0 f (with the Heun average in the corrector) and never reads mu1.
-//  * k_cd_band: mu1 is non-zero only within eps of the body surface; measure! leaves a compact
-//    list of those faces (wl_flow.cu) and this kernel adds sum_j mu1_ij (f_i[c+d_j]-f_i[c-d_j])/2
-//    there, recomputing the six neighbouring r from global memory.
+// f is never stored.  Kernels:
+//  * k_cd_tile3 (3-D, x and y not periodic: every inflow/outflow case) and k_cd_tile2 (everything else): the whole grid.
+//    A block of 256 x ND threads owns a 128 x 8 column of cells and marches along z; the velocity components of the five
+//    planes z-2..z+2 (two-cell halo in x and y) sit in a shared-memory ring, so every value is read from HBM/L2 once per
+//    tile and all stencil reads are conflict-free 16-byte shared loads.  A thread owns four consecutive x cells of ONE
+//    component; every limited face flux is computed once (x faces inside the thread, y faces handed down through shared
+//    memory, z faces kept for the next plane).  k_cd_tile3 fills the ring with TMA boxes, k_cd_tile2 through registers
+//    with the periodic wrap applied while loading.  They write u = V + mu0 f (with the Heun average in the corrector)
+//    and never read mu1.
+//  * k_cd_band: mu1 is non-zero only within eps of the body surface; measure! leaves a compact list of those faces
+//    (wl_flow.cu) and this kernel adds sum_j mu1_ij (f_i[c+d_j]-f_i[c-d_j])/2 there, recomputing the six neighbouring
+//    r from global memory (flux / rhs_comp / f_at below).
 #include <cstdio>
 #include <cstdlib>
 #include "wl_internal.h"
@@ -174,27 +176,6 @@ __device__ __forceinline__ float4 cd_fetch(const Grid& g, const float* __restric
 }
 
 #define CD_ITEMS(ND) ((ND) * CD_R * CD_G)
-#define CD_STAGE(ND) ((CD_ITEMS(ND) + CD_NT - 1) / CD_NT)
-
-template <int ND>
-__device__ __forceinline__ void cd_load_regs(const Grid& g, const float* __restrict__ w, int bx, int by, int cz, float4 (&st)[CD_STAGE(ND)])
-{
-#pragma unroll
-    for (int k = 0; k < CD_STAGE(ND); ++k) {
-        const int item = threadIdx.x + k * CD_NT;
-        if (item < CD_ITEMS(ND)) st[k] = cd_fetch<ND>(g, w, item, bx, by, cz);
-    }
-}
-template <int ND>
-__device__ __forceinline__ void cd_store_regs(float* __restrict__ slot, const float4 (&st)[CD_STAGE(ND)])
-{
-#pragma unroll
-    for (int k = 0; k < CD_STAGE(ND); ++k) {
-        const int item = threadIdx.x + k * CD_NT;
-        if (item < CD_ITEMS(ND)) reinterpret_cast<float4*>(slot)[item] = st[k];   // slot layout = [comp][row][grp]
-    }
-}
-
 // limited flux through one face: wm | wc are the values either side, wup / wun the far-upwind
 // values for phi > 0 / phi <= 0, fbp / fbn the boundary fallbacks of R-H
 __device__ __forceinline__ float face_flux(float phi, float wup, float wm, float wc, float wun, bool fbp, bool fbn, float nu)
@@ -206,221 +187,13 @@ __device__ __forceinline__ float face_flux(float phi, float wup, float wm, float
     return phi * psi - nu * (wc - wm);
 }
 
-// read-only view of the shared ring for one thread: p[comp][dz + 2] = plane z+dz of component comp
-struct CdView {
-    const float* p[3][CD_NP];
-    int tx, ty;
-};
-// group tx+1+dg of shared row ty+2+dy: the thread's own four cells are dg = 0
-__device__ __forceinline__ void v4(const CdView& v, int comp, int dz, int dy, int dg, float* o)
-{
-    const float4 t = reinterpret_cast<const float4*>(v.p[comp][dz + 2])[(v.ty + 2 + dy) * CD_G + v.tx + 1 + dg];
-    o[0] = t.x; o[1] = t.y; o[2] = t.z; o[3] = t.w;
-}
-// one value: col counts from the thread's first cell (-1 = x-1, 4 = x+4)
-__device__ __forceinline__ float v1(const CdView& v, int comp, int dz, int dy, int col)
-{
-    return v.p[comp][dz + 2][(v.ty + 2 + dy) * CD_W + 4 * (v.tx + 1) + col];
-}
-
-// r_I at the thread's four cells (gx..gx+3, gy, gz) from the shared planes; a[] returns the own row
-// of w_I (cells gx-4 .. gx+7)
-template <int ND, int I>
-__device__ __forceinline__ void cd_rhs(const FlowP& P, const CdView& v, int gx, int gy, int gz, float (&a)[12], float (&r)[4])
-{
-    const Grid& g = P.g;
-    const float nu = P.nu;
-    v4(v, I, 0, 0, -1, a); v4(v, I, 0, 0, 0, a + 4); v4(v, I, 0, 0, 1, a + 8);
-    // ---- x faces gx .. gx+4 (shared between the thread's cells)
-    {
-        float px[5];
-        if (I == 0) {
-#pragma unroll
-            for (int f = 0; f < 5; ++f) px[f] = 0.5f * (a[3 + f] + a[4 + f]);
-        } else {
-            float lo[5], hi[5];
-            v4(v, 0, 0, 0, 0, hi); hi[4] = v1(v, 0, 0, 0, 4);
-            if (I == 1) { v4(v, 0, 0, -1, 0, lo); lo[4] = v1(v, 0, 0, -1, 4); }
-            else        { v4(v, 0, -1, 0, 0, lo); lo[4] = v1(v, 0, -1, 0, 4); }
-#pragma unroll
-            for (int f = 0; f < 5; ++f) px[f] = 0.5f * (lo[f] + hi[f]);
-        }
-        float F[5];
-#pragma unroll
-        for (int f = 0; f < 5; ++f) {
-            const int cj = gx + f;
-            const bool fbp = !g.per[0] && cj <= 1 + (I == 0 ? 1 : 0), fbn = !g.per[0] && cj >= g.n[0] + 1;
-            F[f] = face_flux(px[f], a[2 + f], a[3 + f], a[4 + f], a[5 + f], fbp, fbn, nu);
-        }
-#pragma unroll
-        for (int k = 0; k < 4; ++k) r[k] = F[k] - F[k + 1];
-    }
-    // ---- y faces: lower (gy) and upper (gy+1)
-    {
-        float m2[4], m1[4], p1[4], p2[4], pl[4], pu[4];
-        v4(v, I, 0, -2, 0, m2); v4(v, I, 0, -1, 0, m1); v4(v, I, 0, 1, 0, p1); v4(v, I, 0, 2, 0, p2);
-        if (I == 1) {
-#pragma unroll
-            for (int k = 0; k < 4; ++k) { pl[k] = 0.5f * (m1[k] + a[4 + k]); pu[k] = 0.5f * (a[4 + k] + p1[k]); }
-        } else if (I == 0) {
-            float b0[4], b1[4];
-            v4(v, 1, 0, 0, 0, b0); v4(v, 1, 0, 1, 0, b1);
-            const float e0 = v1(v, 1, 0, 0, -1), e1 = v1(v, 1, 0, 1, -1);
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                pl[k] = 0.5f * ((k == 0 ? e0 : b0[k == 0 ? 0 : k - 1]) + b0[k]);
-                pu[k] = 0.5f * ((k == 0 ? e1 : b1[k == 0 ? 0 : k - 1]) + b1[k]);
-            }
-        } else {
-            float b0[4], b1[4], c0[4], c1[4];
-            v4(v, 1, -1, 0, 0, b0); v4(v, 1, 0, 0, 0, c0); v4(v, 1, -1, 1, 0, b1); v4(v, 1, 0, 1, 0, c1);
-#pragma unroll
-            for (int k = 0; k < 4; ++k) { pl[k] = 0.5f * (b0[k] + c0[k]); pu[k] = 0.5f * (b1[k] + c1[k]); }
-        }
-        const bool np = !g.per[1];
-        const bool lfbp = np && gy <= 1 + (I == 1 ? 1 : 0), lfbn = np && gy >= g.n[1] + 1;
-        const bool ufbp = np && gy + 1 <= 1 + (I == 1 ? 1 : 0), ufbn = np && gy + 1 >= g.n[1] + 1;
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-            r[k] += face_flux(pl[k], m2[k], m1[k], a[4 + k], p1[k], lfbp, lfbn, nu)
-                  - face_flux(pu[k], m1[k], a[4 + k], p1[k], p2[k], ufbp, ufbn, nu);
-    }
-    // ---- z faces
-    if (ND == 3) {
-        float m2[4], m1[4], p1[4], p2[4], pl[4], pu[4];
-        v4(v, I, -2, 0, 0, m2); v4(v, I, -1, 0, 0, m1); v4(v, I, 1, 0, 0, p1); v4(v, I, 2, 0, 0, p2);
-        if (I == 2) {
-#pragma unroll
-            for (int k = 0; k < 4; ++k) { pl[k] = 0.5f * (m1[k] + a[4 + k]); pu[k] = 0.5f * (a[4 + k] + p1[k]); }
-        } else if (I == 0) {
-            float b0[4], b1[4];
-            v4(v, 2, 0, 0, 0, b0); v4(v, 2, 1, 0, 0, b1);
-            const float e0 = v1(v, 2, 0, 0, -1), e1 = v1(v, 2, 1, 0, -1);
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                pl[k] = 0.5f * ((k == 0 ? e0 : b0[k == 0 ? 0 : k - 1]) + b0[k]);
-                pu[k] = 0.5f * ((k == 0 ? e1 : b1[k == 0 ? 0 : k - 1]) + b1[k]);
-            }
-        } else {
-            float b0[4], b1[4], c0[4], c1[4];
-            v4(v, 2, 0, -1, 0, b0); v4(v, 2, 0, 0, 0, c0); v4(v, 2, 1, -1, 0, b1); v4(v, 2, 1, 0, 0, c1);
-#pragma unroll
-            for (int k = 0; k < 4; ++k) { pl[k] = 0.5f * (b0[k] + c0[k]); pu[k] = 0.5f * (b1[k] + c1[k]); }
-        }
-        const bool np = !g.per[2];
-        const bool lfbp = np && gz <= 1 + (I == 2 ? 1 : 0), lfbn = np && gz >= g.n[2] + 1;
-        const bool ufbp = np && gz + 1 <= 1 + (I == 2 ? 1 : 0), ufbn = np && gz + 1 >= g.n[2] + 1;
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-            r[k] += face_flux(pl[k], m2[k], m1[k], a[4 + k], p1[k], lfbp, lfbn, nu)
-                  - face_flux(pu[k], m1[k], a[4 + k], p1[k], p2[k], ufbp, ufbn, nu);
-    }
-}
-
 struct CdT { int ntx, nty, ntz, ntiles, zc; };
 
-template <int ND, int I>
-__device__ __forceinline__ void cd_comp(const FlowP& P, const CdView& v, int gx, int gy, int gz, int nv,
-                                        const float* __restrict__ u0, const float* __restrict__ mu0, const float* __restrict__ w,
-                                        float* __restrict__ out, float dt, float Vi, int corrector)
-{
-    const Grid& g = P.g;
-    float a[12], r[4], o[4], uu[4], mm[4];
-    cd_rhs<ND, I>(P, v, gx, gy, gz, a, r);
-    if (nv <= 0) return;
-    const int64_t id = gidx(g, gx, gy, gz);
-    unpack4(ld4(mu0 + I * g.nalloc, id), mm);
-    if (corrector) unpack4(ld4(u0 + I * g.nalloc, id), uu);
-    else {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) uu[k] = a[4 + k];
-    }
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        const float f = uu[k] + dt * r[k] - Vi;
-        const float B = Vi + mm[k] * f;
-        o[k] = corrector ? 0.5f * (a[4 + k] + B) : B;
-    }
-    st4(out + I * g.nalloc, id, o, nv);
-    // the corrector leaves the convective-exit plane at the predictor's value (R-N); the output is
-    // another buffer, so carry the plane over
-    if (I == 0 && corrector && P.exit_bc) {
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-            if (gx + k == g.n[0]) out[id + k + 1] = a[5 + k];
-    }
-}
-
-template <int ND>
-__global__ void __launch_bounds__(CD_NT, 2) k_cd_tile(FlowP P, CdT T, const float* __restrict__ w, const float* __restrict__ u0,
-                                                      const float* __restrict__ mu0, float* __restrict__ out,
-                                                      const DevScal* __restrict__ ds, int corrector)
-{
-    extern __shared__ float4 cd_smem[];
-    float* ring = reinterpret_cast<float*>(cd_smem);
-    const Grid& g = P.g;
-    const float dt = ds->dt;
-    const float V0 = ds->vel[0], V1 = ds->vel[1], V2 = ds->vel[2];
-    constexpr int NP = ND == 3 ? CD_NP : 1;
-    constexpr int SLOT = ND * CD_PLANE;            // floats per ring slot
-    CdView v;
-    v.tx = threadIdx.x & (CD_TX - 1);
-    v.ty = threadIdx.x / CD_TX;
-    for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
-        const int tix = tile % T.ntx, rem = tile / T.ntx;
-        const int tiy = rem % T.nty, tiz = rem / T.nty;
-        const int bx = 1 + 4 * CD_TX * tix, by = 1 + CD_TY * tiy;
-        const int z0 = ND == 3 ? 1 + T.zc * tiz : 0;
-        const int z1 = ND == 3 ? min(z0 + T.zc - 1, g.n[2]) : 0;
-        const int gx = bx + 4 * v.tx, gy = by + v.ty;
-        int nv = g.n[0] - gx + 1;
-        nv = nv > 4 ? 4 : nv;
-        if (gy > g.n[1]) nv = 0;
-        __syncthreads();                           // the previous tile's reads are done
-        {
-            float4 st[CD_STAGE(ND)];
-#pragma unroll 1
-            for (int d = 0; d < NP; ++d) {
-                const int cz = ND == 3 ? src_coord(z0 - 2 + d, g.n[2], g.per[2]) : 0;
-                cd_load_regs<ND>(g, w, bx, by, cz, st);
-                cd_store_regs<ND>(ring + d * SLOT, st);
-            }
-        }
-        __syncthreads();
-        int s0 = 0;                                // ring slot of plane z-2
-#pragma unroll 1
-        for (int z = z0; z <= z1; ++z) {
-            float4 st[CD_STAGE(ND)];
-            const bool more = ND == 3 && z < z1;
-            if (more) cd_load_regs<ND>(g, w, bx, by, src_coord(z + 3, g.n[2], g.per[2]), st);
-#pragma unroll
-            for (int d = 0; d < NP; ++d) {
-                int s = s0 + d;
-                if (s >= NP) s -= NP;
-#pragma unroll
-                for (int c = 0; c < ND; ++c) v.p[c][ND == 3 ? d : 2] = ring + s * SLOT + c * CD_PLANE;
-            }
-            cd_comp<ND, 0>(P, v, gx, gy, z, nv, u0, mu0, w, out, dt, V0, corrector);
-            cd_comp<ND, 1>(P, v, gx, gy, z, nv, u0, mu0, w, out, dt, V1, corrector);
-            if (ND == 3) cd_comp<ND, 2>(P, v, gx, gy, z, nv, u0, mu0, w, out, dt, V2, corrector);
-            if (more) {
-                __syncthreads();
-                cd_store_regs<ND>(ring + s0 * SLOT, st);
-                s0 = s0 + 1 == NP ? 0 : s0 + 1;
-                __syncthreads();
-            }
-        }
-    }
-}
-
 // ====================================================================== the tile kernel, one component per thread
-// k_cd_tile computes every limited face flux of a cell for each of its two neighbours: 63 per thread and plane,
-// 128 registers, two 256-thread blocks per SM -- instruction-bound at 15 % of the DRAM rate (profiles/r1b).
-// k_cd_tile2 works from the same five-plane ring but (a) a thread owns four cells of ONE component (blocks of
-// 256 x ND threads; warps are component-uniform), (b) the flux through a y face is computed once, by the thread above
-// it, and handed down through shared memory, (c) the flux through the upper z face is kept for the next plane of the
-// march, where it is the lower one.  41 instead of 63 fluxes per four cells of the three components, identical
-// values (a flux is the same expression of the same operands whichever thread evaluates it).
+// (a) a thread owns four cells of ONE component (blocks of 256 x ND threads; warps are component-uniform), (b) the flux
+// through a y face is computed once, by the thread above it, and handed down through shared memory, (c) the flux through
+// the upper z face is kept for the next plane of the march, where it is the lower one.  41 instead of 63 fluxes per four
+// cells of the three components (a flux is the same expression of the same operands whichever thread evaluates it).
 // view of the ring for one thread: b[dz + 2] points at the thread's own float4 of component 0 in plane z+dz, so that
 // every stencil read is one shared load at a compile-time offset (component, row and group offsets are immediates)
 struct CdView2 { const float* b[CD_NP]; };
@@ -885,21 +658,14 @@ void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out,
 {
     FlowP P = wl_flowp(s);
     CdT T = cd_tiling(s, P.g);
-    const size_t smem = sizeof(float) * (size_t)(s->nd == 3 ? CD_NP : 1) * s->nd * CD_PLANE;
-    if (!(s->cd_attr_set & 1)) {
-        cudaFuncSetAttribute(k_cd_tile<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * CD_NP * 3 * CD_PLANE));
-        cudaFuncSetAttribute(k_cd_tile<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * 2 * CD_PLANE));
-        s->cd_attr_set |= 1;
-    }
-    const int cd2 = s->cd_kernel >= 2;        // 1: k_cd_tile (three components per thread), 2: k_cd_tile2, 3: k_cd_tile3 where it applies
-    const size_t smem2 = smem + sizeof(float4) * (size_t)s->nd * CD_NT;
-    if (cd2 && !(s->cd_attr_set & 2)) {
+    const size_t smem2 = sizeof(float) * (size_t)(s->nd == 3 ? CD_NP : 1) * s->nd * CD_PLANE + sizeof(float4) * (size_t)s->nd * CD_NT;
+    if (!(s->cd_attr_set & 2)) {
         cudaFuncSetAttribute(k_cd_tile2<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * CD_NP * 3 * CD_PLANE + sizeof(float4) * 3 * CD_NT));
         cudaFuncSetAttribute(k_cd_tile2<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * 2 * CD_PLANE + sizeof(float4) * 2 * CD_NT));
         s->cd_attr_set |= 2;
     }
     // the TMA-fed kernel where a box never has to wrap in x or y
-    int cd3 = s->cd_kernel >= 3 && s->nd == 3 && !P.g.per[0] && !P.g.per[1];
+    int cd3 = s->tma_cd && s->nd == 3 && !P.g.per[0] && !P.g.per[1];
     CUtensorMap tm[3];
     if (cd3)
         for (int c = 0; c < 3 && cd3; ++c) cd3 = wl_tensor_map3(&tm[c], w + c * P.g.nalloc, P.g, CD_W, CD_R);
@@ -913,13 +679,8 @@ void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out,
         k_cd_tile3<<<T.ntiles, CD2_NT(3), smem3, s->st>>>(P, T, u0, s->mu0, out, s->ds, corrector, tm[0], tm[1], tm[2]);
     } else {
         ProfScope ps(s, WLK_CONVDIFF);
-        if (cd2) {
-            if (s->nd == 3) k_cd_tile2<3><<<T.ntiles, CD2_NT(3), smem2, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
-            else            k_cd_tile2<2><<<T.ntiles, CD2_NT(2), smem2, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
-        } else {
-            if (s->nd == 3) k_cd_tile<3><<<T.ntiles, CD_NT, smem, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
-            else            k_cd_tile<2><<<T.ntiles, CD_NT, smem, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
-        }
+        if (s->nd == 3) k_cd_tile2<3><<<T.ntiles, CD2_NT(3), smem2, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
+        else            k_cd_tile2<2><<<T.ntiles, CD2_NT(2), smem2, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
     }
     if (s->cfg.body.kind != WL_BODY_NONE) {
         ProfScope ps(s, WLK_CONVDIFF_BAND);

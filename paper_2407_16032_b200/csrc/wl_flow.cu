@@ -5,25 +5,46 @@
 #include "wl_internal.h"
 
 // ------------------------------------------------------------------ time / body state
-// One thread.  Sets the running dt (host value, or the device-resident CFL result) and the
-// time at which the body is measured (host value, or t + dt: reading R-R), then the
-// translation map c(t) = c0 + amp sin(2 pi f t + phase) e_heave and V = dc/dt.
-// Modes: t_mode / dt_mode = 1: take the host value; 0: device-resident (t + dt / last CFL result);
-// -1: keep the current value.
+// One thread.  Sets the running dt (host value, or the device-resident CFL result) and the time at which the body is
+// placed (host value, or t_step + dt: reading R-R), then the translation map, sinusoidal in every direction,
+//     c_d(t) = c0_d + amp_d sin(2 pi f_d t + phase_d),  V = dc/dt
+// Modes: see wl_internal.h.  The simulation time t_step moves only with wl_step (t_mode 2 and 0), so a wl_measure or
+// wl_pressure_force at some other time cannot shift the trajectory of a device-resident run.
+__device__ __forceinline__ void body_place(const wl_body& b, double t, double (&c)[3], float (&v)[3])
+{
+    const double two_pi = 6.283185307179586476925286766559;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        c[k] = (double)b.centre[k];
+        v[k] = 0.f;
+        if (b.motion == WL_MOTION_SIN) {
+            const double ph = two_pi * (double)b.freq[k] * t + (double)b.phase[k];
+            c[k] += (double)b.amp[k] * sin(ph);
+            v[k] = (float)((double)b.amp[k] * two_pi * (double)b.freq[k] * cos(ph));
+        }
+    }
+}
+
 __global__ void k_set_time(DevScal* ds, wl_body b, double t_host, float dt_host, int t_mode, int dt_mode)
 {
     if (dt_mode == 1) ds->dt = dt_host; else if (dt_mode == 0) ds->dt = ds->dt_next;
-    double t = t_mode == 1 ? t_host : (t_mode == 0 ? ds->t + (double)ds->dt : ds->t);
+    double t = ds->t;
+    if (t_mode == 2) { t = t_host; ds->t_step = t; }
+    else if (t_mode == 1) t = t_host;
+    else if (t_mode == 0) { t = ds->t_step + (double)ds->dt; ds->t_step = t; }
     ds->t = t;
-    double c[3] = { (double)b.centre[0], (double)b.centre[1], (double)b.centre[2] };
-    float v[3] = { 0.f, 0.f, 0.f };
-    if (b.motion == WL_MOTION_HEAVE_SIN) {
-        const double two_pi = 6.283185307179586476925286766559;
-        double ph = two_pi * (double)b.freq * t + (double)b.phase;
-        c[b.heave_dir] += (double)b.amp * sin(ph);
-        v[b.heave_dir] = (float)((double)b.amp * two_pi * (double)b.freq * cos(ph));
-    }
+    double c[3]; float v[3];
+    body_place(b, t, c, v);
     for (int k = 0; k < 3; ++k) { ds->centre[k] = c[k]; ds->vel[k] = v[k]; }
+}
+
+// body centre for the pressure-force integral: at the host time t, or (t = NaN) where measure! last placed the body
+__global__ void k_force_time(DevScal* ds, wl_body b, double t_host)
+{
+    double c[3]; float v[3];
+    if (t_host == t_host) body_place(b, t_host, c, v);
+    else for (int k = 0; k < 3; ++k) c[k] = ds->centre[k];
+    for (int k = 0; k < 3; ++k) ds->centre_f[k] = c[k];
 }
 
 // ------------------------------------------------------------------ measure!
@@ -234,7 +255,7 @@ __global__ void __launch_bounds__(WL_VB) k_cfl(Grid g, VT vt, const float* __res
 template <int ND>
 __global__ void __launch_bounds__(512) k_force(Grid g, Tiling T, BodyP b, const float* __restrict__ p, DevScal* ds, RedBuf rb)
 {
-    double ctr[3] = { ds->centre[0], ds->centre[1], ds->centre[2] };
+    double ctr[3] = { ds->centre_f[0], ds->centre_f[1], ds->centre_f[2] };
     double v[3] = { 0.0, 0.0, 0.0 };
     if (b.kind != WLB_NONE) {
         for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
@@ -257,13 +278,63 @@ __global__ void __launch_bounds__(512) k_force(Grid g, Tiling T, BodyP b, const 
     }
 }
 
+// ------------------------------------------------------------------ kinetic energy and enstrophy (Fig. 4; R-E2)
+//   KE = 1/2 sum_c sum_i u_i[c]^2 ;  Z = 1/2 sum_c |w[c]|^2,  w_k[c] = (u_j[c] - u_j[c-d_i]) - (u_i[c] - u_i[c-d_j]), (i,j,k) cyclic:
+// the circulation around the cell edge along k through the lower corner of cell c.  One thread per four x cells, marching
+// along z with the plane below in registers; ghosts are BC-filled, so the -1 neighbours are plain loads.  fp64 partials,
+// fixed tree.
+template <int ND>
+__global__ void __launch_bounds__(WL_VB) k_energy(Grid g, VT vt, const float* __restrict__ u, DevScal* ds, RedBuf rb)
+{
+    double v[2] = { 0.0, 0.0 };
+    const float* ux = u; const float* uy = u + g.nalloc; const float* uz = u + 2 * g.nalloc;
+    for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
+        VPos p = vt_pos(g, vt, tile);
+        if (p.nv == 0) continue;
+        const int64_t rc = (int64_t)WL_OFF + (int64_t)p.c1 * g.sy + p.c0;
+        float xl[4] = { 0.f, 0.f, 0.f, 0.f }, yl[4] = { 0.f, 0.f, 0.f, 0.f };      // u_x, u_y of the plane below
+        if (ND == 3) { unpack4(ld4(ux, rc + (int64_t)(p.z0 - 1) * g.sz), xl); unpack4(ld4(uy, rc + (int64_t)(p.z0 - 1) * g.sz), yl); }
+        for (int z = p.z0; z <= p.z1; ++z) {
+            const int64_t i = rc + (int64_t)z * g.sz;
+            float a[4], b[4], c[4] = { 0.f, 0.f, 0.f, 0.f }, am[4], cm[4] = { 0.f, 0.f, 0.f, 0.f };
+            unpack4(ld4(ux, i), a); unpack4(ld4(uy, i), b);
+            unpack4(ld4(ux, i - g.sy), am);                      // u_x one row down
+            const float bl = ld1(uy, i - 1);                     // u_y one cell to the left of the group
+            float cl = 0.f;
+            if (ND == 3) { unpack4(ld4(uz, i), c); unpack4(ld4(uz, i - g.sy), cm); cl = ld1(uz, i - 1); }
+            float ke = 0.f, en = 0.f;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                if (k >= p.nv) break;
+                ke += a[k] * a[k] + b[k] * b[k] + c[k] * c[k];
+                const float wz = (b[k] - (k == 0 ? bl : b[k - 1])) - (a[k] - am[k]);
+                en += wz * wz;
+                if (ND == 3) {
+                    const float wx = (c[k] - cm[k]) - (b[k] - yl[k]);
+                    const float wy = (a[k] - xl[k]) - (c[k] - (k == 0 ? cl : c[k - 1]));
+                    en += wx * wx + wy * wy;
+                }
+            }
+            v[0] += 0.5 * (double)ke; v[1] += 0.5 * (double)en;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { xl[k] = a[k]; yl[k] = b[k]; }
+        }
+    }
+    if (grid_reduce<2, OpSum>(v, rb)) {
+        if (threadIdx.x == 0) { ds->energy[0] = v[0]; ds->energy[1] = v[1]; }
+    }
+}
+
 // ------------------------------------------------------------------ initial conditions
-// Taylor-Green vortex (Eq. 3-5; R-W), staggered sampling, whole padded array.
+// Taylor-Green vortex (Eq. 3-5; R-W), staggered sampling, whole padded array.  One period per periodic
+// direction; HALF a period in a non-periodic one, whose slip walls (U = 0) are then symmetry planes of the vortex: the
+// half-domain of P:118.
 template <int ND>
 __global__ void __launch_bounds__(512) k_init_tgv(Grid g, Tiling T, float* u, float* p, int sign)
 {
     const double two_pi = 6.283185307179586476925286766559;
-    const double k0 = two_pi / g.n[0], k1 = two_pi / g.n[1], k2 = ND == 3 ? two_pi / g.n[2] : 0.0;
+    const double k0 = (g.per[0] ? 1.0 : 0.5) * two_pi / g.n[0], k1 = (g.per[1] ? 1.0 : 0.5) * two_pi / g.n[1];
+    const double k2 = ND == 3 ? (g.per[2] ? 1.0 : 0.5) * two_pi / g.n[2] : 0.0;
     for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
         int c0, c1, c2;
         if (!tile_cell(T, tile, c0, c1, c2)) continue;
@@ -327,11 +398,12 @@ void wl_k_measure(wl_sim* s)
     if (s->measured && b.kind != WL_BODY_NONE) {
         int o[3] = { 0, 0, 0 }, e[3] = { g.S[0], g.S[1], g.S[2] };
         for (int d = 0; d < s->nd; ++d) {
-            float ext = b.R;                                          // sphere / circle
+            float ext = b.R;                                          // sphere / circle / cylinder cross-section
             if (b.kind == WL_BODY_TORUS) ext = d == b.axis ? b.r : b.R + b.r;
             float reach = ext + s->cfg.eps + 2.0f;                    // the face positions are half a cell off the centres
-            if (b.motion == WL_MOTION_HEAVE_SIN && d == b.heave_dir) reach += fabsf(b.amp);
+            if (b.motion == WL_MOTION_SIN) reach += fabsf(b.amp[d]);
             int lo = (int)floorf(b.centre[d] - reach), hi = (int)ceilf(b.centre[d] + reach) + 1;      // padded coordinates c = x + 1/2
+            if (b.kind == WL_BODY_CYLINDER && d == b.axis) { lo = 0; hi = g.n[d] + 1; }               // it spans the direction
             if (lo < 0) lo = 0;
             if (hi > g.n[d] + 1) hi = g.n[d] + 1;
             if (g.per[d] && (lo <= 2 || hi >= g.n[d] - 1)) { lo = 0; hi = g.n[d] + 1; }   // ghosts mirror the far side: whole direction
@@ -392,10 +464,23 @@ void wl_k_cfl(wl_sim* s, const float* u)
     else            k_cfl<2><<<wl_vgrid(s, vt), WL_VB, 0, s->st>>>(g, vt, u, s->ds, s->rb, c.nu, c.cfl_c, c.cfl_cnu, c.dt_max);
 }
 
-void wl_k_force(wl_sim* s)
+void wl_k_energy(wl_sim* s, const float* u)
+{
+    const Grid& g = s->lev[0].g;
+    const VT& vt = s->lev[0].vt;
+    ProfScope ps(s, WLK_ENERGY);
+    if (s->nd == 3) k_energy<3><<<wl_vgrid(s, vt), WL_VB, 0, s->st>>>(g, vt, u, s->ds, s->rb);
+    else            k_energy<2><<<wl_vgrid(s, vt), WL_VB, 0, s->st>>>(g, vt, u, s->ds, s->rb);
+}
+
+void wl_k_force(wl_sim* s, double t)
 {
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_interior(s, g);
+    {
+        ProfScope ps(s, WLK_SET_TIME);
+        k_force_time<<<1, 1, 0, s->st>>>(s->ds, s->cfg.body, t);
+    }
     ProfScope ps(s, WLK_FORCE);
     if (s->nd == 3) k_force<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->p, s->ds, s->rb);
     else            k_force<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->p, s->ds, s->rb);

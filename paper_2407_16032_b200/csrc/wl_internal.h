@@ -11,7 +11,7 @@
 enum WlKern {
     WLK_SET_TIME, WLK_MEASURE, WLK_POISSON_UPDATE, WLK_CONVDIFF, WLK_BC, WLK_EXIT_BC, WLK_RESIDUAL,
     WLK_RESTRICT, WLK_PROLONG, WLK_PCG_INIT, WLK_PCG_MATVEC, WLK_PCG_UPDATE, WLK_PCG_DIR,
-    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_CONVDIFF_BAND, WLK_COARSE, WLK_PCG_FUSED, WLK_COUNT
+    WLK_GRADIENT, WLK_CFL, WLK_FORCE, WLK_RESMAX, WLK_MISC, WLK_CONVDIFF_BAND, WLK_COARSE, WLK_PCG_FUSED, WLK_ENERGY, WLK_SMALL, WLK_COUNT
 };
 struct ProfRec { cudaEvent_t a, b; int cls; };
 
@@ -43,7 +43,7 @@ struct LevDev {
 };
 
 // a chain of coarse-level passes run by one k_coarse launch
-enum { COP_RESTRICT = 0, COP_SMOOTH = 1, COP_PROLONG = 2, COP_NOP = 3, COP_BAR = 4 };   // RESTRICT: level -> level+1; PROLONG: level+1 -> level
+enum { COP_RESTRICT = 0, COP_SMOOTH = 1, COP_PROLONG = 2 };   // RESTRICT: level -> level+1; PROLONG: level+1 -> level
 struct CoarseOp { int kind, level, iters; };
 struct CoarseProg { int n; CoarseOp op[3 * WL_MAXLEV]; };
 
@@ -66,21 +66,22 @@ struct wl_sim {
     double* pk_part;         // per-block partial sums of k_coarse
     int pk_level;            // levels >= pk_level run inside k_coarse (nlev: none)
     int pk_blocks;           // co-resident grid of k_coarse (0: not yet queried)
-    int tiny_on;             // tiny levels run in the one-cluster kernel k_tiny (env WL_TINY=0 switches it off)
+    int tiny_on;             // tiny levels run in the one-cluster kernel k_tiny (wl_tuning.no_block_levels switches it off)
     int measured;            // measure! has run over the whole grid once: later calls only visit the box the body can reach
-    int cd_kernel;           // conv_diff kernel: 3 (default) k_cd_tile3 (TMA) where it applies, 2 k_cd_tile2, 1 k_cd_tile (env WL_CD)
-    int bulk_A;              // k_pcg_A_fast takes its operand planes as TMA boxes where it can (env WL_BULK=0 switches it off)
+    int tma_cd;              // conv_diff from the TMA-fed ring (k_cd_tile3) where it applies (wl_tuning.no_tma_cd switches it off)
+    int bulk_A;              // k_pcg_A_fast takes its operand planes as TMA boxes where it can (wl_tuning.no_bulk switches it off)
     int mbox_lo[3], mbox_hi[3]; // padded coordinates of the box the last measure! rewrote (the whole array the first time)
     int fused0;              // level 0 takes the one-sweep PCG form; its r2, q2 live in a dead velocity buffer (wl_api.cu solver_scratch)
-    int fused;               // PCG smoother in its one-sweep form where the level allows (env WL_FUSED=0 switches it off)
-    int fast_A;              // uniform tiles of PCG pass A go through k_pcg_A_fast (env WL_FAST_A=0 switches it off)
+    int fused;               // PCG smoother in its one-sweep form where the level allows (wl_tuning.no_fused switches it off)
+    int fast_A;              // uniform tiles of PCG pass A go through k_pcg_A_fast (wl_tuning.no_fast_a switches it off)
     BodyP body;
     cudaStream_t st;
     int launches;
     int vcycles[2];
     double res[2];
     int solve_slot;
-    int noconv;
+    int noconv;              // a tolerance-mode solve hit max_vcycles since the last wl_cfl (which reports and clears it)
+    int noconv_total;        // ... since create (wl_stats)
     int primed;              // device-resident t and dt are valid (adaptive wl_step)
     int sm_count;
     char err[256];
@@ -127,12 +128,13 @@ Tiling wl_tiles_padded(const wl_sim* s, const Grid& g);
 FlowP wl_flowp(const wl_sim* s);
 
 // wl_flow.cu
-void wl_k_set_time(wl_sim* s, double t, float dt, int t_mode, int dt_mode);   // 1 host, 0 device, -1 keep
+void wl_k_set_time(wl_sim* s, double t, float dt, int t_mode, int dt_mode);   // t: 2 host value, also the simulation time; 1 host value, body only; 0 device (t_step + dt); -1 keep.  dt: 1 host, 0 device, -1 keep
 void wl_k_measure(wl_sim* s);
 void wl_k_bc(wl_sim* s, float* u);
 void wl_k_exit_bc(wl_sim* s, float* u, const float* u0);
 void wl_k_cfl(wl_sim* s, const float* u);
-void wl_k_force(wl_sim* s);
+void wl_k_force(wl_sim* s, double t);                // t = NaN: the body where measure! last placed it
+void wl_k_energy(wl_sim* s, const float* u);
 void wl_k_init_tgv(wl_sim* s, int sign);
 void wl_k_fill(wl_sim* s, float* a, int64_t n, float v);
 void wl_k_fill_u(wl_sim* s, float* u);

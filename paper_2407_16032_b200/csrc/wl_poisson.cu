@@ -774,13 +774,6 @@ __global__ void __launch_bounds__(WL_VB) k_rsum(Grid g, VT vt, const int* __rest
 // products are summed from per-block partials in a fixed order by every block (bit-identical in all
 // blocks, so every block takes the same branches of the PCG guards).  The passes are the same tile
 // functions the fine-level kernels use.
-__device__ __forceinline__ unsigned long long globaltimer_ns()
-{
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-
 struct PkCtx {
     double* part;        // [2][WL_MAX_PARTIALS][WL_PK_SLOT] per-block partial sums (one slot per block), alternating by reduction
     int phase;
@@ -911,19 +904,13 @@ __device__ __forceinline__ void coarse_body(const LevDev* levs, const CoarseProg
     int rsum_level = -1;
     for (int o = 0; o < prog.n; ++o) {
         const CoarseOp op = prog.op[o];
-        if (blockIdx.x == 0 && threadIdx.x == 0) ds->pk_t[o] = globaltimer_ns();
         __syncthreads();
         if (threadIdx.x == 0) {     // level descriptors of this pass into shared memory (typed copies: no punning)
             la = levs[op.level];
             lb = levs[op.level + (op.kind == COP_SMOOTH ? 0 : 1)];
         }
         __syncthreads();
-        if (op.kind == COP_NOP) {                    // timing probes: one reduction / one bare grid barrier
-            double v[1] = { 1.0 };
-            pk_reduce<1>(c, v);
-        } else if (op.kind == COP_BAR) {
-            pk_barrier(c);
-        } else if (op.kind == COP_SMOOTH) {
+        if (op.kind == COP_SMOOTH) {
             PcgScal* sc = &ds->pcg[op.level];
             const double rs = rsum_level == op.level ? rsum : sc->rsum;
             pk_smooth<ND>(c, la, sc, op.iters, rs);
@@ -954,7 +941,6 @@ __device__ __forceinline__ void coarse_body(const LevDev* levs, const CoarseProg
             if (blockIdx.x == 0 && threadIdx.x == 0) ds->pcg[op.level].rsum = v[0];
         }
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) ds->pk_t[prog.n] = globaltimer_ns();
 }
 
 template <int ND>
@@ -1042,7 +1028,7 @@ static void coarse_launch_one(wl_sim* s, const CoarseProg& prog, int tiny)
         if (s->nd == 3) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_coarse<3>, WL_VB, 0);
         else            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_coarse<2>, WL_VB, 0);
         if (per_sm > WL_PK_MINB) per_sm = WL_PK_MINB;
-        if (const char* e = getenv("WL_PK_BPS")) { int v = atoi(e); if (v >= 1 && v < per_sm) per_sm = v; }
+        if (s->cfg.tune.pk_blocks_per_sm > 0 && s->cfg.tune.pk_blocks_per_sm < per_sm) per_sm = s->cfg.tune.pk_blocks_per_sm;
         if (per_sm < 1) per_sm = 1;
         int nb = per_sm * s->sm_count;
         if (nb > WL_MAX_PARTIALS) nb = WL_MAX_PARTIALS;

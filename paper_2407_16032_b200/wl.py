@@ -15,16 +15,16 @@ import numpy as np
 
 from . import build as _build
 
-BODY_NONE, BODY_SPHERE, BODY_TORUS = 0, 1, 2
-MOTION_STATIC, MOTION_HEAVE_SIN = 0, 1
+BODY_NONE, BODY_SPHERE, BODY_TORUS, BODY_CYLINDER = 0, 1, 2, 3
+MOTION_STATIC, MOTION_SIN = 0, 1
 WL_OK, WL_EINVAL, WL_ENOMEM, WL_ECUDA, WL_ENOCONV = 0, -1, -2, -3, -4
 
 EXPORTS = [
     "wl_workspace_bytes", "wl_sim_create", "wl_sim_destroy", "wl_set_fields", "wl_init_tgv", "wl_measure",
-    "wl_mom_step", "wl_cfl", "wl_pressure_force", "wl_get_fields", "wl_step",
+    "wl_mom_step", "wl_cfl", "wl_pressure_force", "wl_energy", "wl_get_fields", "wl_step",
     "wl_dbg_conv_diff_bdim", "wl_dbg_save_u0", "wl_dbg_bc", "wl_dbg_exit_bc", "wl_dbg_project",
     "wl_dbg_residual", "wl_dbg_apply_gradient", "wl_dbg_restrict", "wl_dbg_prolong", "wl_dbg_smooth", "wl_dbg_vcycle",
-    "wl_dbg_coarse_prog", "wl_dbg_coarse_times", "wl_dbg_pcg_scalars",
+    "wl_dbg_coarse_prog", "wl_dbg_pcg_scalars",
     "wl_dbg_get", "wl_dbg_set", "wl_dbg_get_padded", "wl_level_dims", "wl_last_error", "wl_stats", "wl_abi_version",
     "wl_prof_enable", "wl_prof_read",
 ]
@@ -32,8 +32,8 @@ EXPORTS = [
 
 class Body(C.Structure):
     _fields_ = [("kind", C.c_int), ("centre", C.c_float * 3), ("R", C.c_float), ("r", C.c_float),
-                ("axis", C.c_int), ("motion", C.c_int), ("heave_dir", C.c_int),
-                ("amp", C.c_float), ("freq", C.c_float), ("phase", C.c_float)]
+                ("axis", C.c_int), ("motion", C.c_int),
+                ("amp", C.c_float * 3), ("freq", C.c_float * 3), ("phase", C.c_float * 3)]
 
 
 class MG(C.Structure):
@@ -41,16 +41,21 @@ class MG(C.Structure):
                 ("fixed_vcycles", C.c_int), ("tol", C.c_float)]
 
 
+class Tuning(C.Structure):
+    _fields_ = [("no_fused", C.c_int), ("no_fast_a", C.c_int), ("no_bulk", C.c_int), ("no_block_levels", C.c_int),
+                ("no_tma_cd", C.c_int), ("zc", C.c_int), ("pk_max_cells", C.c_longlong), ("pk_blocks_per_sm", C.c_int)]
+
+
 class Config(C.Structure):
     _fields_ = [("ndim", C.c_int), ("dims", C.c_int * 3), ("L", C.c_float), ("U", C.c_float * 3),
                 ("nu", C.c_float), ("periodic", C.c_int * 3), ("exit_bc", C.c_int), ("eps", C.c_float),
                 ("dt0", C.c_float), ("dt_max", C.c_float), ("cfl_c", C.c_float), ("cfl_cnu", C.c_float),
-                ("body", Body), ("mg", MG)]
+                ("body", Body), ("mg", MG), ("tune", Tuning)]
 
 
 class Stats(C.Structure):
     _fields_ = [("vcycles", C.c_int * 2), ("res", C.c_double * 2), ("nlevels", C.c_int),
-                ("kernel_launches", C.c_int), ("nan_flag", C.c_int)]
+                ("kernel_launches", C.c_int), ("nan_flag", C.c_int), ("noconv", C.c_int)]
 
 
 _lib = None
@@ -81,6 +86,7 @@ def load(build_if_missing: bool = True):
     L.wl_step.argtypes = [vp, C.c_double, C.c_float, ip]
     L.wl_cfl.argtypes = [vp, fp]
     L.wl_pressure_force.argtypes = [vp, C.c_double, fp]
+    L.wl_energy.argtypes = [vp, C.POINTER(C.c_double)]
     L.wl_get_fields.argtypes = [vp, vp, vp, vp, ip]
     L.wl_dbg_conv_diff_bdim.argtypes = [vp, C.c_float, ip]
     L.wl_dbg_save_u0.argtypes = [vp]
@@ -93,7 +99,6 @@ def load(build_if_missing: bool = True):
         getattr(L, name).argtypes = [vp, ip]
     L.wl_dbg_smooth.argtypes = [vp, ip, ip]
     L.wl_dbg_coarse_prog.argtypes = [vp, ip, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
-    L.wl_dbg_coarse_times.argtypes = [vp, C.POINTER(C.c_ulonglong), ip]
     L.wl_dbg_pcg_scalars.argtypes = [vp, ip, C.POINTER(C.c_double)]
     L.wl_dbg_get.argtypes = [vp, C.c_char_p, ip, vp, C.c_size_t]
     L.wl_dbg_set.argtypes = [vp, C.c_char_p, ip, vp, C.c_size_t]
@@ -123,13 +128,24 @@ def make_config(cfg: dict) -> Config:
         setattr(c, k, float(cfg[k]))
     c.exit_bc = int(cfg["exit_bc"])
     c.body.kind = int(cfg["body_kind"])
-    for k in ("R", "r", "amp", "freq", "phase"):
+    for k in ("R", "r"):
         setattr(c.body, k, float(cfg[k]))
-    for k in ("axis", "motion", "heave_dir"):
+    for k in ("axis", "motion"):
         setattr(c.body, k, int(cfg[k]))
+    # sinusoidal translation: three-vectors amp3 / freq3 / phase3, or the scalars amp / freq / phase along heave_dir
+    if cfg.get("amp3") is not None:
+        for d in range(3):
+            c.body.amp[d], c.body.freq[d], c.body.phase[d] = float(cfg["amp3"][d]), float(cfg["freq3"][d]), float(cfg["phase3"][d])
+    else:
+        d = int(cfg["heave_dir"])
+        c.body.amp[d], c.body.freq[d], c.body.phase[d] = float(cfg["amp"]), float(cfg["freq"]), float(cfg["phase"])
     for k in ("max_levels", "smooth_iters", "max_vcycles", "fixed_vcycles"):
         setattr(c.mg, k, int(cfg[k]))
     c.mg.tol = float(cfg["tol"])
+    for k, v in (cfg.get("tune") or {}).items():          # wl_tuning: implementation switches, all zero by default
+        if not hasattr(c.tune, k):
+            raise KeyError(f"wl_tuning has no field {k}")
+        setattr(c.tune, k, int(v))
     return c
 
 
@@ -234,6 +250,12 @@ class Sim:
         self._chk(self._L.wl_pressure_force(self._h, float(t), F))
         return np.array([F[0], F[1], F[2]], dtype=np.float64)
 
+    def energy(self) -> np.ndarray:
+        """(kinetic energy, enstrophy) of the current velocity, grid units"""
+        out = (C.c_double * 2)()
+        self._chk(self._L.wl_energy(self._h, out))
+        return np.array([out[0], out[1]])
+
     def get_fields(self, u=None, p=None, mu0=None):
         """Copy into the given buffers (torch cuda / torch cpu / numpy); all on the same side."""
         ptrs, devs = [], []
@@ -256,7 +278,7 @@ class Sim:
         st = Stats()
         self._chk(self._L.wl_stats(self._h, C.byref(st)))
         return {"vcycles": [st.vcycles[0], st.vcycles[1]], "res": [st.res[0], st.res[1]],
-                "nlevels": st.nlevels, "kernel_launches": st.kernel_launches, "nan_flag": st.nan_flag}
+                "nlevels": st.nlevels, "kernel_launches": st.kernel_launches, "nan_flag": st.nan_flag, "noconv": st.noconv}
 
     def prof_enable(self, enable: bool = True):
         self._chk(self._L.wl_prof_enable(self._h, int(enable)))
@@ -337,11 +359,6 @@ class Sim:
         A = C.c_int * n
         self._chk(self._L.wl_dbg_coarse_prog(self._h, n, A(*[int(o[0]) for o in ops]), A(*[int(o[1]) for o in ops]),
                                              A(*[int(o[2]) for o in ops])))
-
-    def dbg_coarse_times(self, n):
-        out = (C.c_ulonglong * n)()
-        self._chk(self._L.wl_dbg_coarse_times(self._h, out, n))
-        return [int(v) for v in out]
 
     def dbg_pcg_scalars(self, level):
         out = (C.c_double * 8)()

@@ -26,15 +26,17 @@ def test_library_exports_every_declared_symbol():
     for n in names:
         assert hasattr(L, n), f"libwl.so does not export {n}"
     assert sorted(wl.EXPORTS) == names
-    assert L.wl_abi_version() == 1
+    assert L.wl_abi_version() == 2
 
 
 def test_config_struct_layout_matches_header():
     """The ctypes mirror must have the C layout: all members are 4-byte scalars, no padding."""
     from paper_2407_16032_b200 import wl
-    assert C.sizeof(wl.Body) == 4 * 12
+    assert C.sizeof(wl.Body) == 4 * (1 + 3 + 2 + 1 + 1 + 9)
     assert C.sizeof(wl.MG) == 4 * 5
-    assert C.sizeof(wl.Config) == 4 * (1 + 3 + 1 + 3 + 1 + 3 + 1 + 1 + 4) + C.sizeof(wl.Body) + C.sizeof(wl.MG)
+    assert C.sizeof(wl.Tuning) == 4 * 6 + 8 + 8              # six ints, one long long (8-aligned), one int + tail padding
+    head = 4 * (1 + 3 + 1 + 3 + 1 + 3 + 1 + 1 + 4) + C.sizeof(wl.Body) + C.sizeof(wl.MG)
+    assert wl.Config.tune.offset == (head + 7) // 8 * 8 and C.sizeof(wl.Config) == wl.Config.tune.offset + C.sizeof(wl.Tuning)
 
 
 def test_workspace_bytes_is_pure_and_sane():
@@ -66,6 +68,12 @@ def test_create_rejects_bad_arguments_without_gpu():
     c.ndim = 5
     assert L.wl_sim_create(C.byref(c), None, 0, None, C.byref(h)) == wl.WL_EINVAL
     assert L.wl_mom_step(None, 0.1) == wl.WL_EINVAL
+
+
+def test_library_reads_no_environment_variable():
+    """include/wl.h promises 'no global state': the implementation switches travel in wl_config.tune."""
+    for path in (ROOT / "paper_2407_16032_b200" / "csrc").iterdir():
+        assert "getenv" not in path.read_text(), path
 
 
 def test_product_never_imports_the_oracle():

@@ -48,6 +48,12 @@ def _body(kind, dims, moving=False):
         return {}
     if kind == "sphere":
         kw = dict(body_kind=wi.BODY_SPHERE, centre=c, R=0.22 * min(dims))
+    elif kind == "cylinder":         # spanning z, two-degree-of-freedom motion when moving
+        kw = dict(body_kind=wi.BODY_CYLINDER, centre=c, R=0.2 * min(dims[:2]), axis=2)
+        if moving:
+            kw.update(motion=wi.MOTION_SIN, amp3=(0.05 * dims[0], 0.12 * dims[1], 0.0), freq3=(0.026, 0.013, 0.0),
+                      phase3=(0.5, 0.0, 0.0))
+            return kw
     else:
         kw = dict(body_kind=wi.BODY_TORUS, centre=c, R=0.25 * min(dims[1:]), r=0.09 * min(dims[1:]), axis=0)
     if moving:
@@ -70,6 +76,9 @@ CASES = [
     ((160, 48, 40), (0, 0, 0), 1, "sphere", False),
     ((136, 40, 24), (1, 1, 1), 0, "torus", False),
     ((272, 36), (0, 1), 1, "sphere", False),
+    # circular cylinder spanning the periodic z direction, static and with the 2-DOF motion
+    ((48, 32, 16), (0, 0, 1), 1, "cylinder", False),
+    ((160, 48, 24), (0, 0, 1), 1, "cylinder", True),
 ]
 
 
@@ -288,12 +297,35 @@ def test_cfl_and_force(case):
 
 
 def test_init_tgv_matches_oracle_and_is_divergence_free():
-    for dims in ((64, 64), (32, 32, 32)):
-        cfg = wi.tgv2d(64) if len(dims) == 2 else wi.tgv3d(32)
+    for cfg in (wi.tgv2d(64), wi.tgv3d(32), wi.tgv3d_half(32), wi.tgv3d_half(40, periodic=(0, 1, 0))):
         o, g = _sims(cfg)
         o.init_tgv(1); g.init_tgv(1)
         assert np.abs(g.dbg_get("u", padded=True) - O(o, "u", padded=True)).max() <= 1e-7
         o.close(); g.close()
+
+
+@pytest.mark.parametrize("case", CASES, ids=_ids)
+def test_energy_and_enstrophy(case):
+    """wl_energy (reading R-E2) against the oracle's sums on the seeded field: fp32 products,
+    fp64 accumulation."""
+    cfg = _cfg(case)
+    o, g = _sims(cfg)
+    _load_state(o, g, case[0], p_too=False)
+    eo, eg = o.energy(), g.energy()
+    assert eg[0] == pytest.approx(eo[0], rel=TOL) and eg[1] == pytest.approx(eo[1], rel=TOL)
+    o.close(); g.close()
+
+
+def test_energy_closed_forms_on_the_device():
+    """the discrete Taylor-Green sums (tests/test_oracle_energy.py derives them): KE = N^3/8, Z = 3/2 sin^2(kappa/2) N^3"""
+    from paper_2407_16032_b200 import wl
+    for cfg, kappa in ((wi.tgv3d(64), 2 * np.pi / 64), (wi.tgv3d_half(64), np.pi / 64)):
+        g = wl.Sim(cfg)
+        g.init_tgv(1)
+        ke, ens = g.energy()
+        assert ke == pytest.approx(64 ** 3 / 8.0, rel=2e-6)
+        assert ens == pytest.approx(1.5 * np.sin(kappa / 2) ** 2 * 64 ** 3, rel=2e-5)
+        g.close()
 
 
 def test_error_paths():

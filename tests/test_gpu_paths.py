@@ -1,9 +1,8 @@
 """GPU parity of the alternative kernel paths of the projection: the shared-memory PCG pass A
 (`k_pcg_A_fast`) against the register-marching one, the persistent coarse-level kernels (`k_coarse`, cooperative;
 `k_tiny`, one thread-block cluster) against stand-alone launches, a fused chain of coarse passes against the same
-passes launched one by one -- each against the fp64 oracle, and against one another.  The environment switches
-(WL_FAST_A, WL_TINY, WL_PK_MAX_CELLS, WL_BULK, WL_CD) are read when a simulation is created."""
-import os
+passes launched one by one -- each against the fp64 oracle, and against one another.  The paths are chosen by the `tune` entry of the config
+(wl_tuning in include/wl.h), copied into the handle when a simulation is created."""
 
 import numpy as np
 import pytest
@@ -15,30 +14,17 @@ pytestmark = pytest.mark.gpu
 
 SWITCHES = [
     {},                                     # default: fast pass A, k_coarse for levels <= 1 M cells, k_tiny below
-    {"WL_FUSED": "0"},                      # two-pass PCG iterations (wl_pcgfast.cu pass A + k_pcg_B) instead of the one-sweep form
-    {"WL_FAST_A": "0"},                     # register-marching pass A everywhere
-    {"WL_TINY": "0"},                       # tiny levels inside the cooperative kernel
-    {"WL_PK_MAX_CELLS": "0"},               # every level by stand-alone kernels
-    {"WL_BULK": "0"},                       # pass A copies its planes with per-thread cp.async instead of TMA boxes
-    {"WL_CD": "2"},                         # conv_diff from the register-staged ring (k_cd_tile2) instead of the TMA-fed one
-    {"WL_CD": "1"},                         # conv_diff with three components per thread (k_cd_tile)
+    {"no_fused": 1},                        # two-pass PCG iterations (wl_pcgfast.cu pass A + k_pcg_B) instead of the one-sweep form
+    {"no_fast_a": 1},                       # register-marching pass A everywhere
+    {"no_block_levels": 1},                 # small levels inside the cooperative kernel
+    {"pk_max_cells": -1},                   # every level by stand-alone kernels
+    {"no_bulk": 1},                         # pass A copies its planes with per-thread cp.async instead of TMA boxes
+    {"no_tma_cd": 1},                       # conv_diff from the register-staged ring (k_cd_tile2) instead of the TMA-fed one
 ]
 
 
-class _env:
-    def __init__(self, kv):
-        self.kv = kv
-
-    def __enter__(self):
-        self.old = {k: os.environ.get(k) for k in self.kv}
-        os.environ.update(self.kv)
-
-    def __exit__(self, *a):
-        for k, v in self.old.items():
-            if v is None:
-                os.environ.pop(k, None)
-            else:
-                os.environ[k] = v
+def _tuned(cfg, sw):
+    return dict(cfg, tune=dict(sw))
 
 
 # the last two take the TMA path of pass A (rows of whole 128-cell tiles, no wrap in x and y)
@@ -63,8 +49,7 @@ def test_every_path_matches_the_oracle_and_the_others(case):
     uo = O(o, "u")
     outs = []
     for sw in SWITCHES:
-        with _env(sw):
-            g = wl.Sim(cfg)
+        g = wl.Sim(_tuned(cfg, sw))
         g.set_fields(u=np.ascontiguousarray(u0, dtype=np.float32))
         for _ in range(3):
             g.mom_step(dt)
@@ -126,18 +111,17 @@ def test_fused_coarse_chain_equals_single_passes(case):
         assert np.array_equal(xa, xb) and np.array_equal(ra, rb)       # same kernels, same order: bit-identical
 
 
-@pytest.mark.parametrize("kernel", ["1", "2", "3"])
+@pytest.mark.parametrize("kernel", ["tile2", "tile3"])
 @pytest.mark.parametrize("case", [c for c in WIDE if not c[1][0] and not c[1][1]] + [CASES[1], CASES[4]], ids=_ids)
 def test_conv_diff_kernels_agree(case, kernel):
-    """conv_diff + BDIM + Heun through each of the three tile kernels (k_cd_tile, k_cd_tile2, the TMA-fed k_cd_tile3 where x and
+    """conv_diff + BDIM + Heun through each of the two tile kernels (k_cd_tile2, the TMA-fed k_cd_tile3 where x and
     y do not wrap): predictor and corrector against the oracle at the per-kernel tolerance."""
     from paper_2407_16032_b200 import wl
     cfg = _cfg(case)
     for corrector in (0, 1):
         o, _g = _sims(cfg)
         _g.close()
-        with _env({"WL_CD": kernel}):
-            g = wl.Sim(cfg)
+        g = wl.Sim(_tuned(cfg, {"no_tma_cd": 1} if kernel == "tile2" else {}))
         _load_state(o, g, case[0], seed=wi.SEED, p_too=False)
         o.arr("u0")[...] = o.arr("u"); g.dbg_save_u0()
         if corrector:
@@ -176,7 +160,7 @@ def test_smoother_removes_residual_mean_on_the_gpu():
 
 
 # levels the one-sweep smoother (wl_pcgfused.cu) takes: 3-D, at least 68 cells along x, no wrap in x and y; with
-# WL_PK_MAX_CELLS=0 level 1 of the second case (128 x 16 x 12) is a stand-alone level too and takes it as well
+# pk_max_cells = -1 level 1 of the second case (128 x 16 x 12) is a stand-alone level too and takes it as well
 FUSED = [((128, 40, 24), (0, 0, 0), 1, "sphere", False), ((256, 32, 24), (0, 0, 1), 1, "torus", False),
          ((160, 44, 24), (0, 0, 0), 1, "sphere", False)]          # the last: rows of 1.25 tiles, 5.5 tiles along y
 
@@ -213,11 +197,10 @@ def test_one_sweep_smoother_matches_the_oracle_and_the_two_pass_form(case, iters
     from paper_2407_16032_b200 import wl
     cfg = _cfg(case)
     outs = []
-    for sw in ({"WL_PK_MAX_CELLS": "0"}, {"WL_PK_MAX_CELLS": "0", "WL_FUSED": "0"}):
+    for sw in ({"pk_max_cells": -1}, {"pk_max_cells": -1, "no_fused": 1}):
         o, g0 = _sims(cfg)
         g0.close()
-        with _env(sw):
-            g = wl.Sim(cfg)
+        g = wl.Sim(_tuned(cfg, sw))
         res = []
         for l in _fused_levels(case):
             r0 = _smoother_inputs(o, g, l)
@@ -243,8 +226,7 @@ def test_one_sweep_smoother_stops_like_the_oracle(case):
     cfg = _cfg(case)
     o, g0 = _sims(cfg)
     g0.close()
-    with _env({"WL_PK_MAX_CELLS": "0"}):
-        g = wl.Sim(cfg)
+    g = wl.Sim(_tuned(cfg, {"pk_max_cells": -1}))
     for l in _fused_levels(case):
         r0 = _smoother_inputs(o, g, l)
         iD = O(o, "iD", l)[0]

@@ -61,6 +61,10 @@ SCALED = [
     # the most sensitive case: the method itself amplifies a 1e-7 perturbation of u to 1.3e-4 in these ten steps (oracle
     # against oracle); the CUDA path stays at 2.8e-5 because k_measure evaluates the SDF in fp64
     ("C5_heaving_96x64x64", lambda: wi.baseline_config(4, scale=4), dict()),
+    # the 2-DOF cylinder in a periodic-z box at 1/8 of the benchmark size (D = 8 cells, 72 x 48 x 16)
+    ("N1_cylinder_2dof_72x48x16", lambda: wi.cylinder_2dof(8), dict()),
+    # the half-domain Taylor-Green vortex between symmetry planes, 32^3
+    ("N3_tgv_half_32", lambda: wi.tgv3d_half(32), dict(tgv=True)),
     ("2D_cylinder_exit_96x64", lambda: wi.make(ndim=2, dims=(96, 64), exit_bc=1, nu=0.05, body_kind=wi.BODY_SPHERE,
                                                centre=(24.3, 32.2), R=6.0), dict()),
 ]
@@ -121,6 +125,35 @@ def test_force_after_100_steps():
     o.close(); g.close()
 
 
+def test_energy_history_half_domain_tgv():
+    """kinetic energy and enstrophy of the half-domain vortex (PAPER.md:169-173 plots them) over 20
+    adaptive steps at 32^3 against the oracle's sums."""
+    cfg = wi.tgv3d_half(32)
+    o, g = _sims(cfg)
+    o.init_tgv(1); g.init_tgv(1)
+    dt = o.cfl()
+    for _ in range(20):
+        o.mom_step(dt); g.mom_step(dt)
+        dt = o.cfl()
+        eo, eg = o.energy(), g.energy()
+        assert eg[0] == pytest.approx(eo[0], rel=2e-5) and eg[1] == pytest.approx(eo[1], rel=1e-4)
+    assert eo[0] < 32 ** 3 / 8.0                       # it decays
+    o.close(); g.close()
+
+
+def test_force_and_power_two_dof_cylinder_50_steps():
+    """force on the 2-DOF cylinder (PAPER.md:181 reports force and power coefficients) over 50 steps at
+    1/8 scale, both components in the plane of motion, and the power F.V."""
+    cfg = wi.cylinder_2dof(8)
+    o, g = _sims(cfg)
+    t, F = _run(o, g, cfg, 50, force=True)
+    Fo, Fg = np.array([a for a, b in F]), np.array([b for a, b in F])
+    sc = np.abs(Fo[5:]).max()
+    assert np.abs(Fg[5:] - Fo[5:]).max() <= 1e-3 * sc
+    assert np.abs(Fg[:, 2]).max() <= 1e-3 * sc         # nothing along the span
+    o.close(); g.close()
+
+
 def test_force_moving_body_50_steps():
     cfg = wi.baseline_config(4, scale=4)
     o, g = _sims(cfg)
@@ -178,6 +211,13 @@ def test_adaptive_device_resident_step_matches_manual_loop():
     assert np.abs(ua - ub).max() <= 2e-6
     Fa, Fb = a.pressure_force(t), b.pressure_force()
     assert np.abs(Fa - Fb).max() <= 1e-4 * np.abs(Fa).max()
+    # a force or a measure at some OTHER time must not shift the device-resident trajectory (the simulation time is
+    # advanced by wl_step alone)
+    b.pressure_force(t + 17.0)
+    for k in range(2):
+        a.measure(t + dt); a.mom_step(dt); t += dt; dt = a.cfl()
+        b.step(0.0, cfg["dt0"], adaptive=True)
+    assert np.abs(a.fields()[0] - b.fields()[0]).max() <= 2e-6
     a.close(); b.close()
 
 
