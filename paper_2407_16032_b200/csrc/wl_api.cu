@@ -331,6 +331,7 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     s->fast_A = !cfg->tune.no_fast_a;
     s->fused = !cfg->tune.no_fused;
     s->tiny_on = !cfg->tune.no_block_levels;
+    s->small_cmax = -1;
     s->bulk_A = !cfg->tune.no_bulk;
     s->tma_cd = !cfg->tune.no_tma_cd;
     s->body.kind = cfg->body.kind; s->body.axis = cfg->body.axis;
@@ -533,7 +534,8 @@ extern "C" int wl_level_dims(const wl_sim* s, int level, int dims_out[3])
 // ---- per-kernel-class timing (CUDA events on the handle's stream)
 static const char* const kern_names[WLK_COUNT] = {
     "set_time", "measure", "poisson_update", "conv_diff_bdim", "bc", "exit_bc", "residual", "restrict", "prolong",
-    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc", "conv_diff_band", "vcycle", "pcg_fused"
+    "pcg_init", "pcg_matvec", "pcg_update", "pcg_dir", "apply_gradient", "cfl", "force", "resmax", "misc", "conv_diff_band", "vcycle", "pcg_fused",
+    "energy", "small_levels"
 };
 
 extern "C" int wl_prof_enable(wl_sim* s, int enable)

@@ -58,7 +58,7 @@ struct wl_sim {
     float* mu1;              // nd*nd comps
     long long* band_list;    // faces with mu1 != 0, written by measure!: (array offset << 2) | component
     int band_cap;            // capacity of band_list (entries)
-    int cd_attr_set;         // dynamic shared-memory attributes set: bits 1, 2, 4 conv_diff kernels, 8 cluster size of k_tiny, 16 k_pcg_fused
+    int cd_attr_set;         // dynamic shared-memory attributes set: bits 2, 4 conv_diff kernels, 16 k_pcg_fused
     DevScal* ds;             // device-resident scalars
     DevScal* hs;             // pinned host mirror for read-back
     RedBuf rb;
@@ -66,7 +66,8 @@ struct wl_sim {
     double* pk_part;         // per-block partial sums of k_coarse
     int pk_level;            // levels >= pk_level run inside k_coarse (nlev: none)
     int pk_blocks;           // co-resident grid of k_coarse (0: not yet queried)
-    int tiny_on;             // tiny levels run in the one-cluster kernel k_tiny (wl_tuning.no_block_levels switches it off)
+    int tiny_on;             // small levels run on chip in the one-cluster kernel k_small (wl_tuning.no_block_levels switches it off)
+    int small_cmax;          // largest cluster k_small can be launched with on this device (-1: not yet queried, 0: none)
     int measured;            // measure! has run over the whole grid once: later calls only visit the box the body can reach
     int tma_cd;              // conv_diff from the TMA-fed ring (k_cd_tile3) where it applies (wl_tuning.no_tma_cd switches it off)
     int bulk_A;              // k_pcg_A_fast takes its operand planes as TMA boxes where it can (wl_tuning.no_bulk switches it off)
@@ -148,6 +149,10 @@ void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout)
 // wl_pcgfused.cu
 int wl_pcg_fused_shape(int nd, const Grid& g, const VT& vt);    // the one-sweep form can take a level of this shape
 int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r);              // 0: not taken (the caller runs the two-pass form)
+// wl_small.cu
+int wl_small_max_cluster(wl_sim* s);
+int wl_small_blocks(const Grid& g);
+int wl_k_small_prog(wl_sim* s, const CoarseProg& P, int C);
 // wl_poisson.cu
 void wl_k_poisson_update(wl_sim* s);                 // iD on level 0, coarse L and iD
 void wl_k_residual(wl_sim* s, const float* u, float w);   // pscale = w*dt; x = pscale*p; r = div u - A x

@@ -15,7 +15,7 @@
 // uniform modes TM_PLB / TM_PLI take them from the cell position / as constants.  On 3-D levels
 // pass A runs in wl_pcgfast.cu (shared memory, TMA); k_pcg_A here serves 2-D and ragged levels and
 // the persistent kernels.  Levels of at most 1 M cells run as chains of passes inside k_coarse
-// (cooperative launch, grid barrier between passes) and k_tiny (one thread-block cluster).
+// (cooperative launch, grid barrier between passes); the small ones on chip in k_small (wl_small.cu, one thread-block cluster).
 #include <cstdio>
 #include <cstdlib>
 #include "wl_internal.h"
@@ -28,12 +28,6 @@
 #endif
 #ifndef WL_B_MINB
 #define WL_B_MINB 4
-#endif
-#ifndef WL_TINY_CLUSTER
-#define WL_TINY_CLUSTER 16    // blocks of the k_tiny cluster (16 = the opt-in maximum on B200; 8 is the portable one)
-#endif
-#ifndef WL_TINY_TILES
-#define WL_TINY_TILES 16      // levels with at most this many tiles run in k_tiny
 #endif
 #ifndef WL_PK_SLOT
 #define WL_PK_SLOT 4      // doubles per block slot of the k_coarse partial sums: one 32-byte sector each
@@ -777,18 +771,12 @@ __global__ void __launch_bounds__(WL_VB) k_rsum(Grid g, VT vt, const int* __rest
 struct PkCtx {
     double* part;        // [2][WL_MAX_PARTIALS][WL_PK_SLOT] per-block partial sums (one slot per block), alternating by reduction
     int phase;
-    int cluster;         // 1: the launch is ONE thread-block cluster (k_tiny): hardware cluster barrier instead of the grid barrier
 };
 #define PK_NV 2
 
-// barrier over all blocks of the launch: every global write before it is visible to every block after it.
-// Cooperative launch: grid barrier (3.2 us on B200).  Single cluster: barrier.cluster arrive.release / wait.acquire
-// (~0.2 us), which orders global memory at cluster scope and invalidates L1 like the gpu-scope fence does.
-__device__ __forceinline__ void pk_barrier(PkCtx& c)
-{
-    if (c.cluster) cooperative_groups::this_cluster().sync();
-    else           cooperative_groups::this_grid().sync();
-}
+// barrier over all blocks of the cooperative launch: every global write before it is visible to every block after it
+// (3.2 us on B200)
+__device__ __forceinline__ void pk_barrier(PkCtx&) { cooperative_groups::this_grid().sync(); }
 
 // grid-wide sum of NV values; includes a grid barrier (all writes before it are visible after it)
 template <int NV>
@@ -895,11 +883,11 @@ __device__ __forceinline__ void pk_smooth(PkCtx& c, const LevDev& lv, PcgScal* s
 }
 
 template <int ND>
-__device__ __forceinline__ void coarse_body(const LevDev* levs, const CoarseProg& prog, DevScal* ds, double* part, int cluster)
+__device__ __forceinline__ void coarse_body(const LevDev* levs, const CoarseProg& prog, DevScal* ds, double* part)
 {
     __shared__ LevDev la, lb;
     PkCtx c;
-    c.part = part; c.phase = 0; c.cluster = cluster;
+    c.part = part; c.phase = 0;
     double rsum = 0.0;
     int rsum_level = -1;
     for (int o = 0; o < prog.n; ++o) {
@@ -946,15 +934,7 @@ __device__ __forceinline__ void coarse_body(const LevDev* levs, const CoarseProg
 template <int ND>
 __global__ void __launch_bounds__(WL_VB, WL_PK_MINB) k_coarse(const LevDev* levs, const __grid_constant__ CoarseProg prog, DevScal* ds, double* part)
 {
-    coarse_body<ND>(levs, prog, ds, part, 0);
-}
-
-// The same chain of passes for the TINY levels (at most a few tiles each): the grid is one thread-block cluster,
-// its blocks meet at the hardware cluster barrier.  A pass costs ~1 us instead of ~5 us under the grid barrier.
-template <int ND>
-__global__ void __launch_bounds__(WL_VB, WL_PK_MINB) k_tiny(const LevDev* levs, const __grid_constant__ CoarseProg prog, DevScal* ds, double* part)
-{
-    coarse_body<ND>(levs, prog, ds, part, 1);
+    coarse_body<ND>(levs, prog, ds, part);
 }
 
 // ================================================================== host launchers
@@ -1019,8 +999,8 @@ void wl_k_apply_gradient(wl_sim* s, float* u)
     VDISPATCH(s, WLK_GRADIENT, 0, lv.vt, k_apply_gradient<2>, k_apply_gradient<3>, lv.g, lv.vt, lv.plain, u, lv.L, lv.Lc, lv.x, s->p, s->ds);
 }
 
-// one k_coarse (cooperative, whole GPU) or k_tiny (one cluster) launch
-static void coarse_launch_one(wl_sim* s, const CoarseProg& prog, int tiny)
+// one k_coarse launch (cooperative, whole GPU)
+static void coarse_launch_one(wl_sim* s, const CoarseProg& prog)
 {
     if (prog.n <= 0) return;
     if (!s->pk_blocks) {
@@ -1038,44 +1018,42 @@ static void coarse_launch_one(wl_sim* s, const CoarseProg& prog, int tiny)
     const LevDev* levs = s->levdev;
     DevScal* ds = s->ds;
     double* part = s->pk_part;
-    if (tiny) {
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3(WL_TINY_CLUSTER); cfg.blockDim = dim3(WL_VB); cfg.dynamicSmemBytes = 0; cfg.stream = s->st;
-        cudaLaunchAttribute at[1];
-        at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = WL_TINY_CLUSTER; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-        cfg.attrs = at; cfg.numAttrs = 1;
-        if (WL_TINY_CLUSTER > 8 && !(s->cd_attr_set & 8)) {     // cluster sizes above 8 are opt-in
-            cudaFuncSetAttribute(k_tiny<3>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-            cudaFuncSetAttribute(k_tiny<2>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-            s->cd_attr_set |= 8;
-        }
-        if (s->nd == 3) cudaLaunchKernelEx(&cfg, k_tiny<3>, levs, prog, ds, part);
-        else            cudaLaunchKernelEx(&cfg, k_tiny<2>, levs, prog, ds, part);
-        return;
-    }
     void* args[] = { (void*)&levs, (void*)&prog, (void*)&ds, (void*)&part };
     if (s->nd == 3) cudaLaunchCooperativeKernel((const void*)k_coarse<3>, dim3(s->pk_blocks), dim3(WL_VB), args, 0, s->st);
     else            cudaLaunchCooperativeKernel((const void*)k_coarse<2>, dim3(s->pk_blocks), dim3(WL_VB), args, 0, s->st);
 }
 
-// a pass belongs to the tiny part when the level whose tiles it walks has at most WL_TINY_TILES tiles
-static int op_is_tiny(const wl_sim* s, const CoarseOp& op)
+// blocks of the k_small cluster a pass needs (the level whose cells it walks), or 0 when the pass belongs to k_coarse
+static int op_small_blocks(wl_sim* s, const CoarseOp& op)
 {
     if (!s->tiny_on) return 0;
+    if (s->small_cmax < 0) s->small_cmax = wl_small_max_cluster(s);      // once per handle
     const int walked = op.kind == COP_RESTRICT ? op.level + 1 : op.level;
-    return s->lev[walked].vt.ntiles <= WL_TINY_TILES;
+    const int C = wl_small_blocks(s->lev[walked].g);
+    return C <= s->small_cmax ? C : 0;
 }
 
-// runs a chain of coarse-level passes: consecutive passes of the same kind (whole-GPU / one cluster) share a launch
+// runs a chain of coarse-level passes: consecutive passes of the same kind (whole-GPU cooperative kernel / one on-chip cluster)
+// share a launch
 static void coarse_launch(wl_sim* s, const CoarseProg& prog)
 {
     int i = 0;
     while (i < prog.n) {
-        const int tiny = op_is_tiny(s, prog.op[i]);
+        const int small = op_small_blocks(s, prog.op[i]) > 0;
         CoarseProg P; P.n = 0;
-        while (i < prog.n && op_is_tiny(s, prog.op[i]) == tiny) P.op[P.n++] = prog.op[i++];
-        coarse_launch_one(s, P, tiny);
+        int C = 1;
+        while (i < prog.n && (op_small_blocks(s, prog.op[i]) > 0) == small) {
+            const int c = op_small_blocks(s, prog.op[i]);
+            if (c > C) C = c;
+            P.op[P.n++] = prog.op[i++];
+        }
+        if (small) {
+            if (!wl_k_small_prog(s, P, C)) {        // the cluster could not be launched after all: the cooperative kernel from now on
+                cudaGetLastError();
+                s->small_cmax = 0;
+                coarse_launch_one(s, P);
+            }
+        } else coarse_launch_one(s, P);
     }
 }
 
