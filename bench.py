@@ -1,26 +1,36 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the B200 mom_step hot path (libwl) on BASELINE.json's workloads.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C3|C4|C5] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--repeats R] [--workload C2|C3|C4|C5|N1|N3]
+                    [--impl reference] [--no-cpu] [--no-also] [--no-tol] [--stages]
 
-One "step" is one pass of the whole hot path of SURVEY.md 8(a) through the C ABI: wl_step =
-measure (moving body only) + mom_step (predictor + corrector, two multigrid projections) + the
-CFL reduction, on a synthetic BASELINE config.  The default workload is
-C4 (torus, 512x256x256 = 33.5 M cells): BASELINE.json quotes its metric ("ns per cell per time
-step (3D fp32) and achieved HBM GB/s") and its target (">= 60 % of HBM roofline on the >= 16 M-cell
-3D cases") on the large 3-D cases; C2 (configs[1], 2 M cells) fits in the 126 MB L2 and is reported
-under "also" together with C3 and C5.
+One "step" is one pass of the whole hot path of SURVEY.md 8(a) through the C ABI: wl_step = measure (moving body
+only) + mom_step (predictor + corrector, two multigrid projections) + the CFL reduction, on a synthetic BASELINE
+config.  The default workload is C4 (torus, 512x256x256 = 33.5 M cells): BASELINE.json quotes
+its metric ("ns per cell per time step (3D fp32) and achieved HBM GB/s") and its target (">= 60 % of HBM roofline on
+the >= 16 M-cell 3D cases") on the large 3-D cases; C2 (configs[1], 2 M cells) fits in the 126 MB L2 and is reported
+under "also" together with C3, C5 and the two SURVEY 8(f) workloads (N1: the paper's moving cylinder, 28.3 M cells;
+N3: its half-domain Taylor-Green vortex at 512^3, 134 M cells -- the shape of its 1.57 ns/DOF/step headline).
 
-Prints ONE JSON line (rank 0).  Keys: the driver contract (metric/value/unit/n_gpus/steps/warmup/
-ms_per_step/higher_is_better/scaling/vs_baseline/dtype/data/config/clocks/e2e/gpu_launches) plus
-"roofline" (dominant kernel class, CUDA-event timed inside this run) and "cpu_baseline" (the fp64
-oracle timed on this box's host cores on a bounded sample).
+Protocol: W warm-up steps, then R (default 5) timed blocks of K steps each, every block bracketed by
+barrier + synchronize and timed with CUDA events on the simulation's stream; `value` is the MEDIAN block (min and max
+are reported beside it).  Fixed two V-cycles per solve (the parity configuration); the tolerance mode (tol = 1e-4) is
+timed separately with its mean number of V-cycles per solve.  C3 is timed with the pressure force read every step, as
+BASELINE.json states it.
 
-Multi-GPU: the path does not shard (BASELINE.json north_star: one GPU, no collectives; DESIGN.md
-section 9) => "replicas only": every rank runs an independent simulation of the same workload;
-value = time / (cells x steps x ranks), time = max over ranks.
+Prints ONE JSON line (rank 0).  Keys: the driver contract (metric/value/unit/n_gpus/steps/warmup/ms_per_step/
+higher_is_better/scaling/vs_baseline/dtype/data/config/clocks/e2e/gpu_launches) plus "roofline" (dominant kernel
+class, CUDA-event timed inside this run; `traffic` = the ncu DRAM bytes of that kernel from this round's capture,
+profiles/r2_ncu_traffic_c4.csv), "cpu_baseline" (the fp64 oracle timed on this box's host cores on the workload
+itself), "tolerance_mode" and "also".
 
---impl reference times the oracle itself (oracle/wl_oracle.c, as it stands) on the host cores.
+Multi-GPU: the path does not shard (BASELINE.json north_star: one GPU, no collectives) =>
+"replicas only": every rank runs an independent simulation of the same workload; value = time / (cells x steps x
+ranks), time = max over ranks.
+
+--impl reference times the oracle itself (oracle/wl_oracle.c, as it stands) on the host cores, same workload.
+--stages launches every fine-level stage once inside a cudaProfilerStart/Stop range (for `ncu --profile-from-start
+off --set full`, see profiles/); it prints no JSON line and times nothing.
 """
 from __future__ import annotations
 
@@ -39,7 +49,22 @@ sys.path.insert(0, str(ROOT))
 
 import wl_inputs as wi  # noqa: E402
 
-WORKLOADS = {"C2": 1, "C3": 2, "C4": 3, "C5": 4}
+WORKLOADS = {"C2": 1, "C3": 2, "C4": 3, "C5": 4, "N1": 5, "N3": 6}
+NAMES = wi.WORKLOAD_NAMES + ["N1_cylinder_2dof_576x384x128", "N3_tgv_half_512"]
+
+
+def workload_config(k: int, scale: int = 1) -> dict:
+    """BASELINE.json configs[k] for k < 5; k = 5, 6: the SURVEY 8(f) NEXT-1 / NEXT-3 workloads."""
+    if k < 5:
+        return wi.baseline_config(k, scale=scale)
+    if k == 5:
+        return wi.cylinder_2dof(64 // scale)
+    return wi.tgv3d_half(512 // scale)
+
+
+def is_tgv(cfg) -> bool:
+    return cfg["body_kind"] == wi.BODY_NONE and tuple(cfg["U"][:3]) == (0.0, 0.0, 0.0)
+
 METRIC = "ns per cell per time step (3D fp32)"
 UNIT = "ns/cell/step"
 
@@ -62,11 +87,20 @@ ALG_BYTES = {
 }
 
 
-# DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the fine-level kernels on C4, from the
-# ncu --set full captures summarised in profiles/r1c_stages_c4_ncu.md and (pcg_fused) profiles/r1e_pcg_fused_c4_ncu.md
-# (bytes; other workloads: not captured)
-NCU_TRAFFIC_C4 = {"pcg_fused": 1200e6, "pcg_update": 793e6, "pcg_matvec": 593e6, "residual": 882e6, "prolong": 577e6,
-                  "apply_gradient": 1088e6, "cfl": 420e6, "restrict": 160e6, "conv_diff_bdim": 1430e6}
+TRAFFIC_FILE = ROOT / "profiles" / "r2_ncu_traffic_c4.csv"
+
+
+def ncu_traffic(workload: str) -> dict:
+    """{kernel class: DRAM bytes per launch (read + write)} from this round's `ncu --set full` capture of every
+    fine-level kernel (profiles/r2_ncu_traffic_c4.md names the command); C4 only, {} when the file is absent."""
+    if workload != "C4" or not TRAFFIC_FILE.exists():
+        return {}
+    out = {}
+    for line in TRAFFIC_FILE.read_text().splitlines()[1:]:
+        f = line.split(",")
+        if len(f) >= 4 and f[0]:
+            out[f[0]] = float(f[2]) + float(f[3])
+    return out
 
 
 def conv_alg_bytes(cfg) -> float:
@@ -124,50 +158,13 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------- oracle legs
-def oracle_sample(cfg_full: dict, k: int, budget_s: float = 15.0) -> dict:
-    """Time the fp64 oracle (as it stands) on a bounded sample of workload k: the same config at
-    half the linear size (same shape, same Reynolds number), 1 warm-up + n timed steps."""
-    from oracle import wl_oracle as wo
-    cfg = wi.baseline_config(k, scale=2)
-    n = ncells(cfg)
-    o = wo.OracleSim(cfg)
-    moving = cfg["motion"] != wi.MOTION_STATIC
-    if cfg["body_kind"] == wi.BODY_NONE:
-        o.init_tgv(1)
-        dt = o.cfl()
-    else:
-        dt = cfg["dt0"]
-    t = 0.0
-
-    def one(dt, t):
-        if moving:
-            o.measure(t + dt)
-        o.mom_step(dt)
-        return o.cfl(), t + dt
-
-    t0 = time.perf_counter()
-    dt, t = one(dt, t)
-    first = time.perf_counter() - t0
-    steps = max(1, min(20, int(budget_s / max(first, 1e-3)) - 1))
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        dt, t = one(dt, t)
-    el = time.perf_counter() - t0
-    threads = wo.num_threads()
-    o.close()
-    return {"value": el / steps / n * 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": f"{wi.WORKLOAD_NAMES[k]} at 1/2 linear scale ({'x'.join(map(str, cfg['dims']))} = {n} cells, "
-                      f"same shape and Re), fp64, 1 warm-up + {steps} timed steps, {el:.1f} s wall",
-            "steps": steps, "seconds": el, "cells": n}
-
-
 def _oracle_run(k: int, scale: int, nsteps: int, state=None):
     """Advance the oracle `nsteps` steps of workload k at 1/scale linear size; returns (seconds, state)."""
     from oracle import wl_oracle as wo
     if state is None:
-        cfg = wi.baseline_config(k, scale=scale)
+        cfg = workload_config(k, scale=scale)
         o = wo.OracleSim(cfg)
-        if cfg["body_kind"] == wi.BODY_NONE:
+        if is_tgv(cfg):
             o.init_tgv(1)
             dt = o.cfl()
         else:
@@ -185,48 +182,67 @@ def _oracle_run(k: int, scale: int, nsteps: int, state=None):
     return time.perf_counter() - t0, state
 
 
+def oracle_timed(k: int, warmup: int, steps: int, budget_s: float):
+    """The fp64 oracle, as it stands, on workload k ITSELF (full size): `warmup` + `steps` steps.  Only if the first step
+    shows that this would take longer than `budget_s` is the same config taken at 1/2 (then 1/4) linear size, and the
+    sample says so.  Returns (seconds of the timed steps, steps, scale, cfg of the sample, threads)."""
+    from oracle import wl_oracle as wo
+    scale = 1
+    while True:
+        el, state = _oracle_run(k, scale, 1)                  # first step of this size: the warm-up step
+        if el * (max(warmup, 1) + steps) <= budget_s or scale >= 4:
+            break
+        state["o"].close()
+        scale *= 2
+    if warmup > 1:
+        _oracle_run(k, scale, warmup - 1, state)
+    el, state = _oracle_run(k, scale, steps, state)
+    cfg = state["cfg"]
+    state["o"].close()
+    return el, steps, scale, cfg, wo.num_threads()
+
+
+def _sample_text(k, scale, cfg, warmup, steps, el):
+    dims = "x".join(map(str, cfg["dims"][: cfg["ndim"]]))
+    size = "the workload itself" if scale == 1 else f"the workload at 1/{scale} linear scale (same shape and Re)"
+    return (f"{NAMES[k]}: {size}, {dims} = {ncells(cfg)} cells, fp64 oracle as it stands, "
+            f"{max(warmup, 1)} warm-up + {steps} timed steps, {el:.1f} s wall")
+
+
+def oracle_sample(k: int) -> dict:
+    """cpu_baseline: 1 warm-up + 3 timed oracle steps of the workload itself (SURVEY 8(d) 'Oracle timed beside it')."""
+    el, steps, scale, cfg, threads = oracle_timed(k, 1, 3, budget_s=120.0)
+    n = ncells(cfg)
+    return {"value": el / steps / n * 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": _sample_text(k, scale, cfg, 1, steps, el), "same_config": scale == 1,
+            "steps": steps, "seconds": el, "cells": n}
+
+
 def run_reference(args) -> None:
-    """The reference arm of this tier is the oracle, as it stands, on the host cores.  A step is
-    one oracle time step on a bounded sample of the workload: the same config at 1/scale linear
-    size, scale chosen (2, 4 or 8) so that W + K steps end within a few minutes."""
+    """The reference arm of this tier is the oracle, as it stands, on the host cores, on the workload itself."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from oracle import wl_oracle as wo
     k = WORKLOADS[args.workload]
-    cfg = wi.baseline_config(k)
-    total = args.warmup + args.steps
-    scale, state, warm_done = 2, None, 0
-    while True:
-        el, state = _oracle_run(k, scale, 1)            # first step of this sample size (counts as warm-up)
-        warm_done = 1
-        if el * total <= 200.0 or scale >= 8:
-            break
-        state["o"].close()
-        scale, state = scale * 2, None
-    if args.warmup > warm_done:
-        _oracle_run(k, scale, args.warmup - warm_done, state)
-    el, state = _oracle_run(k, scale, args.steps, state)
-    scfg = state["cfg"]
+    cfg = workload_config(k)
+    el, steps, scale, scfg, threads = oracle_timed(k, args.warmup, args.steps, budget_s=400.0)
     n = ncells(scfg)
-    state["o"].close()
-    val = el / args.steps / n * 1e9
-    threads = wo.num_threads()
-    sample = (f"{wi.WORKLOAD_NAMES[k]} at 1/{scale} linear scale ({'x'.join(map(str, scfg['dims'][:scfg['ndim']]))} = {n} cells, "
-              f"same shape and Re), fp64 oracle, {max(args.warmup, warm_done)} warm-up + {args.steps} timed steps, {el:.1f} s wall")
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": el / args.steps * 1e3, "higher_is_better": False, "scaling": "weak",
+    val = el / steps / n * 1e9
+    sample = _sample_text(k, scale, scfg, args.warmup, steps, el)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": el / steps * 1e3, "higher_is_better": False, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": config_dict(cfg, args.workload, k, note="oracle timed on a bounded sample: " + sample),
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "config": config_dict(cfg, k, note="oracle timed on: " + sample),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                             "same_config": scale == 1},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
-def config_dict(cfg, wl_name, k, note=None) -> dict:
-    d = {"workload": wi.WORKLOAD_NAMES[k], "baseline_config_index": k, "dims": list(cfg["dims"][: cfg["ndim"]]),
-         "cells": ncells(cfg), "body": ["none", "sphere", "torus"][cfg["body_kind"]],
+def config_dict(cfg, k, note=None) -> dict:
+    d = {"workload": NAMES[k], "baseline_config_index": k if k < 5 else None, "dims": list(cfg["dims"][: cfg["ndim"]]),
+         "cells": ncells(cfg), "body": ["none", "sphere", "torus", "cylinder"][cfg["body_kind"]],
          "moving_body": bool(cfg["motion"]), "nu": cfg["nu"], "dt": "CFL-adaptive, device-resident",
          "mg": {"fixed_vcycles": cfg["fixed_vcycles"], "smooth_iters": cfg["smooth_iters"]},
          "l2": "working set (>= 3 GB for C4/C5) is far larger than the 126 MB L2; no flush needed between steps"}
@@ -239,7 +255,7 @@ def config_dict(cfg, wl_name, k, note=None) -> dict:
 def make_sim(cfg, device):
     from paper_2407_16032_b200 import wl
     s = wl.Sim(cfg, device=device)
-    if cfg["body_kind"] == wi.BODY_NONE and all(cfg["periodic"][: cfg["ndim"]]):
+    if is_tgv(cfg):
         s.init_tgv(1)
         dt0 = s.cfl()
     else:
@@ -247,11 +263,15 @@ def make_sim(cfg, device):
     return s, dt0
 
 
-def time_steps(torch, sim, dt0, steps, warmup, dist=None):
+def time_steps(torch, sim, dt0, steps, warmup, dist=None, force=False):
     """W untimed + K timed wl_step calls, device-timed with CUDA events on the sim's stream,
-    bracketed by barrier + synchronize; returns ms (this rank)."""
+    bracketed by barrier + synchronize; returns ms (this rank).  force: the pressure force is read every step."""
+    def one(first):
+        sim.step(dt0 if first else 0.0, dt0, adaptive=True)
+        if force:
+            sim.pressure_force()
     for i in range(warmup):
-        sim.step(dt0 if i == 0 else 0.0, dt0, adaptive=True)
+        one(i == 0)
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
@@ -259,7 +279,7 @@ def time_steps(torch, sim, dt0, steps, warmup, dist=None):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(sim._stream)
     for _ in range(steps):
-        sim.step(0.0, dt0, adaptive=True)
+        one(False)
     e1.record(sim._stream)
     torch.cuda.synchronize()
     if dist is not None:
@@ -272,6 +292,77 @@ def aggregate(ms_local: float, cells: int, steps: int, world: int, reduce_max=No
     ms = reduce_max(ms_local) if reduce_max is not None else ms_local
     total = cells * steps * world
     return {"ms": ms, "ns_per_cell_step": ms * 1e6 / total, "cells_steps_per_s": total / (ms * 1e-3)}
+
+
+def alg_bytes_table(cfg, prof) -> dict:
+    alg = dict(ALG_BYTES)
+    alg["conv_diff_bdim"] = conv_alg_bytes(cfg)
+    if "pcg_fused" in prof:                           # one-sweep form: every fine-level pcg_matvec launch is a first sweep, r -> e', q
+        alg["pcg_matvec"] = 4 * (1 + 2)
+        # ... and of the two last sweeps of a solve (fixed two V-cycles) the second leaves r alone (x, e' -> x): mean of 24 and 12
+        alg["pcg_update"] = (4 * (4 + 2) + 4 * (2 + 1)) / 2
+    return alg
+
+
+def profile_classes(torch, sim, cfg, dt0, steps, hbm_peak, ms_per_step, force=False):
+    """The same steps again with every launch bracketed by CUDA events: per-kernel-class times, and the step-level view:
+    algorithmic bytes of all fine-level passes per step against the step time."""
+    cells = ncells(cfg)
+    sim.prof_enable(True)
+    ms_prof = time_steps(torch, sim, dt0, steps, 0, None, force=force)
+    prof = sim.prof_read()
+    sim.prof_enable(False)
+    tot = sum(v[0] for v in prof.values())
+    alg = alg_bytes_table(cfg, prof)
+    kernels = {}
+    for name, (ms, n) in sorted(prof.items(), key=lambda kv: -kv[1][0]):
+        ent = {"ms_per_step": ms / steps, "launches_per_step": n / steps, "share": ms / tot}
+        if alg.get(name):                             # fine-level classes only (".coarse" = multigrid levels >= 1)
+            ent["alg_gbs"] = alg[name] * cells * n / (ms * 1e-3) / 1e9
+            ent["frac_of_measured_peak"] = ent["alg_gbs"] / hbm_peak
+        kernels[name] = ent
+    step_bytes = sum((alg.get(nm) or 0) * cells * n for nm, (ms, n) in prof.items() if not nm.endswith(".coarse")) / steps
+    gbs = step_bytes / (ms_per_step * 1e-3) / 1e9
+    coarse_ms = sum(ms for nm, (ms, n) in prof.items() if nm.endswith(".coarse")) / steps
+    step = {"alg_bytes_per_cell_per_step": step_bytes / cells, "achieved_gbs": gbs, "frac_of_measured_peak": gbs / hbm_peak,
+            "frac_of_nominal_8TBs": gbs / 8000.0, "levels_ge_1_ms_per_step": coarse_ms, "profiled_ms_per_step": ms_prof / steps}
+    return prof, alg, kernels, step
+
+
+def run_stages(args) -> None:
+    """--stages: every fine-level stage of the hot path launched ONCE on the full-size grid inside a cudaProfilerStart/Stop
+    range, so that `ncu --profile-from-start off --set full` captures exactly one launch of each kernel (after a few
+    warm-up steps, which are not captured)."""
+    import torch
+    k = WORKLOADS[args.workload]
+    cfg = workload_config(k)
+    s, dt0 = make_sim(cfg, "cuda:0")
+    for i in range(max(args.warmup, 1)):
+        s.step(dt0 if i == 0 else 0.0, dt0, adaptive=True)
+    dt = s.cfl()
+    torch.cuda.synchronize()
+    torch.cuda.profiler.start()
+    s.measure(1.0)
+    s.dbg_save_u0()
+    s.dbg_conv_diff_bdim(dt, 0)
+    s.dbg_bc()
+    if cfg["exit_bc"]:
+        s.dbg_exit_bc(dt)
+    s.dbg_conv_diff_bdim(dt, 1)
+    s.dbg_residual()
+    s.dbg_restrict(0)
+    s.dbg_prolong(0)
+    s.dbg_smooth(0, 3)
+    s.dbg_residual()
+    s.dbg_apply_gradient()
+    s.cfl()
+    s.energy()
+    if cfg["body_kind"] != wi.BODY_NONE:
+        s.pressure_force(1.0)
+    torch.cuda.synchronize()
+    torch.cuda.profiler.stop()
+    s.close()
+    print("bench.py --stages: done", file=sys.stderr)
 
 
 def run_gpu(args) -> None:
@@ -297,8 +388,9 @@ def run_gpu(args) -> None:
         return float(t.item())
 
     k = WORKLOADS[args.workload]
-    cfg = wi.baseline_config(k)
+    cfg = workload_config(k)
     cells = ncells(cfg)
+    force = (k == 2)                                   # BASELINE configs[2]: "pressure force each step"
     sim, dt0 = make_sim(cfg, device)
     peaks = {}
     try:
@@ -308,57 +400,39 @@ def run_gpu(args) -> None:
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback (B200_PROFILING.md 6.65 TB/s)"
 
-    # ---- timed region: K steps, device-timed, clocks sampled meanwhile
-    l0 = sim.stats()["kernel_launches"]
+    # ---- timed region: R blocks of K steps, device-timed, clocks sampled meanwhile
     for i in range(args.warmup):
         sim.step(dt0 if i == 0 else 0.0, dt0, adaptive=True)
+        if force:
+            sim.pressure_force()
     l1 = sim.stats()["kernel_launches"]
     sampler = ClockSampler(local) if rank == 0 else None
-    ms_local = time_steps(torch, sim, dt0, args.steps, 0, dist)
+    blocks = [reduce_max(time_steps(torch, sim, dt0, args.steps, 0, dist, force=force)) for _ in range(args.repeats)]
     clocks = sampler.stop() if sampler else None
     l2 = sim.stats()["kernel_launches"]
-    agg = aggregate(ms_local, cells, args.steps, world, reduce_max)
+    ms_med = statistics.median(blocks)
+    agg = aggregate(ms_med, cells, args.steps, world)
     dt_now = sim.cfl()
     st = sim.stats()
 
-    # ---- same K steps again with every launch bracketed by CUDA events: per-kernel-class times
-    sim.prof_enable(True)
-    ms_prof = time_steps(torch, sim, dt0, args.steps, 0, None)
-    prof = sim.prof_read()
-    sim.prof_enable(False)
+    prof, alg, kernels, step = profile_classes(torch, sim, cfg, dt0, args.steps, hbm_peak, agg["ms"] / args.steps, force=force)
+    if world > 1:
+        step["achieved_gbs"] = step["frac_of_measured_peak"] = step["frac_of_nominal_8TBs"] = None
     tot_prof = sum(v[0] for v in prof.values())
-    alg = dict(ALG_BYTES)
-    alg["conv_diff_bdim"] = conv_alg_bytes(cfg)
-    if "pcg_fused" in prof:                           # one-sweep form: every fine-level pcg_matvec launch is a first sweep, r -> e', q
-        alg["pcg_matvec"] = 4 * (1 + 2)
-        # ... and of the two last sweeps of a solve (fixed two V-cycles) the second leaves r alone (x, e' -> x): mean of 24 and 12
-        alg["pcg_update"] = (4 * (4 + 2) + 4 * (2 + 1)) / 2
-    breakdown = {}
-    for name, (ms, n) in sorted(prof.items(), key=lambda kv: -kv[1][0]):
-        ent = {"ms_per_step": ms / args.steps, "launches_per_step": n / args.steps, "share": ms / tot_prof}
-        if name in alg and alg[name]:                 # fine-level classes only (".coarse" = multigrid levels >= 1)
-            ent["alg_gbs"] = alg[name] * cells * n / (ms * 1e-3) / 1e9
-        breakdown[name] = ent
     # the dominant kernel with a roofline: the fine-level class that takes the most time
-    dom = next((nm for nm in breakdown if alg.get(nm)), next(iter(breakdown)))
+    dom = next((nm for nm in kernels if alg.get(nm)), next(iter(kernels)))
     dom_ms, dom_n = prof[dom]
-    base = dom.split(".")[0]
-    achieved = (alg.get(base) or 0) * cells * dom_n / (dom_ms * 1e-3) / 1e9 if not dom.endswith(".coarse") else None
-    # step-level view: algorithmic bytes of all fine-level passes / step time
-    step_bytes = sum((alg.get(nm) or 0) * cells * n for nm, (ms, n) in prof.items() if not nm.endswith(".coarse")) / args.steps
+    achieved = alg[dom] * cells * dom_n / (dom_ms * 1e-3) / 1e9 if alg.get(dom) else None
+    traffic = ncu_traffic(args.workload)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
                 "frac": (achieved / hbm_peak) if achieved else None, "frac_of_nominal_8TBs": (achieved / 8000.0) if achieved else None,
                 "peak_source": peak_src,
-                "traffic": NCU_TRAFFIC_C4.get(base) if args.workload == "C4" else None,
-                "traffic_source": (("profiles/r1e_pcg_fused_c4_ncu.md" if base == "pcg_fused" else "profiles/r1c_stages_c4_ncu.md")
-                                   + " (ncu --set full, one launch)") if args.workload == "C4" else None,
-                "alg_bytes_per_cell_per_launch": alg.get(base), "avg_launch_us": dom_ms / dom_n * 1e3,
-                "share_of_step": dom_ms / tot_prof,
-                "step": {"alg_bytes_per_cell_per_step": step_bytes / cells,
-                         "achieved_gbs": step_bytes / (agg["ms"] / args.steps * 1e-3) / 1e9 if world == 1 else None,
-                         "frac": step_bytes / (agg["ms"] / args.steps * 1e-3) / 1e9 / hbm_peak if world == 1 else None},
-                "profiled_ms_per_step": ms_prof / args.steps,
-                "kernels": breakdown}
+                "traffic": traffic.get(dom),
+                "traffic_source": "profiles/r2_ncu_traffic_c4.csv (ncu --set full, one launch of every fine-level kernel, this round)"
+                                  if traffic.get(dom) else None,
+                "traffic_all_kernels": traffic or None,
+                "alg_bytes_per_cell_per_launch": alg.get(dom), "avg_launch_us": dom_ms / dom_n * 1e3,
+                "share_of_step": dom_ms / tot_prof, "step": step, "kernels": kernels}
 
     # ---- end to end through the C ABI with HOST buffers: set_fields(host) + step + get_fields(host)
     e2e_steps = max(1, min(args.steps, 5))
@@ -384,47 +458,71 @@ def run_gpu(args) -> None:
            "call": "wl_set_fields(host u,p) + wl_step + wl_get_fields(host u,p), pinned host memory, wall clock"}
     sim.close()
     del hu, hp
+    torch.cuda.empty_cache()
 
-    # ---- the other 3-D BASELINE workloads, short runs (rank 0, N = 1 only)
+    # ---- tolerance mode (reported separately, with the mean number of V-cycles per solve)
+    tol_mode = None
+    if world == 1 and not args.no_tol:
+        ct = dict(cfg, fixed_vcycles=0, tol=1e-4, max_vcycles=32)
+        s2, d0 = make_sim(ct, device)
+        for i in range(args.warmup):
+            s2.step(d0 if i == 0 else 0.0, d0, adaptive=True)
+        torch.cuda.synchronize()
+        nv, res = [], []
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(s2._stream)
+        for _ in range(args.steps):
+            s2.step(0.0, d0, adaptive=True)
+            q = s2.stats()                             # host-side counters: no synchronisation
+            nv += q["vcycles"]; res += q["res"]
+        e1.record(s2._stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        tol_mode = {"tol": 1e-4, "max_vcycles": 32, "ns_per_cell_step": ms * 1e6 / (cells * args.steps), "ms_per_step": ms / args.steps,
+                    "mean_vcycles_per_solve": sum(nv) / len(nv), "max_vcycles_seen": max(nv), "max_residual": max(res),
+                    "not_converged": s2.stats()["noconv"],
+                    "note": "each V-cycle ends with a host read of max|r| (the only host round trip of the path)"}
+        s2.close()
+        torch.cuda.empty_cache()
+
+    # ---- the other workloads, one timed block each (rank 0, N = 1 only): BASELINE.md section 3's table
     also = {}
     if world == 1 and not args.no_also:
         for name, kk in WORKLOADS.items():
             if name == args.workload:
                 continue
-            c2 = wi.baseline_config(kk)
-            s2, d0 = make_sim(c2, device)
-            ms = time_steps(torch, s2, d0, args.steps, args.warmup, None)
-            also[wi.WORKLOAD_NAMES[kk]] = {"cells": ncells(c2), "ns_per_cell_step": ms * 1e6 / (ncells(c2) * args.steps),
-                                           "ms_per_step": ms / args.steps}
-            s2.close()
+            try:
+                c2 = workload_config(kk)
+                s2, d0 = make_sim(c2, device)
+                nst = args.steps if ncells(c2) < 100e6 else min(args.steps, 10)
+                f2 = (kk == 2)
+                ms = time_steps(torch, s2, d0, nst, args.warmup, None, force=f2)
+                _, _, kern2, step2 = profile_classes(torch, s2, c2, d0, nst, hbm_peak, ms / nst, force=f2)
+                top = next(iter(kern2))
+                also[NAMES[kk]] = {"cells": ncells(c2), "steps": nst, "ns_per_cell_step": ms * 1e6 / (ncells(c2) * nst),
+                                   "ms_per_step": ms / nst, "force_every_step": f2, **step2,
+                                   "top_kernel": top, "top_kernel_share": kern2[top]["share"]}
+                s2.close()
+            except Exception as e:                       # e.g. not enough free memory on a shared box
+                also[NAMES[kk]] = {"skipped": str(e)[:120]}
             torch.cuda.empty_cache()
-        # the shape of the paper's headline figure (TGV 512^3, 134 M cells; here fully periodic and with
-        # the fixed two V-cycles of the BASELINE configs): context beside the paper's 1.57 ns on an H100, not a config
-        try:
-            c2 = wi.tgv3d(512)
-            s2, d0 = make_sim(c2, device)
-            ms = time_steps(torch, s2, d0, min(args.steps, 10), 3, None)
-            also["TGV3D_512_paper_headline_shape"] = {"cells": ncells(c2), "ns_per_cell_step": ms * 1e6 / (ncells(c2) * min(args.steps, 10)),
-                                                      "ms_per_step": ms / min(args.steps, 10)}
-            s2.close()
-        except Exception as e:                       # not enough free memory on a shared box: skip the context line
-            also["TGV3D_512_paper_headline_shape"] = {"skipped": str(e)[:120]}
-        torch.cuda.empty_cache()
 
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
-    cpu = oracle_sample(cfg, k) if (world == 1 and not args.no_cpu) else None
+    cpu = oracle_sample(k) if (world == 1 and not args.no_cpu) else None
     line = {"metric": METRIC, "value": agg["ns_per_cell_step"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": agg["ms"] / args.steps, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": config_dict(cfg, args.workload, k, note="replicas only: every rank runs this workload" if world > 1 else None),
-            "cells_steps_per_s": agg["cells_steps_per_s"],
-            "clocks": clocks, "e2e": e2e, "gpu_launches": l2 - l1, "gpu_launches_per_step": (l2 - l1) / args.steps,
+            "config": config_dict(cfg, k, note="replicas only: every rank runs this workload" if world > 1 else None),
+            "repeats": {"n": args.repeats, "statistic": "median", "ms_per_step_min": min(blocks) / args.steps,
+                        "ms_per_step_median": ms_med / args.steps, "ms_per_step_max": max(blocks) / args.steps},
+            "cells_steps_per_s": agg["cells_steps_per_s"], "force_every_step": force,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": l2 - l1, "gpu_launches_per_step": (l2 - l1) / (args.steps * args.repeats),
             "vcycles_per_solve": st["vcycles"], "nan_flag": st["nan_flag"], "dt_last": dt_now,
-            "roofline": roofline, "cpu_baseline": cpu, "also": also,
-            "context": "paper: 1.57 ns/DOF/step on H100 64GB, fp32, TGV 512^3 (PAPER.md:143); another machine and workload, not a target"}
+            "roofline": roofline, "cpu_baseline": cpu, "tolerance_mode": tol_mode, "also": also,
+            "context": "paper: 1.57 ns/DOF/step on H100 64GB, fp32, half-domain TGV 512^3 (PAPER.md:143); another machine, not a target"}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -435,15 +533,20 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--repeats", type=int, default=5, help="timed blocks of --steps steps; the median is reported")
     ap.add_argument("--workload", choices=sorted(WORKLOADS), default="C4")
     ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     ap.add_argument("--no-also", action="store_true", help="skip the other workloads")
+    ap.add_argument("--no-tol", action="store_true", help="skip the tolerance-mode leg")
+    ap.add_argument("--stages", action="store_true", help="one launch per fine-level stage inside a profiler range (for ncu); no JSON")
     args = ap.parse_args()
-    if args.warmup < 3 and args.impl == "b200":
+    if args.warmup < 3 and args.impl == "b200" and not args.stages:
         print(f"bench.py: warning: --warmup {args.warmup} < 3 (timing rules ask for >= 3)", file=sys.stderr)
     if args.impl == "reference":
         run_reference(args)
+    elif args.stages:
+        run_stages(args)
     else:
         run_gpu(args)
 

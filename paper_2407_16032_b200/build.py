@@ -63,7 +63,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         if p.returncode != 0:
             sys.stderr.write(logs[-1])
             raise RuntimeError(f"nvcc failed on {src}")
-    cmd = [nvcc, "-shared", "-o", str(LIB), *objs, "-lcudart"]
+    cmd = [nvcc, "-shared", "-o", str(LIB), *objs, "-lcudart", "-ldl"]
     r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     logs.append(f"$ {' '.join(cmd)}\n{r.stdout}")
     if r.returncode != 0:

@@ -74,6 +74,20 @@ def test_reference_arm_prints_contract_line():
     assert line["impl"] == "reference" and line["unit"] == "ns/cell/step" and line["higher_is_better"] is False
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["value"] > 0
+    # the reference arm times the workload itself (C2: 128^3), not a scaled sample
+    assert line["cpu_baseline"]["same_config"] is True and line["config"]["cells"] == 128 ** 3
+    assert "128x128x128" in line["cpu_baseline"]["sample"]
+
+
+def test_traffic_table_is_read_from_profiles():
+    """roofline.traffic comes from the committed ncu summary of this round, not from constants in bench.py"""
+    sys.path.insert(0, str(ROOT))
+    import bench
+    assert "NCU_TRAFFIC" not in (ROOT / "bench.py").read_text()
+    t = bench.ncu_traffic("C4")
+    if bench.TRAFFIC_FILE.exists():
+        assert t and all(v > 0 for v in t.values()) and "pcg_fused" in t
+    assert bench.ncu_traffic("C3") == {}
 
 
 def test_reference_arm_other_ranks_exit_quietly():
