@@ -27,7 +27,8 @@
  * projection, free-stream preservation, 2-D Taylor-Green closed-form decay, CFL closed
  * forms, force vs divergence theorem; the two constants the readings add (the decoupling
  * threshold of level_diag, the relative stop of wlo_smooth) by hand-set coefficients and by a
- * two-eigenmode residual with closed-form iterates.  No function here is "parity unpinned" except
+ * two-eigenmode residual with closed-form iterates; general bodies (shell, non-rigid map, spin, SDF arithmetic) by the
+ * uniformly scaled sphere, finite differences of the map, and the paper's jellyfish listing.  No function here is "parity unpinned" except
  * whole-run physical values (C_D etc.), which need the paper's run lengths and data.
  */
 #include <math.h>
@@ -41,8 +42,25 @@
 #define WLO_MAXLEV 16
 #define WLO_PI 3.14159265358979323846
 
-enum { WLO_BODY_NONE = 0, WLO_BODY_SPHERE = 1, WLO_BODY_TORUS = 2, WLO_BODY_CYLINDER = 3 };
+enum { WLO_BODY_NONE = 0, WLO_BODY_SPHERE = 1, WLO_BODY_TORUS = 2, WLO_BODY_CYLINDER = 3, WLO_BODY_PLANE = 4 };
+enum { WLO_OP_UNION = 0, WLO_OP_DIFFERENCE = 1 };
+#define WLO_MAX_EXTRA 3
 enum { WLO_MOTION_STATIC = 0, WLO_MOTION_SIN = 1 };
+
+/* one further primitive of a composite body (SDF arithmetic, "body = big + small", "sphere - plane"):
+ * the same fields as the first primitive, which lives in wlo_config itself */
+typedef struct {
+    int kind;
+    double centre[3];
+    double R, r;
+    int axis;
+    int motion;
+    double amp[3], freq[3], phase[3];
+    double shell;
+    double scale_amp[3], scale_freq, scale_phase;
+    double spin;
+    int op;             /* WLO_OP_*: how this primitive combines with the body built so far */
+} wlo_part;
 
 typedef struct {
     int ndim;
@@ -64,6 +82,13 @@ typedef struct {
     /* multigrid */
     int max_levels, smooth_iters, max_vcycles, fixed_vcycles;
     double tol;
+    /* general bodies (reading R-E3): thin shell, non-rigid diagonal map, spin, further primitives */
+    double shell;       /* > 0: the body is the shell of this half-thickness around the surface: sdf <- |sdf| - shell */
+    double scale_amp[3], scale_freq, scale_phase;   /* map xi_d = s_d(t) (x_d - c_d(t)), s_d = 1 + scale_amp[d] cos(2 pi scale_freq t + scale_phase) ("A(t) .* x + B(t)") */
+    double spin;        /* angular velocity of the primitive about its axis (z in 2-D) through its centre: the SDF is unchanged
+                           (bodies of revolution about that axis), the surface velocity is not ("spinning circles") */
+    int nextra;
+    wlo_part extra[WLO_MAX_EXTRA];
 } wlo_config;
 
 typedef struct {
@@ -155,53 +180,125 @@ double wlo_kernel_mu1(double d, double eps)
  * P:104 "AutoBody type holds the signed-distance function as well as the coordinates
  * mapping"; "signed-distance d and normal n from any point in space".  Reading R-E:
  * analytic gradients of the parametric SDFs (same values the paper gets by AD).
- * Maps are translations xi = x - c(t), sinusoidal in every direction,
- *   c_d(t) = c0_d + amp_d sin(2 pi f_d t + phase_d)
- * (the heaving sphere of BASELINE configs[4]: one direction; the two-degree-of-freedom cylinder of P:181,
- * y = A_y sin(w t), x = A_x sin(2 w t + theta): two), so J = I and V = dc/dt (uniform).  |grad| < 1e-12 => n = 0.
- * The circular cylinder of P:121 (radius R, axis e_a, spanning a periodic direction): d = |xi - (xi.e_a) e_a| - R.
+ * Reading R-E3 (general bodies, SURVEY O2 "n = J^T grad sdf / |.|, V = -J^-1 dmap/dt"):
+ *   map     xi_d = s_d(t) (x_d - c_d(t)),  c_d(t) = c0_d + amp_d sin(2 pi f_d t + phase_d)   (translation; the heaving
+ *           sphere of BASELINE configs[4]: one direction; the 2-DOF cylinder of P:181: two),
+ *           s_d(t) = 1 + scale_amp_d cos(2 pi scale_freq t + scale_phase)                    (the "A(t) .* x" of P:237);
+ *           J = diag(s).
+ *   sdf     d0 = sdf(xi) of the primitive, g = grad_xi sdf; shell > 0: d0 <- |d0| - shell, g <- sign(d0) g;
+ *   normal  grad_x d0 = J^T g = s .* g, m = |s .* g|; n = (s .* g)/m;
+ *   distance d = d0/m: the first-order distance in physical space (exact for a uniformly scaled sphere: |x-c| - R/s);
+ *           m < 1e-12 => n = 0, d = d0;
+ *   velocity a material point has fixed xi: x(t) = c + xi ./ s, so V_d = dc_d/dt - (ds_d/dt / s_d)(x_d - c_d)  (= -J^-1 dmap/dt),
+ *           plus spin * e_axis x (x - c) for a primitive spinning about its axis.
+ * Primitives: sphere |xi| - R (circle in 2-D); torus (axis a); circular cylinder of P:121 (radius R, axis e_a, spanning a
+ * periodic direction) rho - R; half-space xi_a (below the plane through the centre with normal +e_a).
+ * SDF arithmetic: union  d = min(d_A, d_B), difference A - B  d = max(d_A, -d_B); normal and velocity are
+ * those of the primitive that decides (for -d_B: -n_B, V_B).
  * Returns d; fills nrm[3], vel[3].
  */
-double wlo_body_eval(const wlo_config *cf, const double *xpt, double t, double *nrm, double *vel)
+static double prim_sdf(int nd, int kind, int axis, double R, double r, const double *xi, double *g)
 {
-    int nd = cf->ndim;
-    double c[3] = { cf->centre[0], cf->centre[1], cf->centre[2] };
-    nrm[0] = nrm[1] = nrm[2] = 0.0;
-    vel[0] = vel[1] = vel[2] = 0.0;
-    if (cf->body_kind == WLO_BODY_NONE) return 1e30;
-    if (cf->motion == WLO_MOTION_SIN) {
-        for (int k = 0; k < nd; ++k) {
-            double ph = 2.0 * WLO_PI * cf->freq[k] * t + cf->phase[k];
-            c[k] += cf->amp[k] * sin(ph);
-            vel[k] = cf->amp[k] * 2.0 * WLO_PI * cf->freq[k] * cos(ph);
-        }
-    }
-    double xi[3] = { 0, 0, 0 };
-    for (int k = 0; k < nd; ++k) xi[k] = xpt[k] - c[k];
-    if (cf->body_kind == WLO_BODY_SPHERE) {      /* circle in 2-D */
+    g[0] = g[1] = g[2] = 0.0;
+    if (kind == WLO_BODY_SPHERE) {               /* circle in 2-D */
         double rr = 0;
         for (int k = 0; k < nd; ++k) rr += xi[k] * xi[k];
         rr = sqrt(rr);
-        if (rr >= 1e-12) for (int k = 0; k < nd; ++k) nrm[k] = xi[k] / rr;
-        return rr - cf->R;
+        if (rr >= 1e-12) for (int k = 0; k < nd; ++k) g[k] = xi[k] / rr;
+        return rr - R;
     }
+    if (kind == WLO_BODY_PLANE) { g[axis] = 1.0; return xi[axis]; }
     /* torus and cylinder (3-D): axis a; rho = distance from the axis in the (b,c) plane */
-    int a = cf->axis, b = (a + 1) % 3, cc = (a + 2) % 3;
+    int a = axis, b = (a + 1) % 3, cc = (a + 2) % 3;
     double rho = sqrt(xi[b] * xi[b] + xi[cc] * xi[cc]);
-    if (cf->body_kind == WLO_BODY_CYLINDER) {
-        if (rho >= 1e-12) { nrm[b] = xi[b] / rho; nrm[cc] = xi[cc] / rho; }
-        return rho - cf->R;
+    if (kind == WLO_BODY_CYLINDER) {
+        if (rho >= 1e-12) { g[b] = xi[b] / rho; g[cc] = xi[cc] / rho; }
+        return rho - R;
     }
-    double w = rho - cf->R;
-    double g = sqrt(w * w + xi[a] * xi[a]);
-    if (g >= 1e-12 && rho >= 1e-12) {
-        nrm[a] = xi[a] / g;
-        nrm[b] = (w / g) * (xi[b] / rho);
-        nrm[cc] = (w / g) * (xi[cc] / rho);
-    } else if (g >= 1e-12) {
-        nrm[a] = xi[a] / g;     /* on the axis: in-plane direction undefined */
+    double w = rho - R;
+    double q = sqrt(w * w + xi[a] * xi[a]);
+    if (q >= 1e-12 && rho >= 1e-12) {
+        g[a] = xi[a] / q;
+        g[b] = (w / q) * (xi[b] / rho);
+        g[cc] = (w / q) * (xi[cc] / rho);
+    } else if (q >= 1e-12) {
+        g[a] = xi[a] / q;       /* on the axis: in-plane direction undefined */
     }
-    return g - cf->r;
+    return q - r;
+}
+
+static double part_eval(int nd, const wlo_part *p, const double *xpt, double t, double *nrm, double *vel)
+{
+    double c[3], cdot[3] = { 0, 0, 0 }, sc[3] = { 1, 1, 1 }, sdot[3] = { 0, 0, 0 }, xi[3] = { 0, 0, 0 }, g[3];
+    for (int k = 0; k < 3; ++k) c[k] = p->centre[k];
+    if (p->motion == WLO_MOTION_SIN)
+        for (int k = 0; k < nd; ++k) {
+            double ph = 2.0 * WLO_PI * p->freq[k] * t + p->phase[k];
+            c[k] += p->amp[k] * sin(ph);
+            cdot[k] = p->amp[k] * 2.0 * WLO_PI * p->freq[k] * cos(ph);
+        }
+    {
+        double ph = 2.0 * WLO_PI * p->scale_freq * t + p->scale_phase;
+        for (int k = 0; k < nd; ++k) {
+            sc[k] = 1.0 + p->scale_amp[k] * cos(ph);
+            sdot[k] = -p->scale_amp[k] * 2.0 * WLO_PI * p->scale_freq * sin(ph);
+        }
+    }
+    for (int k = 0; k < nd; ++k) xi[k] = sc[k] * (xpt[k] - c[k]);
+    double d0 = prim_sdf(nd, p->kind, p->axis, p->R, p->r, xi, g);
+    if (p->shell > 0.0) {
+        double sg = d0 < 0.0 ? -1.0 : 1.0;
+        d0 = fabs(d0) - p->shell;
+        for (int k = 0; k < 3; ++k) g[k] *= sg;
+    }
+    double m = 0;
+    for (int k = 0; k < nd; ++k) { g[k] *= sc[k]; m += g[k] * g[k]; }
+    m = sqrt(m);
+    nrm[0] = nrm[1] = nrm[2] = 0.0;
+    double d = d0;
+    if (m >= 1e-12) {
+        d = d0 / m;
+        for (int k = 0; k < nd; ++k) nrm[k] = g[k] / m;
+    }
+    vel[0] = vel[1] = vel[2] = 0.0;
+    for (int k = 0; k < nd; ++k) vel[k] = cdot[k] - (sdot[k] / sc[k]) * (xpt[k] - c[k]);
+    if (p->spin != 0.0) {                        /* spin e_a x (x - c); 2-D: a = z */
+        int a = nd == 3 ? p->axis : 2, b = (a + 1) % 3, cc = (a + 2) % 3;
+        double xb = b < nd ? xpt[b] - c[b] : 0.0, xc = cc < nd ? xpt[cc] - c[cc] : 0.0;
+        if (b < nd) vel[b] += -p->spin * xc;
+        if (cc < nd) vel[cc] += p->spin * xb;
+    }
+    return d;
+}
+
+double wlo_body_eval(const wlo_config *cf, const double *xpt, double t, double *nrm, double *vel)
+{
+    int nd = cf->ndim;
+    nrm[0] = nrm[1] = nrm[2] = 0.0;
+    vel[0] = vel[1] = vel[2] = 0.0;
+    if (cf->body_kind == WLO_BODY_NONE) return 1e30;
+    wlo_part first;
+    memset(&first, 0, sizeof(first));
+    first.kind = cf->body_kind; first.R = cf->R; first.r = cf->r; first.axis = cf->axis; first.motion = cf->motion;
+    first.shell = cf->shell; first.scale_freq = cf->scale_freq; first.scale_phase = cf->scale_phase; first.spin = cf->spin;
+    for (int k = 0; k < 3; ++k) {
+        first.centre[k] = cf->centre[k]; first.amp[k] = cf->amp[k]; first.freq[k] = cf->freq[k]; first.phase[k] = cf->phase[k];
+        first.scale_amp[k] = cf->scale_amp[k];
+    }
+    double d = part_eval(nd, &first, xpt, t, nrm, vel);
+    for (int e = 0; e < cf->nextra; ++e) {
+        double n2[3], v2[3];
+        double d2 = part_eval(nd, &cf->extra[e], xpt, t, n2, v2);
+        if (cf->extra[e].op == WLO_OP_DIFFERENCE) {
+            d2 = -d2;
+            for (int k = 0; k < 3; ++k) n2[k] = -n2[k];
+            if (d2 > d) { d = d2; for (int k = 0; k < 3; ++k) { nrm[k] = n2[k]; vel[k] = v2[k]; } }
+        } else if (d2 < d) {
+            d = d2;
+            for (int k = 0; k < 3; ++k) { nrm[k] = n2[k]; vel[k] = v2[k]; }
+        }
+    }
+    return d;
 }
 
 /* -------------------------------------------------- O7: Poisson diagonal
@@ -940,8 +1037,15 @@ static int config_ok(const wlo_config *cf)
     if (cf->ndim != 2 && cf->ndim != 3) return 0;
     for (int d = 0; d < cf->ndim; ++d) if (cf->dims[d] < 4) return 0;
     if (cf->nu < 0 || !(cf->eps > 0)) return 0;
-    if (cf->body_kind < 0 || cf->body_kind > 3) return 0;
+    if (cf->body_kind < 0 || cf->body_kind > 4) return 0;
     if ((cf->body_kind == WLO_BODY_TORUS || cf->body_kind == WLO_BODY_CYLINDER) && (cf->ndim != 3 || cf->axis < 0 || cf->axis > 2)) return 0;
+    if (cf->body_kind == WLO_BODY_PLANE && (cf->axis < 0 || cf->axis >= cf->ndim)) return 0;
+    if (cf->nextra < 0 || cf->nextra > WLO_MAX_EXTRA || (cf->nextra > 0 && cf->body_kind == WLO_BODY_NONE)) return 0;
+    for (int e = 0; e < cf->nextra; ++e) {
+        const wlo_part *p = &cf->extra[e];
+        if (p->kind < 1 || p->kind > 4 || p->axis < 0 || p->axis > 2) return 0;
+        if ((p->kind == WLO_BODY_TORUS || p->kind == WLO_BODY_CYLINDER) && cf->ndim != 3) return 0;
+    }
     return 1;
 }
 

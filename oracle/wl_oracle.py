@@ -21,8 +21,17 @@ import numpy as np
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "wl_oracle.c"
 
-BODY_NONE, BODY_SPHERE, BODY_TORUS, BODY_CYLINDER = 0, 1, 2, 3
+BODY_NONE, BODY_SPHERE, BODY_TORUS, BODY_CYLINDER, BODY_PLANE = 0, 1, 2, 3, 4
 MOTION_STATIC, MOTION_SIN = 0, 1
+
+
+class Part(C.Structure):
+    _fields_ = [
+        ("kind", C.c_int), ("centre", C.c_double * 3), ("R", C.c_double), ("r", C.c_double), ("axis", C.c_int),
+        ("motion", C.c_int), ("amp", C.c_double * 3), ("freq", C.c_double * 3), ("phase", C.c_double * 3),
+        ("shell", C.c_double), ("scale_amp", C.c_double * 3), ("scale_freq", C.c_double), ("scale_phase", C.c_double),
+        ("spin", C.c_double), ("op", C.c_int),
+    ]
 
 
 class Config(C.Structure):
@@ -37,6 +46,8 @@ class Config(C.Structure):
         ("amp", C.c_double * 3), ("freq", C.c_double * 3), ("phase", C.c_double * 3),
         ("max_levels", C.c_int), ("smooth_iters", C.c_int), ("max_vcycles", C.c_int),
         ("fixed_vcycles", C.c_int), ("tol", C.c_double),
+        ("shell", C.c_double), ("scale_amp", C.c_double * 3), ("scale_freq", C.c_double), ("scale_phase", C.c_double),
+        ("spin", C.c_double), ("nextra", C.c_int), ("extra", Part * 3),
     ]
 
 
@@ -149,6 +160,27 @@ def make_config(cfg: dict) -> Config:
     for k in ("exit_bc", "body_kind", "axis", "motion", "max_levels", "smooth_iters",
               "max_vcycles", "fixed_vcycles"):
         setattr(c, k, int(cfg[k]))
+    # general bodies: shell, diagonal scaling map, spin, further primitives (all optional in the dict)
+    c.shell, c.scale_freq, c.scale_phase = float(cfg.get("shell", 0.0)), float(cfg.get("scale_freq", 0.0)), float(cfg.get("scale_phase", 0.0))
+    c.spin = float(cfg.get("spin", 0.0))
+    for d in range(3):
+        c.scale_amp[d] = float((cfg.get("scale_amp") or (0.0, 0.0, 0.0))[d])
+    parts = cfg.get("parts") or []
+    c.nextra = len(parts)
+    for e, pd in enumerate(parts):
+        q = c.extra[e]
+        full = dict(centre=(0.0, 0.0, 0.0), R=0.0, r=0.0, axis=0, motion=MOTION_STATIC, heave_dir=1, amp=0.0, freq=0.0, phase=0.0,
+                    amp3=None, freq3=None, phase3=None, shell=0.0, scale_amp=(0.0, 0.0, 0.0), scale_freq=0.0, scale_phase=0.0,
+                    spin=0.0, op="+")
+        full.update(pd)
+        q.kind, q.R, q.r, q.axis, q.motion = int(full["kind"]), float(full["R"]), float(full["r"]), int(full["axis"]), int(full["motion"])
+        amp, freq, phase = wi_motion(full)
+        for d in range(3):
+            q.centre[d] = float(full["centre"][d]) if d < len(full["centre"]) else 0.0
+            q.amp[d], q.freq[d], q.phase[d] = amp[d], freq[d], phase[d]
+            q.scale_amp[d] = float(full["scale_amp"][d])
+        q.shell, q.scale_freq, q.scale_phase, q.spin = float(full["shell"]), float(full["scale_freq"]), float(full["scale_phase"]), float(full["spin"])
+        q.op = 1 if full["op"] == "-" else 0
     return c
 
 

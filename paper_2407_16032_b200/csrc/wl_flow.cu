@@ -387,6 +387,29 @@ void wl_k_set_time(wl_sim* s, double t, float dt, int t_mode, int dt_mode)
     k_set_time<<<1, 1, 0, s->st>>>(s->ds, s->cfg.body, t, dt, t_mode, dt_mode);
 }
 
+// The box of padded cells the body can reach, grown by `margin` cells: the supported motion is a sinusoidal translation of
+// known amplitude, so the box is known on the host although t is device-resident.  interior: clip to the interior cells.
+void wl_body_box(const wl_sim* s, float margin, int interior, int o[3], int e[3])
+{
+    const Grid& g = s->lev[0].g;
+    const wl_body& b = s->cfg.body;
+    for (int d = 0; d < 3; ++d) { o[d] = interior && d < s->nd ? 1 : 0; e[d] = interior ? g.n[d] : g.S[d]; }
+    for (int d = 0; d < s->nd; ++d) {
+        const int first = interior ? 1 : 0, last = interior ? g.n[d] : g.n[d] + 1;
+        float ext = b.R;                                          // sphere / circle / cylinder cross-section
+        if (b.kind == WL_BODY_TORUS) ext = d == b.axis ? b.r : b.R + b.r;
+        float reach = ext + margin;
+        if (b.motion == WL_MOTION_SIN) reach += fabsf(b.amp[d]);
+        int lo = (int)floorf(b.centre[d] - reach), hi = (int)ceilf(b.centre[d] + reach) + 1;      // padded coordinates c = x + 1/2
+        if (b.kind == WL_BODY_CYLINDER && d == b.axis) { lo = first; hi = last; }                 // it spans the direction
+        if (lo < first) lo = first;
+        if (hi > last) hi = last;
+        if (g.per[d] && (lo <= 2 || hi >= g.n[d] - 1)) { lo = first; hi = last; }   // ghosts mirror the far side: whole direction
+        if (hi < lo) { lo = first; hi = last; }
+        o[d] = lo; e[d] = hi - lo + 1;
+    }
+}
+
 // measure! over the whole padded grid the first time; afterwards only over the box the body can reach: mu0 = 1 and
 // mu1 = 0 further than eps from the surface never change (the boundary-face zeros of mu0 neither), and the supported
 // motion is a sinusoidal translation of known amplitude, so the box is known on the host although t is device-resident.
@@ -396,20 +419,8 @@ void wl_k_measure(wl_sim* s)
     Tiling T = wl_tiles_padded(s, g);
     const wl_body& b = s->cfg.body;
     if (s->measured && b.kind != WL_BODY_NONE) {
-        int o[3] = { 0, 0, 0 }, e[3] = { g.S[0], g.S[1], g.S[2] };
-        for (int d = 0; d < s->nd; ++d) {
-            float ext = b.R;                                          // sphere / circle / cylinder cross-section
-            if (b.kind == WL_BODY_TORUS) ext = d == b.axis ? b.r : b.R + b.r;
-            float reach = ext + s->cfg.eps + 2.0f;                    // the face positions are half a cell off the centres
-            if (b.motion == WL_MOTION_SIN) reach += fabsf(b.amp[d]);
-            int lo = (int)floorf(b.centre[d] - reach), hi = (int)ceilf(b.centre[d] + reach) + 1;      // padded coordinates c = x + 1/2
-            if (b.kind == WL_BODY_CYLINDER && d == b.axis) { lo = 0; hi = g.n[d] + 1; }               // it spans the direction
-            if (lo < 0) lo = 0;
-            if (hi > g.n[d] + 1) hi = g.n[d] + 1;
-            if (g.per[d] && (lo <= 2 || hi >= g.n[d] - 1)) { lo = 0; hi = g.n[d] + 1; }   // ghosts mirror the far side: whole direction
-            if (hi < lo) { lo = 0; hi = g.n[d] + 1; }
-            o[d] = lo; e[d] = hi - lo + 1;
-        }
+        int o[3], e[3];
+        wl_body_box(s, s->cfg.eps + 2.0f, 0, o, e);                   // the face positions are half a cell off the centres
         T = wl_tiling(s->nd, o, e);
     }
     for (int d = 0; d < 3; ++d) { s->mbox_lo[d] = T.o[d]; s->mbox_hi[d] = T.o[d] + T.e[d] - 1; }
@@ -477,6 +488,11 @@ void wl_k_force(wl_sim* s, double t)
 {
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_interior(s, g);
+    if (s->cfg.body.kind != WL_BODY_NONE) {          // K(d) vanishes further than one cell from the surface: the body's box is enough
+        int o[3], e[3];
+        wl_body_box(s, 3.0f, 1, o, e);
+        T = wl_tiling(s->nd, o, e);
+    }
     {
         ProfScope ps(s, WLK_SET_TIME);
         k_force_time<<<1, 1, 0, s->st>>>(s->ds, s->cfg.body, t);

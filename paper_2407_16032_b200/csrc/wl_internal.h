@@ -131,6 +131,7 @@ FlowP wl_flowp(const wl_sim* s);
 // wl_flow.cu
 void wl_k_set_time(wl_sim* s, double t, float dt, int t_mode, int dt_mode);   // t: 2 host value, also the simulation time; 1 host value, body only; 0 device (t_step + dt); -1 keep.  dt: 1 host, 0 device, -1 keep
 void wl_k_measure(wl_sim* s);
+void wl_body_box(const wl_sim* s, float margin, int interior, int o[3], int e[3]);
 void wl_k_bc(wl_sim* s, float* u);
 void wl_k_exit_bc(wl_sim* s, float* u, const float* u0);
 void wl_k_cfl(wl_sim* s, const float* u);

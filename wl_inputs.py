@@ -15,7 +15,7 @@ import numpy as np
 
 SEED = 20240716  # per-kernel parity inputs
 
-BODY_NONE, BODY_SPHERE, BODY_TORUS, BODY_CYLINDER = 0, 1, 2, 3
+BODY_NONE, BODY_SPHERE, BODY_TORUS, BODY_CYLINDER, BODY_PLANE = 0, 1, 2, 3, 4
 MOTION_STATIC, MOTION_SIN = 0, 1
 MOTION_HEAVE_SIN = MOTION_SIN          # one direction of the sinusoidal translation (heave_dir, amp, freq, phase)
 
@@ -27,6 +27,10 @@ CONFIG_DEFAULTS = dict(
     motion=MOTION_STATIC, heave_dir=1, amp=0.0, freq=0.0, phase=0.0,
     amp3=None, freq3=None, phase3=None,     # sinusoidal translation in every direction (overrides the four above)
     tune=None,                              # implementation switches of the CUDA library (wl_tuning), a dict
+    # general bodies: thin shell |sdf| - shell, non-rigid map xi_d = s_d(t)(x_d - c_d(t)) with
+    # s_d = 1 + scale_amp[d] cos(2 pi scale_freq t + scale_phase), spin about the axis, and further primitives combined by
+    # SDF arithmetic: parts = [dict(kind=..., centre=..., ..., op="+" | "-"), ...] (same keys as the first primitive)
+    shell=0.0, scale_amp=(0.0, 0.0, 0.0), scale_freq=0.0, scale_phase=0.0, spin=0.0, parts=None,
     max_levels=0, smooth_iters=6, max_vcycles=32, fixed_vcycles=2, tol=1e-4,
 )
 
@@ -96,6 +100,44 @@ def cylinder_2dof(L=64, Re=1000.0, **kw) -> dict:
     base = dict(ndim=3, dims=(9 * L, 6 * L, 2 * L), L=D, U=(1.0, 0.0, 0.0), nu=D / Re, periodic=(0, 0, 1), exit_bc=1,
                 body_kind=BODY_CYLINDER, axis=2, centre=(3.0 * L, 3.0 * L, 0.0), R=D / 2.0, motion=MOTION_SIN,
                 amp3=(0.4 * D, 1.6 * D, 0.0), freq3=(2.0 * f, f, 0.0), phase3=(math.pi / 6.0, 0.0, 0.0))
+    base.update(kw)
+    return make(**base)
+
+
+def jelly(p=5, Re=500.0, U=1.0, **kw) -> dict:
+    """SURVEY 8(f) NEXT-2, the pulsing jellyfish of PAPER.md:235-243: a spherical shell |  |xi| - R | - 1 under the non-rigid map
+    xi = A(t) .* x + B(t) + C(t), minus the half-space xi_3 < h under the translation x + C(t) ("body = sphere - plane"), in a
+    box n x n x 4n with n = 2^p, R = 2n/3, h = 4n - 2R, nu = U R / Re, omega = 2U/R, boundary velocity (0, 0, -U):
+        A = 1 - [1,1,0] 0.1 cos(wt),  B = [0,0,1] ((cos(wt) - 1) R/4 - h),  C = [0,0,1] sin(wt) R/4.
+    In this module's parametrisation xi_d = s_d(t)(x_d - c_d(t)): s = A, c = -(B + C) ./ A, i.e. for the sphere
+    c_z = h + R/4 - (R sqrt(2)/4) sin(wt + pi/4); for the plane c_z = -C_z... (xi_3 - h = x_3 + C_z - h): c_z = h - (R/4) sin(wt)."""
+    n = 2 ** p
+    R = 2.0 * n / 3.0
+    h = 4.0 * n - 2.0 * R
+    w = 2.0 * U / R
+    f = w / (2.0 * math.pi)
+    base = dict(ndim=3, dims=(n, n, 4 * n), L=R, U=(0.0, 0.0, -U), nu=U * R / Re, periodic=(0, 0, 0), exit_bc=0,
+                body_kind=BODY_SPHERE, centre=(0.0, 0.0, h + R / 4.0), R=R, shell=1.0, motion=MOTION_SIN,
+                amp3=(0.0, 0.0, -R * math.sqrt(2.0) / 4.0), freq3=(0.0, 0.0, f), phase3=(0.0, 0.0, math.pi / 4.0),
+                scale_amp=(-0.1, -0.1, 0.0), scale_freq=f, scale_phase=0.0,
+                parts=[dict(kind=BODY_PLANE, axis=2, centre=(0.0, 0.0, h), motion=MOTION_SIN,
+                            amp3=(0.0, 0.0, -R / 4.0), freq3=(0.0, 0.0, f), phase3=(0.0, 0.0, 0.0), op="-")])
+    base.update(kw)
+    return make(**base)
+
+
+def control_cylinders(D=32, Re=500.0, xi=3.0, **kw) -> dict:
+    """SURVEY 8(f) NEXT-2, the controlled cylinder of PAPER.md:202-210 ("body = big + small"): a circle of diameter D with a small
+    spinning circle (d/D = 0.15, gap g/D = 0.05, surface speed xi U = d Omega / 2) placed 120 degrees from the inflow
+    direction, upper half of the flow only (symmetry plane y = 0), 2-D box 6D x 2D."""
+    d, gap = 0.15 * D, 0.05 * D
+    rc = D / 2.0 + gap + d / 2.0
+    ang = math.radians(120.0)                         # measured from the upstream direction (-x)
+    cx, cy = 2.0 * D, 0.0
+    sx, sy = cx - rc * math.cos(ang), cy + rc * math.sin(ang)
+    base = dict(ndim=2, dims=(6 * D, 2 * D), L=float(D), U=(1.0, 0.0), nu=D / Re, periodic=(0, 0), exit_bc=1,
+                body_kind=BODY_SPHERE, centre=(cx, cy), R=D / 2.0,
+                parts=[dict(kind=BODY_SPHERE, centre=(sx, sy), R=d / 2.0, spin=-2.0 * xi / d, op="+")])
     base.update(kw)
     return make(**base)
 
