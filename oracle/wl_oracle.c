@@ -188,7 +188,7 @@ double wlo_kernel_mu1(double d, double eps)
  *   sdf     d0 = sdf(xi) of the primitive, g = grad_xi sdf; shell > 0: d0 <- |d0| - shell, g <- sign(d0) g;
  *   normal  grad_x d0 = J^T g = s .* g, m = |s .* g|; n = (s .* g)/m;
  *   distance d = d0/m: the first-order distance in physical space (exact for a uniformly scaled sphere: |x-c| - R/s);
- *           m < 1e-12 => n = 0, d = d0;
+ *           m < 1e-12 => n = 0, d = d0; a rigid map (every scale_amp = 0) skips the normalisation: d = d0, n = g as in R-E;
  *   velocity a material point has fixed xi: x(t) = c + xi ./ s, so V_d = dc_d/dt - (ds_d/dt / s_d)(x_d - c_d)  (= -J^-1 dmap/dt),
  *           plus spin * e_axis x (x - c) for a primitive spinning about its axis.
  * Primitives: sphere |xi| - R (circle in 2-D); torus (axis a); circular cylinder of P:121 (radius R, axis e_a, spanning a
@@ -251,14 +251,18 @@ static double part_eval(int nd, const wlo_part *p, const double *xpt, double t, 
         d0 = fabs(d0) - p->shell;
         for (int k = 0; k < 3; ++k) g[k] *= sg;
     }
-    double m = 0;
-    for (int k = 0; k < nd; ++k) { g[k] *= sc[k]; m += g[k] * g[k]; }
-    m = sqrt(m);
     nrm[0] = nrm[1] = nrm[2] = 0.0;
     double d = d0;
-    if (m >= 1e-12) {
-        d = d0 / m;
-        for (int k = 0; k < nd; ++k) nrm[k] = g[k] / m;
+    if (p->scale_amp[0] == 0.0 && p->scale_amp[1] == 0.0 && p->scale_amp[2] == 0.0) {
+        for (int k = 0; k < nd; ++k) nrm[k] = g[k];          /* rigid map: the SDF is exact, g is the unit normal (R-E) */
+    } else {
+        double m = 0;
+        for (int k = 0; k < nd; ++k) { g[k] *= sc[k]; m += g[k] * g[k]; }
+        m = sqrt(m);
+        if (m >= 1e-12) {
+            d = d0 / m;
+            for (int k = 0; k < nd; ++k) nrm[k] = g[k] / m;
+        }
     }
     vel[0] = vel[1] = vel[2] = 0.0;
     for (int k = 0; k < nd; ++k) vel[k] = cdot[k] - (sdot[k] / sc[k]) * (xpt[k] - c[k]);
