@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the B200 mom_step hot path (libwl) on BASELINE.json's workloads.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--repeats R] [--workload C2|C3|C4|C5|N1|N3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--repeats R] [--workload C2|C3|C4|C5|N1|N2|N3]
                     [--impl reference] [--no-cpu] [--no-also] [--no-tol] [--stages]
 
 One "step" is one pass of the whole hot path of SURVEY.md 8(a) through the C ABI: wl_step = measure (moving body
@@ -9,8 +9,9 @@ only) + mom_step (predictor + corrector, two multigrid projections) + the CFL re
 config.  The default workload is C4 (torus, 512x256x256 = 33.5 M cells): BASELINE.json quotes
 its metric ("ns per cell per time step (3D fp32) and achieved HBM GB/s") and its target (">= 60 % of HBM roofline on
 the >= 16 M-cell 3D cases") on the large 3-D cases; C2 (configs[1], 2 M cells) fits in the 126 MB L2 and is reported
-under "also" together with C3, C5 and the two SURVEY 8(f) workloads (N1: the paper's moving cylinder, 28.3 M cells;
-N3: its half-domain Taylor-Green vortex at 512^3, 134 M cells -- the shape of its 1.57 ns/DOF/step headline).
+under "also" together with C3, C5 and the SURVEY 8(f) workloads (N1: the paper's moving cylinder, 28.3 M cells; N2: its
+pulsing jellyfish, a composite non-rigid body, 8.4 M cells; N3: its half-domain Taylor-Green vortex at 512^3, 134 M
+cells -- the shape of its 1.57 ns/DOF/step headline).
 
 Protocol: W warm-up steps, then R (default 5) timed blocks of K steps each, every block bracketed by
 barrier + synchronize and timed with CUDA events on the simulation's stream; `value` is the MEDIAN block (min and max
@@ -49,16 +50,18 @@ sys.path.insert(0, str(ROOT))
 
 import wl_inputs as wi  # noqa: E402
 
-WORKLOADS = {"C2": 1, "C3": 2, "C4": 3, "C5": 4, "N1": 5, "N3": 6}
-NAMES = wi.WORKLOAD_NAMES + ["N1_cylinder_2dof_576x384x128", "N3_tgv_half_512"]
+WORKLOADS = {"C2": 1, "C3": 2, "C4": 3, "C5": 4, "N1": 5, "N3": 6, "N2": 7}
+NAMES = wi.WORKLOAD_NAMES + ["N1_cylinder_2dof_576x384x128", "N3_tgv_half_512", "N2_jelly_128x128x512"]
 
 
 def workload_config(k: int, scale: int = 1) -> dict:
-    """BASELINE.json configs[k] for k < 5; k = 5, 6: the SURVEY 8(f) NEXT-1 / NEXT-3 workloads."""
+    """BASELINE.json configs[k] for k < 5; k = 5, 6, 7: the SURVEY 8(f) NEXT-1 / NEXT-3 / NEXT-2 workloads."""
     if k < 5:
         return wi.baseline_config(k, scale=scale)
     if k == 5:
         return wi.cylinder_2dof(64 // scale)
+    if k == 7:
+        return wi.jelly(7 - {1: 0, 2: 1, 4: 2}[scale])
     return wi.tgv3d_half(512 // scale)
 
 
@@ -242,7 +245,7 @@ def run_reference(args) -> None:
 
 def config_dict(cfg, k, note=None) -> dict:
     d = {"workload": NAMES[k], "baseline_config_index": k if k < 5 else None, "dims": list(cfg["dims"][: cfg["ndim"]]),
-         "cells": ncells(cfg), "body": ["none", "sphere", "torus", "cylinder"][cfg["body_kind"]],
+         "cells": ncells(cfg), "body": ["none", "sphere", "torus", "cylinder", "plane"][cfg["body_kind"]] + ("+%d more" % len(cfg["parts"]) if cfg.get("parts") else ""),
          "moving_body": bool(cfg["motion"]), "nu": cfg["nu"], "dt": "CFL-adaptive, device-resident",
          "mg": {"fixed_vcycles": cfg["fixed_vcycles"], "smooth_iters": cfg["smooth_iters"]},
          "l2": "working set (>= 3 GB for C4/C5) is far larger than the 126 MB L2; no flush needed between steps"}

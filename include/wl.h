@@ -48,16 +48,28 @@ extern "C" {
  *     c_d(t) = centre[d] + amp[d] sin(2 pi freq[d] t + phase[d]),   V_d = dc_d/dt  (uniform in space),
  * which covers the heaving sphere (one non-zero amp) and the two-degree-of-freedom cylinder of P:181,
  * y = A_y sin(w t), x = A_x sin(2 w t + theta). */
-enum { WL_BODY_NONE = 0, WL_BODY_SPHERE = 1 /* circle in 2-D */, WL_BODY_TORUS = 2, WL_BODY_CYLINDER = 3 };
+enum { WL_BODY_NONE = 0, WL_BODY_SPHERE = 1 /* circle in 2-D */, WL_BODY_TORUS = 2, WL_BODY_CYLINDER = 3,
+       WL_BODY_PLANE = 4 /* half-space below the plane through `centre` with normal +e_axis */ };
 enum { WL_MOTION_STATIC = 0, WL_MOTION_SIN = 1 };
+enum { WL_OP_UNION = 0, WL_OP_DIFFERENCE = 1 };
+#define WL_MAX_EXTRA 3
 
+/* One primitive: SDF + map.  General bodies (reading R-E3 of DESIGN.md):
+ *   map       xi_d = s_d(t) (x_d - c_d(t)),  s_d(t) = 1 + scale_amp[d] cos(2 pi scale_freq t + scale_phase)   ("A(t) .* x + B(t)");
+ *   shell > 0 the body is the thin shell |sdf| - shell around the primitive's surface;
+ *   normal    J^T grad sdf / |J^T grad sdf|, distance sdf / |J^T grad sdf| when the map is non-rigid, J = diag(s);
+ *   velocity  V = -J^-1 dmap/dt = dc/dt - (ds/dt / s) .* (x - c), plus spin e_axis x (x - c) (z axis in 2-D): a body of
+ *             revolution spinning about its axis keeps its SDF, not its surface velocity. */
 typedef struct {
     int   kind;          /* WL_BODY_* */
     float centre[3];     /* c0, grid units */
     float R, r;          /* sphere / cylinder radius R; torus major R, minor r */
-    int   axis;          /* torus / cylinder axis 0..2 */
+    int   axis;          /* torus / cylinder / plane axis 0..2 */
     int   motion;        /* WL_MOTION_* */
     float amp[3], freq[3], phase[3];
+    float shell;
+    float scale_amp[3], scale_freq, scale_phase;
+    float spin;
 } wl_body;
 
 typedef struct {
@@ -98,6 +110,13 @@ typedef struct {
     wl_body body;
     wl_mg   mg;
     wl_tuning tune;
+    /* SDF arithmetic ("body = big + small", "body = sphere - plane"): the body is
+     * ((body op[0] extra[0]) op[1] extra[1]) ..., union = min of the distances, difference = max(d, -d_extra); normal and
+     * velocity are those of the primitive that decides.  With more than one primitive, a non-rigid map or spin the body
+     * velocity is a per-face field (one more array of ndim components); otherwise three scalars. */
+    int     nextra;
+    wl_body extra[WL_MAX_EXTRA];
+    int     extra_op[WL_MAX_EXTRA];   /* WL_OP_* */
 } wl_config;
 
 typedef struct wl_sim wl_sim;
@@ -185,7 +204,7 @@ int wl_dbg_coarse_prog(wl_sim* s, int n, const int* kinds, const int* levels, co
 /* Device-resident PCG scalars of a level: rho, gamma, alpha, beta, rho0, sum of r over the coupled cells (R-T2),
  * number of coupled cells, live flag.  Synchronises. */
 int wl_dbg_pcg_scalars(wl_sim* s, int level, double out[8]);
-/* Raw access to a solver array for tests: name in {"u","u0","p","mu0","mu1","L","iD","x","r"};
+/* Raw access to a solver array for tests: name in {"u","u0","p","mu0","mu1","V" (general bodies only),"L","iD","x","r"};
  * interior-sized copy into `out` (host), ncomp arrays; returns ncomp or a negative status. */
 int wl_dbg_get(wl_sim* s, const char* name, int level, float* out, size_t out_floats);
 int wl_dbg_set(wl_sim* s, const char* name, int level, const float* in, size_t in_floats);

@@ -61,6 +61,7 @@ FlowP wl_flowp(const wl_sim* s)
     P.nu = s->cfg.nu;
     for (int k = 0; k < 3; ++k) P.U[k] = s->cfg.U[k];
     P.exit_bc = s->cfg.exit_bc;
+    P.Vf = s->Vf;
     return P;
 }
 
@@ -71,13 +72,29 @@ static int config_ok(const wl_config* c)
     if (c->ndim != 2 && c->ndim != 3) return 0;
     for (int d = 0; d < c->ndim; ++d) if (c->dims[d] < 4 || c->dims[d] > 16384) return 0;
     if (!(c->nu >= 0.0f) || !(c->eps > 0.0f)) return 0;
-    if (c->body.kind < 0 || c->body.kind > 3) return 0;
-    if ((c->body.kind == WL_BODY_TORUS || c->body.kind == WL_BODY_CYLINDER) && (c->ndim != 3 || c->body.axis < 0 || c->body.axis > 2)) return 0;
-    if (c->body.motion < 0 || c->body.motion > 1) return 0;
+    if (c->nextra < 0 || c->nextra > WL_MAX_EXTRA || (c->nextra > 0 && c->body.kind == WL_BODY_NONE)) return 0;
+    for (int e = -1; e < c->nextra; ++e) {
+        const wl_body& b = e < 0 ? c->body : c->extra[e];
+        if (b.kind < (e < 0 ? 0 : 1) || b.kind > 4) return 0;
+        if ((b.kind == WL_BODY_TORUS || b.kind == WL_BODY_CYLINDER) && (c->ndim != 3 || b.axis < 0 || b.axis > 2)) return 0;
+        if (b.kind == WL_BODY_PLANE && (b.axis < 0 || b.axis >= c->ndim)) return 0;
+        if (b.motion < 0 || b.motion > 1) return 0;
+        if (e >= 0 && (c->extra_op[e] < 0 || c->extra_op[e] > 1)) return 0;
+        for (int d = 0; d < 3; ++d) if (!(fabsf(b.scale_amp[d]) < 0.9f)) return 0;     // the map must stay invertible
+    }
     if (c->tune.zc < 0 || c->tune.zc > 64 || c->tune.pk_blocks_per_sm < 0) return 0;
     if (c->exit_bc && c->periodic[0]) return 0;
     if (c->mg.smooth_iters < 1) return 0;
     return 1;
+}
+
+// the body velocity is a field rather than three scalars: several primitives, a non-rigid map, or spin (R-E3)
+static int body_general(const wl_config* c)
+{
+    if (c->body.kind == WL_BODY_NONE) return 0;
+    if (c->nextra > 0) return 1;
+    const wl_body& b = c->body;
+    return b.scale_amp[0] != 0.0f || b.scale_amp[1] != 0.0f || b.scale_amp[2] != 0.0f || b.spin != 0.0f;
 }
 
 static Grid make_grid(int nd, const int* n, const int* per)
@@ -168,6 +185,7 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
     float* p = (float*)cv.take(sc);
     float* mu0 = (float*)cv.take(sc * nd);
     float* mu1 = (float*)cv.take(sc * nd * nd);
+    float* Vf = body_general(c) ? (float*)cv.take(sc * nd) : nullptr;
     // band list: faces within eps of the body surface; a generous share of all faces (overflow falls back to a scan)
     int64_t ncell = (int64_t)dims[0][0] * dims[0][1] * dims[0][2];
     int64_t bcap = ncell * nd / 4;
@@ -179,7 +197,7 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
         s->ds = ds; s->rb.partial = partial; s->rb.counter = counter;
         s->levdev = levdev; s->pk_part = pk_part;
         for (int k = 0; k < 3; ++k) s->ubuf[k] = ub[k];
-        s->p = p; s->mu0 = mu0; s->mu1 = mu1;
+        s->p = p; s->mu0 = mu0; s->mu1 = mu1; s->Vf = Vf;
         s->band_list = band; s->band_cap = (int)bcap;
         s->nlev = nlev; s->nd = nd;
     }
@@ -345,8 +363,16 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     s->small_cmax = -1;
     s->bulk_A = !cfg->tune.no_bulk;
     s->tma_cd = !cfg->tune.no_tma_cd;
-    s->body.kind = cfg->body.kind; s->body.axis = cfg->body.axis;
-    s->body.R = cfg->body.R; s->body.r = cfg->body.r; s->body.eps = cfg->eps;
+    s->body.n = cfg->body.kind == WL_BODY_NONE ? 0 : 1 + cfg->nextra;
+    s->body.eps = cfg->eps;
+    s->body.general = body_general(cfg);
+    for (int e = 0; e < s->body.n; ++e) {
+        const wl_body& b = e == 0 ? cfg->body : cfg->extra[e - 1];
+        PartP& q = s->body.part[e];
+        q.kind = b.kind; q.axis = b.axis; q.R = b.R; q.r = b.r; q.shell = b.shell; q.spin = b.spin;
+        q.scaled = b.scale_amp[0] != 0.0f || b.scale_amp[1] != 0.0f || b.scale_amp[2] != 0.0f;
+        q.op = e == 0 ? 0 : cfg->extra_op[e - 1];
+    }
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
@@ -681,6 +707,7 @@ static int find_array(wl_sim* s, const char* name, int level, float** arr, int* 
     if (!strcmp(name, "p")) { *arr = s->p; return WL_OK; }
     if (!strcmp(name, "mu0")) { *arr = s->mu0; *ncomp = s->nd; return WL_OK; }
     if (!strcmp(name, "mu1")) { *arr = s->mu1; *ncomp = s->nd * s->nd; return WL_OK; }
+    if (!strcmp(name, "V") && s->Vf) { *arr = s->Vf; *ncomp = s->nd; return WL_OK; }
     return WL_EINVAL;
 }
 static int dbg_get(wl_sim* s, const char* name, int level, float* out, size_t out_floats, int whole)

@@ -5,17 +5,29 @@
 #pragma once
 #include "wl_common.cuh"
 
-struct BodyP {
-    int kind;        // WL_BODY_*
-    int axis;        // torus / cylinder axis
-    float R, r;      // sphere / cylinder radius R; torus major R / minor r
-    float eps;       // BDIM kernel half-width
-};
-
 #define WLB_NONE 0
 #define WLB_SPHERE 1
 #define WLB_TORUS 2
 #define WLB_CYLINDER 3
+#define WLB_PLANE 4
+#define WLB_MAXPART 4
+
+// static description of one primitive of the body (the time-dependent part of its map lives in DevScal: PartState)
+struct PartP {
+    int kind;        // WL_BODY_*
+    int axis;        // torus / cylinder / plane axis
+    float R, r;      // sphere / cylinder radius R; torus major R / minor r
+    float shell;     // > 0: thin shell |sdf| - shell
+    float spin;      // angular velocity about the axis through the centre
+    int scaled;      // the map has a non-rigid part (some scale_amp != 0): first-order distance d0 / |J^T grad sdf|
+    int op;          // 0 union, 1 difference (with the body built from the primitives before it)
+};
+struct BodyP {
+    int n;           // primitives (0: no body)
+    PartP part[WLB_MAXPART];
+    float eps;       // BDIM kernel half-width
+    int general;     // the body velocity is a field (several primitives, a non-rigid map or spin): V array instead of three scalars
+};
 
 // cosine kernel K(s) = (1 + cos(pi s/eps)) / (2 eps) on |s| < eps
 __device__ __forceinline__ float bdim_K(float s, float eps)
@@ -50,11 +62,11 @@ __device__ __forceinline__ float bdim_mu1(float d, float eps)
     return eps * (0.25f - 0.25f * a * a - (a * sp + (1.0f + cp) * 0.3183098861837907f) * 0.15915494309189535f);
 }
 
-// Signed distance and unit normal at body-frame position xi (translation map: J = I).  T = double in measure!
-// (a face 100 cells from the origin carries 6e-6 of fp32 round-off in its position, which mu0's slope 1/2eps turns
-// into 3e-6 of mu0: evaluated in fp64 and rounded once, d is good to 6e-8), T = float elsewhere.
+// Signed distance and its gradient at body-frame position xi for one primitive.  T = double in measure! (a face 100 cells
+// from the origin carries 6e-6 of fp32 round-off in its position, which mu0's slope 1/2eps turns into 3e-6 of mu0:
+// evaluated in fp64 and rounded once, d is good to 6e-8), T = float elsewhere.
 template <int ND, class T>
-__device__ __forceinline__ T body_sdf(const BodyP& b, const T (&xi)[3], T (&nrm)[3])
+__device__ __forceinline__ T prim_sdf(const PartP& b, const T (&xi)[3], T (&nrm)[3])
 {
     nrm[0] = nrm[1] = nrm[2] = T(0);
     const T tiny = T(1e-12);
@@ -69,6 +81,10 @@ __device__ __forceinline__ T body_sdf(const BodyP& b, const T (&xi)[3], T (&nrm)
             for (int k = 0; k < ND; ++k) nrm[k] = xi[k] * inv;
         }
         return rr - (T)b.R;
+    }
+    if (b.kind == WLB_PLANE) {             // half-space below the plane through the centre, normal +e_axis
+        nrm[b.axis] = T(1);
+        return xi[b.axis];
     }
     // torus and cylinder: axis a, rho = distance from the axis
     T xa, xb, xc;
@@ -97,4 +113,67 @@ __device__ __forceinline__ T body_sdf(const BodyP& b, const T (&xi)[3], T (&nrm)
     else if (b.axis == 1) { nrm[1] = na; nrm[2] = nb; nrm[0] = nc; }
     else { nrm[2] = na; nrm[0] = nb; nrm[1] = nc; }
     return gq - (T)b.r;
+}
+
+// The whole body at the point x (absolute grid coordinates), reading R-E3: for every primitive the map xi = s .* (x - c),
+// the primitive's SDF (shell: |d0| - shell), normal J^T grad / |.| and first-order distance d0 / |J^T grad| when the map is
+// non-rigid, velocity dc/dt - (ds/dt / s)(x - c) + spin e_a x (x - c); union = min, difference = max(d, -d_B), normal and
+// velocity from the primitive that decides.  Returns d; fills nrm and vel.
+template <int ND, class T>
+__device__ __forceinline__ T body_eval(const BodyP& B, const PartState* __restrict__ st, const double (&x)[3], T (&nrm)[3], float (&vel)[3])
+{
+    T d = T(1e30);
+    nrm[0] = nrm[1] = nrm[2] = T(0);
+    vel[0] = vel[1] = vel[2] = 0.0f;
+    for (int e = 0; e < B.n; ++e) {
+        const PartP& p = B.part[e];
+        const PartState& q = st[e];
+        T xi[3] = { T(0), T(0), T(0) }, g[3];
+        double rel[3] = { 0.0, 0.0, 0.0 };
+#pragma unroll
+        for (int k = 0; k < ND; ++k) { rel[k] = x[k] - q.c[k]; xi[k] = (T)(q.s[k] * rel[k]); }
+        T d0 = prim_sdf<ND, T>(p, xi, g);
+        if (p.shell > 0.0f) {
+            const T sg = d0 < T(0) ? T(-1) : T(1);
+            d0 = fabs(d0) - (T)p.shell;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) g[k] *= sg;
+        }
+        if (p.scaled) {
+            T m = T(0);
+#pragma unroll
+            for (int k = 0; k < ND; ++k) { g[k] *= (T)q.s[k]; m += g[k] * g[k]; }
+            m = sqrt(m);
+            if (m >= T(1e-12)) {
+                const T im = T(1) / m;
+                d0 *= im;
+#pragma unroll
+                for (int k = 0; k < ND; ++k) g[k] *= im;
+            } else {
+                g[0] = g[1] = g[2] = T(0);
+            }
+        }
+        if (p.op == 1) {
+            d0 = -d0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) g[k] = -g[k];
+        }
+        const bool take = e == 0 || (p.op == 1 ? d0 > d : d0 < d);
+        if (take) {
+            d = d0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) nrm[k] = g[k];
+            float v[3] = { 0.f, 0.f, 0.f };
+#pragma unroll
+            for (int k = 0; k < ND; ++k) v[k] = (float)((double)q.cdot[k] - (double)q.sdot_s[k] * rel[k]);
+            if (p.spin != 0.0f) {
+                const int a = ND == 3 ? p.axis : 2, b1 = (a + 1) % 3, c1 = (a + 2) % 3;
+                if (b1 < ND) v[b1] += (float)(-(double)p.spin * rel[c1]);
+                if (c1 < ND) v[c1] += (float)((double)p.spin * rel[b1]);
+            }
+#pragma unroll
+            for (int k = 0; k < 3; ++k) vel[k] = v[k];
+        }
+    }
+    return d;
 }

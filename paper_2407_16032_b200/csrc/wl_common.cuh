@@ -52,12 +52,20 @@ struct PcgScal {
     int stop_k; // one-sweep form (wl_pcgfused.cu): the iteration whose stopping criterion fired with its update still owed (0: none)
 };
 
+// time-dependent state of the map of one primitive of the body: xi = s .* (x - c)  (k_set_time)
+struct PartState {
+    double c[3];         // centre at the time the body was last placed
+    double s[3];         // diagonal of the map
+    double cdot[3];      // dc/dt
+    double sdot_s[3];    // (ds/dt) / s
+};
+
 struct DevScal {
     PcgScal pcg[WL_MAXLEV];
     double t;            // time at which the body was last placed (measure!)
     double t_step;       // simulation time advanced by wl_step (never touched by wl_measure / wl_pressure_force)
-    double centre[3];    // body centre at time t
-    double centre_f[3];  // body centre the pressure-force integral is taken at
+    PartState part[4];   // the primitives of the body at time t
+    PartState part_f[4]; // ... at the time the pressure-force integral is taken at
     float  vel[3];       // body velocity V (rigid translation: uniform)
     float  dt;           // time step of the running step
     float  dt_next;      // CFL result

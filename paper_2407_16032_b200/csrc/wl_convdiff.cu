@@ -131,7 +131,9 @@ __device__ float f_at(const FlowP& P, const float* __restrict__ w, const float* 
         S.set(g, c[0], c[1], c[2]);
         r = rhs_comp<ND, I>(P, w, S);
     }
-    return u0[I * g.nalloc + gidx(g, c[0], c[1], c[2])] + dt * r - Vi;
+    const int64_t id = gidx(g, c[0], c[1], c[2]);
+    if (P.Vf) Vi = P.Vf[I * g.nalloc + id];          // a general body: V at THIS face
+    return u0[I * g.nalloc + id] + dt * r - Vi;
 }
 
 
@@ -381,12 +383,15 @@ __device__ __forceinline__ void cd2_output(const FlowP& P, int gx, int gy, int g
         for (int k = 0; k < 4; ++k) uu[k] = q.wc[k];
     }
 #pragma unroll
+    float vv[4] = { Vi, Vi, Vi, Vi };
+    if (P.Vf) unpack4(ld4(P.Vf + I * g.nalloc, id), vv);      // a general body: V is a field
+#pragma unroll
     for (int k = 0; k < 4; ++k) {
         float r = q.rx[k];
         r += q.fyl[k] - fyu[k];
         if (ND == 3) r += q.fzd[k];
-        const float f = uu[k] + dt * r - Vi;
-        const float B = Vi + mm[k] * f;
+        const float f = uu[k] + dt * r - vv[k];
+        const float B = vv[k] + mm[k] * f;
         o[k] = corrector ? 0.5f * (q.wc[k] + B) : B;
     }
     st4(out + I * g.nalloc, id, o, nv);

@@ -2,6 +2,7 @@
 // exit, CFL reduction, pressure force, initial conditions, pack/unpack of user buffers.
 // Citations "P:<line>" are /root/reference/PAPER.md; "R-<x>" are the readings of DESIGN.md s.3.
 #include <cstdio>
+#include <cstring>
 #include "wl_internal.h"
 
 // ------------------------------------------------------------------ time / body state
@@ -10,22 +11,27 @@
 //     c_d(t) = c0_d + amp_d sin(2 pi f_d t + phase_d),  V = dc/dt
 // Modes: see wl_internal.h.  The simulation time t_step moves only with wl_step (t_mode 2 and 0), so a wl_measure or
 // wl_pressure_force at some other time cannot shift the trajectory of a device-resident run.
-__device__ __forceinline__ void body_place(const wl_body& b, double t, double (&c)[3], float (&v)[3])
+struct BodyAll { int n; wl_body part[WLB_MAXPART]; };     // every primitive's map parameters (kernel argument)
+
+__device__ __forceinline__ void body_place(const wl_body& b, double t, PartState& q)
 {
     const double two_pi = 6.283185307179586476925286766559;
+    const double phs = two_pi * (double)b.scale_freq * t + (double)b.scale_phase;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        c[k] = (double)b.centre[k];
-        v[k] = 0.f;
+        q.c[k] = (double)b.centre[k];
+        q.cdot[k] = 0.0;
         if (b.motion == WL_MOTION_SIN) {
             const double ph = two_pi * (double)b.freq[k] * t + (double)b.phase[k];
-            c[k] += (double)b.amp[k] * sin(ph);
-            v[k] = (float)((double)b.amp[k] * two_pi * (double)b.freq[k] * cos(ph));
+            q.c[k] += (double)b.amp[k] * sin(ph);
+            q.cdot[k] = (double)b.amp[k] * two_pi * (double)b.freq[k] * cos(ph);
         }
+        q.s[k] = 1.0 + (double)b.scale_amp[k] * cos(phs);
+        q.sdot_s[k] = -(double)b.scale_amp[k] * two_pi * (double)b.scale_freq * sin(phs) / q.s[k];
     }
 }
 
-__global__ void k_set_time(DevScal* ds, wl_body b, double t_host, float dt_host, int t_mode, int dt_mode)
+__global__ void k_set_time(DevScal* ds, BodyAll B, double t_host, float dt_host, int t_mode, int dt_mode)
 {
     if (dt_mode == 1) ds->dt = dt_host; else if (dt_mode == 0) ds->dt = ds->dt_next;
     double t = ds->t;
@@ -33,18 +39,17 @@ __global__ void k_set_time(DevScal* ds, wl_body b, double t_host, float dt_host,
     else if (t_mode == 1) t = t_host;
     else if (t_mode == 0) { t = ds->t_step + (double)ds->dt; ds->t_step = t; }
     ds->t = t;
-    double c[3]; float v[3];
-    body_place(b, t, c, v);
-    for (int k = 0; k < 3; ++k) { ds->centre[k] = c[k]; ds->vel[k] = v[k]; }
+    for (int e = 0; e < B.n; ++e) body_place(B.part[e], t, ds->part[e]);
+    for (int k = 0; k < 3; ++k) ds->vel[k] = B.n > 0 ? (float)ds->part[0].cdot[k] : 0.0f;     // one rigid translation: V is uniform
 }
 
-// body centre for the pressure-force integral: at the host time t, or (t = NaN) where measure! last placed the body
-__global__ void k_force_time(DevScal* ds, wl_body b, double t_host)
+// the body for the pressure-force integral: at the host time t, or (t = NaN) where measure! last placed it
+__global__ void k_force_time(DevScal* ds, BodyAll B, double t_host)
 {
-    double c[3]; float v[3];
-    if (t_host == t_host) body_place(b, t_host, c, v);
-    else for (int k = 0; k < 3; ++k) c[k] = ds->centre[k];
-    for (int k = 0; k < 3; ++k) ds->centre_f[k] = c[k];
+    for (int e = 0; e < B.n; ++e) {
+        if (t_host == t_host) body_place(B.part[e], t_host, ds->part_f[e]);
+        else ds->part_f[e] = ds->part[e];
+    }
 }
 
 // ------------------------------------------------------------------ measure!
@@ -55,10 +60,9 @@ __global__ void k_force_time(DevScal* ds, wl_body b, double t_host)
 // problem).  V is a uniform vector for the translation maps supported and lives in DevScal.
 template <int ND>
 __global__ void __launch_bounds__(512) k_measure(Grid g, Tiling T, BodyP b, const DevScal* __restrict__ ds,
-                                                 float* __restrict__ mu0, float* __restrict__ mu1,
+                                                 float* __restrict__ mu0, float* __restrict__ mu1, float* __restrict__ Vf,
                                                  DevScal* dsw, long long* __restrict__ band, int band_cap)
 {
-    double ctr[3] = { ds->centre[0], ds->centre[1], ds->centre[2] };
     for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
         int c[3];
         if (!tile_cell(T, tile, c[0], c[1], c[2])) continue;
@@ -68,15 +72,12 @@ __global__ void __launch_bounds__(512) k_measure(Grid g, Tiling T, BodyP b, cons
         for (int k = 0; k < 3; ++k) xc[k] = k < ND ? (float)wrapc(c[k], g.n[k], g.per[k]) - 0.5f : 0.0f;
 #pragma unroll
         for (int i = 0; i < ND; ++i) {
-            float m0 = 1.0f, m1 = 0.0f, nrm[3] = { 0.f, 0.f, 0.f };
-            if (b.kind != WLB_NONE) {
-                double xi[3], nd[3];
+            float m0 = 1.0f, m1 = 0.0f, nrm[3] = { 0.f, 0.f, 0.f }, vel[3] = { 0.f, 0.f, 0.f };
+            if (b.n > 0) {
+                double xf[3], nd[3];
 #pragma unroll
-                for (int k = 0; k < 3; ++k) {
-                    double xf = (double)xc[k] - (k == i ? 0.5 : 0.0);
-                    xi[k] = k < ND ? xf - ctr[k] : 0.0;
-                }
-                const float d = (float)body_sdf<ND, double>(b, xi, nd);
+                for (int k = 0; k < 3; ++k) xf[k] = k < ND ? (double)xc[k] - (k == i ? 0.5 : 0.0) : 0.0;
+                const float d = (float)body_eval<ND, double>(b, ds->part, xf, nd, vel);
 #pragma unroll
                 for (int k = 0; k < 3; ++k) nrm[k] = (float)nd[k];
                 m0 = bdim_mu0(d, b.eps);
@@ -84,6 +85,7 @@ __global__ void __launch_bounds__(512) k_measure(Grid g, Tiling T, BodyP b, cons
             }
             if (!g.per[i] && (c[i] == 1 || c[i] == g.n[i] + 1)) m0 = 0.0f;
             mu0[i * g.nalloc + id] = m0;
+            if (Vf) Vf[i * g.nalloc + id] = vel[i];
             bool any = false;
 #pragma unroll
             for (int j = 0; j < ND; ++j) {
@@ -255,16 +257,16 @@ __global__ void __launch_bounds__(WL_VB) k_cfl(Grid g, VT vt, const float* __res
 template <int ND>
 __global__ void __launch_bounds__(512) k_force(Grid g, Tiling T, BodyP b, const float* __restrict__ p, DevScal* ds, RedBuf rb)
 {
-    double ctr[3] = { ds->centre_f[0], ds->centre_f[1], ds->centre_f[2] };
     double v[3] = { 0.0, 0.0, 0.0 };
-    if (b.kind != WLB_NONE) {
+    if (b.n > 0) {
         for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
             int c[3];
             if (!tile_cell(T, tile, c[0], c[1], c[2])) continue;
-            float xi[3], nrm[3];
+            double xc[3];
+            float nrm[3], vel[3];
 #pragma unroll
-            for (int k = 0; k < 3; ++k) xi[k] = k < ND ? (float)(((double)c[k] - 0.5) - ctr[k]) : 0.0f;
-            float d = body_sdf<ND, float>(b, xi, nrm);
+            for (int k = 0; k < 3; ++k) xc[k] = k < ND ? (double)c[k] - 0.5 : 0.0;
+            float d = body_eval<ND, float>(b, ds->part_f, xc, nrm, vel);
             float kk = bdim_K(d, 1.0f);
             if (kk == 0.0f) continue;
             float pk = p[gidx(g, c[0], c[1], c[2])] * kk;
@@ -381,10 +383,21 @@ __global__ void __launch_bounds__(512) k_unpack(Grid g, Tiling T, const float* _
 
 // ================================================================== host launchers
 
+static BodyAll body_all(const wl_sim* s)
+{
+    BodyAll B;
+    memset(&B, 0, sizeof(B));
+    if (s->cfg.body.kind == WL_BODY_NONE) return B;
+    B.n = 1 + s->cfg.nextra;
+    B.part[0] = s->cfg.body;
+    for (int e = 0; e < s->cfg.nextra; ++e) B.part[1 + e] = s->cfg.extra[e];
+    return B;
+}
+
 void wl_k_set_time(wl_sim* s, double t, float dt, int t_mode, int dt_mode)
 {
     ProfScope ps(s, WLK_SET_TIME);
-    k_set_time<<<1, 1, 0, s->st>>>(s->ds, s->cfg.body, t, dt, t_mode, dt_mode);
+    k_set_time<<<1, 1, 0, s->st>>>(s->ds, body_all(s), t, dt, t_mode, dt_mode);
 }
 
 // The box of padded cells the body can reach, grown by `margin` cells: the supported motion is a sinusoidal translation of
@@ -418,7 +431,7 @@ void wl_k_measure(wl_sim* s)
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_padded(s, g);
     const wl_body& b = s->cfg.body;
-    if (s->measured && b.kind != WL_BODY_NONE) {
+    if (s->measured && b.kind != WL_BODY_NONE && !s->body.general) {      // a general body: the whole grid every time
         int o[3], e[3];
         wl_body_box(s, s->cfg.eps + 2.0f, 0, o, e);                   // the face positions are half a cell off the centres
         T = wl_tiling(s->nd, o, e);
@@ -428,8 +441,8 @@ void wl_k_measure(wl_sim* s)
     cudaMemsetAsync(&s->ds->band_count, 0, sizeof(int), s->st);
     {
         ProfScope ps(s, WLK_MEASURE);
-        if (s->nd == 3) k_measure<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1, s->ds, s->band_list, s->band_cap);
-        else            k_measure<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1, s->ds, s->band_list, s->band_cap);
+        if (s->nd == 3) k_measure<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1, s->Vf, s->ds, s->band_list, s->band_cap);
+        else            k_measure<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1, s->Vf, s->ds, s->band_list, s->band_cap);
     }
     wl_k_poisson_update(s);
 }
@@ -488,14 +501,14 @@ void wl_k_force(wl_sim* s, double t)
 {
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_interior(s, g);
-    if (s->cfg.body.kind != WL_BODY_NONE) {          // K(d) vanishes further than one cell from the surface: the body's box is enough
+    if (s->cfg.body.kind != WL_BODY_NONE && !s->body.general) {      // K(d) vanishes further than one cell from the surface: the body's box is enough
         int o[3], e[3];
         wl_body_box(s, 3.0f, 1, o, e);
         T = wl_tiling(s->nd, o, e);
     }
     {
         ProfScope ps(s, WLK_SET_TIME);
-        k_force_time<<<1, 1, 0, s->st>>>(s->ds, s->cfg.body, t);
+        k_force_time<<<1, 1, 0, s->st>>>(s->ds, body_all(s), t);
     }
     ProfScope ps(s, WLK_FORCE);
     if (s->nd == 3) k_force<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->p, s->ds, s->rb);

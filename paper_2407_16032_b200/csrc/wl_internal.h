@@ -56,6 +56,7 @@ struct wl_sim {
     float* p;                // pressure (unscaled)
     float* mu0;              // nd comps
     float* mu1;              // nd*nd comps
+    float* Vf;               // body velocity per face (nd comps) when the body is general (BodyP::general), else null: V is ds->vel
     long long* band_list;    // faces with mu1 != 0, written by measure!: (array offset << 2) | component
     int band_cap;            // capacity of band_list (entries)
     int cd_attr_set;         // dynamic shared-memory attributes set: bits 2, 4 conv_diff kernels, 16 k_pcg_fused
@@ -117,6 +118,7 @@ struct FlowP {
     float nu;
     float U[3];
     int exit_bc;
+    const float* Vf;   // body velocity per face (general bodies), or null: uniform V from DevScal
 };
 
 // launch geometry

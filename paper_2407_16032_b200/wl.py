@@ -15,7 +15,7 @@ import numpy as np
 
 from . import build as _build
 
-BODY_NONE, BODY_SPHERE, BODY_TORUS, BODY_CYLINDER = 0, 1, 2, 3
+BODY_NONE, BODY_SPHERE, BODY_TORUS, BODY_CYLINDER, BODY_PLANE = 0, 1, 2, 3, 4
 MOTION_STATIC, MOTION_SIN = 0, 1
 WL_OK, WL_EINVAL, WL_ENOMEM, WL_ECUDA, WL_ENOCONV = 0, -1, -2, -3, -4
 
@@ -33,7 +33,9 @@ EXPORTS = [
 class Body(C.Structure):
     _fields_ = [("kind", C.c_int), ("centre", C.c_float * 3), ("R", C.c_float), ("r", C.c_float),
                 ("axis", C.c_int), ("motion", C.c_int),
-                ("amp", C.c_float * 3), ("freq", C.c_float * 3), ("phase", C.c_float * 3)]
+                ("amp", C.c_float * 3), ("freq", C.c_float * 3), ("phase", C.c_float * 3),
+                ("shell", C.c_float), ("scale_amp", C.c_float * 3), ("scale_freq", C.c_float), ("scale_phase", C.c_float),
+                ("spin", C.c_float)]
 
 
 class MG(C.Structure):
@@ -50,7 +52,8 @@ class Config(C.Structure):
     _fields_ = [("ndim", C.c_int), ("dims", C.c_int * 3), ("L", C.c_float), ("U", C.c_float * 3),
                 ("nu", C.c_float), ("periodic", C.c_int * 3), ("exit_bc", C.c_int), ("eps", C.c_float),
                 ("dt0", C.c_float), ("dt_max", C.c_float), ("cfl_c", C.c_float), ("cfl_cnu", C.c_float),
-                ("body", Body), ("mg", MG), ("tune", Tuning)]
+                ("body", Body), ("mg", MG), ("tune", Tuning),
+                ("nextra", C.c_int), ("extra", Body * 3), ("extra_op", C.c_int * 3)]
 
 
 class Stats(C.Structure):
@@ -114,6 +117,25 @@ def load(build_if_missing: bool = True):
     return L
 
 
+def _fill_body(b: Body, d: dict) -> None:
+    """one primitive (wl_body) from a plain dict; missing keys take the defaults of wl_inputs.CONFIG_DEFAULTS"""
+    b.kind = int(d["kind"])
+    ctr = d.get("centre", (0.0, 0.0, 0.0))
+    for k in range(3):
+        b.centre[k] = float(ctr[k]) if k < len(ctr) else 0.0
+        b.scale_amp[k] = float((d.get("scale_amp") or (0.0, 0.0, 0.0))[k])
+    b.R, b.r, b.axis, b.motion = float(d.get("R", 0.0)), float(d.get("r", 0.0)), int(d.get("axis", 0)), int(d.get("motion", MOTION_STATIC))
+    # sinusoidal translation: three-vectors amp3 / freq3 / phase3, or the scalars amp / freq / phase along heave_dir
+    if d.get("amp3") is not None:
+        for k in range(3):
+            b.amp[k], b.freq[k], b.phase[k] = float(d["amp3"][k]), float(d["freq3"][k]), float(d["phase3"][k])
+    else:
+        k = int(d.get("heave_dir", 1))
+        b.amp[k], b.freq[k], b.phase[k] = float(d.get("amp", 0.0)), float(d.get("freq", 0.0)), float(d.get("phase", 0.0))
+    b.shell, b.scale_freq, b.scale_phase = float(d.get("shell", 0.0)), float(d.get("scale_freq", 0.0)), float(d.get("scale_phase", 0.0))
+    b.spin = float(d.get("spin", 0.0))
+
+
 def make_config(cfg: dict) -> Config:
     """Plain dict (wl_inputs.make) -> wl_config."""
     c = Config()
@@ -127,18 +149,12 @@ def make_config(cfg: dict) -> Config:
     for k in ("L", "nu", "eps", "dt0", "dt_max", "cfl_c", "cfl_cnu"):
         setattr(c, k, float(cfg[k]))
     c.exit_bc = int(cfg["exit_bc"])
-    c.body.kind = int(cfg["body_kind"])
-    for k in ("R", "r"):
-        setattr(c.body, k, float(cfg[k]))
-    for k in ("axis", "motion"):
-        setattr(c.body, k, int(cfg[k]))
-    # sinusoidal translation: three-vectors amp3 / freq3 / phase3, or the scalars amp / freq / phase along heave_dir
-    if cfg.get("amp3") is not None:
-        for d in range(3):
-            c.body.amp[d], c.body.freq[d], c.body.phase[d] = float(cfg["amp3"][d]), float(cfg["freq3"][d]), float(cfg["phase3"][d])
-    else:
-        d = int(cfg["heave_dir"])
-        c.body.amp[d], c.body.freq[d], c.body.phase[d] = float(cfg["amp"]), float(cfg["freq"]), float(cfg["phase"])
+    _fill_body(c.body, dict(cfg, kind=cfg["body_kind"]))
+    parts = cfg.get("parts") or []
+    c.nextra = len(parts)
+    for e, pd in enumerate(parts):
+        _fill_body(c.extra[e], pd)
+        c.extra_op[e] = 1 if pd.get("op", "+") == "-" else 0
     for k in ("max_levels", "smooth_iters", "max_vcycles", "fixed_vcycles"):
         setattr(c.mg, k, int(cfg[k]))
     c.mg.tol = float(cfg["tol"])
@@ -310,7 +326,7 @@ class Sim:
         ld = self.level_dims(level if name in ("L", "iD", "x", "r", "e", "q") else 0)
         if padded:
             ld = tuple(n + 2 for n in ld)
-        ncomp = {"u": self.nd, "u0": self.nd, "mu0": self.nd, "L": self.nd, "mu1": self.nd * self.nd}.get(name, 1)
+        ncomp = {"u": self.nd, "u0": self.nd, "mu0": self.nd, "L": self.nd, "V": self.nd, "mu1": self.nd * self.nd}.get(name, 1)
         out = np.empty((ncomp,) + tuple(reversed(ld)), dtype=np.float32)
         fn = self._L.wl_dbg_get_padded if padded else self._L.wl_dbg_get
         self._chk(fn(self._h, name.encode(), int(level), C.c_void_p(out.ctypes.data), C.c_size_t(out.size)))

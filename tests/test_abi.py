@@ -32,11 +32,14 @@ def test_library_exports_every_declared_symbol():
 def test_config_struct_layout_matches_header():
     """The ctypes mirror must have the C layout: all members are 4-byte scalars, no padding."""
     from paper_2407_16032_b200 import wl
-    assert C.sizeof(wl.Body) == 4 * (1 + 3 + 2 + 1 + 1 + 9)
+    assert C.sizeof(wl.Body) == 4 * (1 + 3 + 2 + 1 + 1 + 9 + 1 + 5 + 1)
     assert C.sizeof(wl.MG) == 4 * 5
     assert C.sizeof(wl.Tuning) == 4 * 6 + 8 + 8              # six ints, one long long (8-aligned), one int + tail padding
     head = 4 * (1 + 3 + 1 + 3 + 1 + 3 + 1 + 1 + 4) + C.sizeof(wl.Body) + C.sizeof(wl.MG)
-    assert wl.Config.tune.offset == (head + 7) // 8 * 8 and C.sizeof(wl.Config) == wl.Config.tune.offset + C.sizeof(wl.Tuning)
+    assert wl.Config.tune.offset == (head + 7) // 8 * 8
+    tail = 4 + 3 * C.sizeof(wl.Body) + 4 * 3                  # nextra, extra[3], extra_op[3]
+    assert wl.Config.nextra.offset == wl.Config.tune.offset + C.sizeof(wl.Tuning)
+    assert C.sizeof(wl.Config) == (wl.Config.nextra.offset + tail + 7) // 8 * 8
 
 
 def test_workspace_bytes_is_pure_and_sane():

@@ -46,6 +46,16 @@ def _body(kind, dims, moving=False):
     c = tuple(0.45 * n + 0.3 for n in dims)          # off-lattice centre
     if kind == "none":
         return {}
+    if kind == "jelly":              # shell under a pulsing non-rigid map, minus a heaving half-space
+        R = 0.3 * min(dims[:2])
+        return dict(body_kind=wi.BODY_SPHERE, centre=c, R=R, shell=1.0, motion=wi.MOTION_SIN, amp3=(0.0, 0.0, 0.1 * R),
+                    freq3=(0.0, 0.0, 0.02), phase3=(0.0, 0.0, 0.7), scale_amp=(-0.1, -0.1, 0.0), scale_freq=0.02, scale_phase=0.0,
+                    parts=[dict(kind=wi.BODY_PLANE, axis=2, centre=(0.0, 0.0, c[2] - 0.2 * R), motion=wi.MOTION_SIN,
+                                amp3=(0.0, 0.0, -0.05 * R), freq3=(0.0, 0.0, 0.02), phase3=(0.0, 0.0, 0.0), op="-")])
+    if kind == "control":            # big circle + small spinning circle, 2-D
+        D = 0.4 * dims[1]
+        return dict(body_kind=wi.BODY_SPHERE, centre=c, R=D / 2,
+                    parts=[dict(kind=wi.BODY_SPHERE, centre=(c[0] + 0.35 * D, c[1] + 0.6 * D), R=0.075 * D, spin=-3.0 / (0.075 * D), op="+")])
     if kind == "sphere":
         kw = dict(body_kind=wi.BODY_SPHERE, centre=c, R=0.22 * min(dims))
     elif kind == "cylinder":         # spanning z, two-degree-of-freedom motion when moving
@@ -79,6 +89,10 @@ CASES = [
     # circular cylinder spanning the periodic z direction, static and with the 2-DOF motion
     ((48, 32, 16), (0, 0, 1), 1, "cylinder", False),
     ((160, 48, 24), (0, 0, 1), 1, "cylinder", True),
+    # general bodies (the body velocity is a field)
+    ((32, 32, 48), (0, 0, 0), 0, "jelly", True),
+    ((136, 40, 40), (0, 0, 0), 1, "jelly", True),
+    ((96, 64), (0, 0), 1, "control", False),
 ]
 
 
@@ -116,6 +130,9 @@ def test_measure_and_poisson_coefficients(case):
         m1o = O(o, "mu1", padded=True)
         m1g = g.dbg_get("mu1", padded=True)
         assert np.abs(m1g - m1o).max() <= TOL * max(1.0, np.abs(m1o).max())
+        if case[3] in ("jelly", "control"):              # a general body: V is a per-face field
+            Vo = O(o, "V", padded=True)
+            assert np.abs(g.dbg_get("V", padded=True) - Vo).max() <= TOL * np.abs(Vo).max()
         for l in range(o.nlevels):
             assert g.level_dims(l) == tuple(O(o, "iD", l).shape[1:][::-1])
             assert relerr(g.dbg_get("L", l), O(o, "L", l)) <= TOL

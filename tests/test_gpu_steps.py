@@ -65,6 +65,10 @@ SCALED = [
     ("N1_cylinder_2dof_72x48x16", lambda: wi.cylinder_2dof(8), dict()),
     # the half-domain Taylor-Green vortex between symmetry planes, 32^3
     ("N3_tgv_half_32", lambda: wi.tgv3d_half(32), dict(tgv=True)),
+    # the pulsing jellyfish (sphere shell under A(t).*x + B(t), minus a plane) at p = 4 (16 x 16 x 64) and the
+    # big + small spinning circle pair at D = 16 (96 x 32)
+    ("N2_jelly_16x16x64", lambda: wi.jelly(4), dict()),
+    ("N2_control_cylinders_96x32", lambda: wi.control_cylinders(16), dict()),
     ("2D_cylinder_exit_96x64", lambda: wi.make(ndim=2, dims=(96, 64), exit_bc=1, nu=0.05, body_kind=wi.BODY_SPHERE,
                                                centre=(24.3, 32.2), R=6.0), dict()),
 ]
@@ -151,6 +155,17 @@ def test_force_and_power_two_dof_cylinder_50_steps():
     sc = np.abs(Fo[5:]).max()
     assert np.abs(Fg[5:] - Fo[5:]).max() <= 1e-3 * sc
     assert np.abs(Fg[:, 2]).max() <= 1e-3 * sc         # nothing along the span
+    o.close(); g.close()
+
+
+def test_force_jelly_50_steps():
+    """force on the composite, non-rigid body over 50 steps (p = 4), the thrust component along z"""
+    cfg = wi.jelly(4)
+    o, g = _sims(cfg)
+    t, F = _run(o, g, cfg, 50, force=True)
+    Fo, Fg = np.array([a for a, b in F]), np.array([b for a, b in F])
+    sc = np.abs(Fo[5:]).max()
+    assert np.abs(Fg[5:] - Fo[5:]).max() <= 1e-3 * sc
     o.close(); g.close()
 
 
