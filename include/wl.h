@@ -117,7 +117,20 @@ typedef struct {
     int     nextra;
     wl_body extra[WL_MAX_EXTRA];
     int     extra_op[WL_MAX_EXTRA];   /* WL_OP_* */
+    /* Scalar type of the simulation ("T=Float32"; "T = Dual"):
+     *   precision = 0        fp32, the tuned kernels (the hot path this library is about);
+     *   precision = 1        fp64, through the generic engine (one plain kernel per stage, same algorithm);
+     *   tangent_param != 0   forward-mode tangent: every kernel of the step carries d/d(theta) beside the value (fp64 dual
+     *                        numbers, generic engine), theta = the parameter named by WL_SEED_* (tangent_index: the direction
+     *                        for U / AMP / CENTRE, the primitive 0..nextra for SPIN).  dt is taken as independent of theta.
+     * The generic engine supports every entry point except the wl_dbg_* stage hooks and wl_prof_*; wl_step's device-resident
+     * dt becomes a host round trip per step. */
+    int     precision;
+    int     tangent_param;
+    int     tangent_index;
 } wl_config;
+
+enum { WL_SEED_NONE = 0, WL_SEED_NU = 1, WL_SEED_U = 2, WL_SEED_R = 3, WL_SEED_SPIN = 4, WL_SEED_AMP = 5, WL_SEED_CENTRE = 6 };
 
 typedef struct wl_sim wl_sim;
 
@@ -179,6 +192,17 @@ int wl_energy(wl_sim* s, double out[2]);
 /* Copy interior fields out; any pointer may be NULL.  u: ndim arrays; p, mu0 likewise
  * (mu0: ndim arrays).  Synchronises when host. */
 int wl_get_fields(wl_sim* s, float* u, float* p, float* mu0, int on_device);
+
+/* fp64 views of the state for the fp64 and tangent modes (generic engine only: WL_EINVAL otherwise).  tangent = 0: the
+ * values; 1: the derivatives d/d(theta) (tangent mode only).  Interior-sized buffers as wl_get_fields. */
+int wl_get_fields_f64(wl_sim* s, double* u, double* p, int tangent, int on_device);
+int wl_set_fields_f64(wl_sim* s, const double* u, const double* p, int on_device);
+/* pressure force and its derivative (dF may be NULL; zero in fp64 mode) */
+int wl_pressure_force_f64(wl_sim* s, double t, double F[3], double dF[3]);
+/* kinetic energy, enstrophy and their derivatives (dout may be NULL) */
+int wl_energy_f64(wl_sim* s, double out[2], double dout[2]);
+/* interior copy of a solver array ("u","p","mu0","mu1","V","L","iD","x","r") as doubles into a HOST buffer; returns ncomp */
+int wl_dbg_get_f64(wl_sim* s, const char* name, int level, int tangent, double* out, size_t out_doubles);
 
 /* Fused step: wl_measure(t) (only if the body moves) + wl_mom_step(dt) + the CFL reduction, all asynchronous; t is
  * the time the step ends at (R-R) and becomes the simulation time.  With `adaptive` != 0 the NEXT call ignores `t` and

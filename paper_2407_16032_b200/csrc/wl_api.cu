@@ -83,6 +83,8 @@ static int config_ok(const wl_config* c)
         for (int d = 0; d < 3; ++d) if (!(fabsf(b.scale_amp[d]) < 0.9f)) return 0;     // the map must stay invertible
     }
     if (c->tune.zc < 0 || c->tune.zc > 64 || c->tune.pk_blocks_per_sm < 0) return 0;
+    if (c->precision < 0 || c->precision > 1 || c->tangent_param < 0 || c->tangent_param > WL_SEED_CENTRE) return 0;
+    if (c->tangent_index < 0 || c->tangent_index > WL_MAX_EXTRA) return 0;
     if (c->exit_bc && c->periodic[0]) return 0;
     if (c->mg.smooth_iters < 1) return 0;
     return 1;
@@ -232,9 +234,12 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
     return cv.off;
 }
 
+static int is_generic(const wl_config* c) { return c->precision == 1 || c->tangent_param != WL_SEED_NONE; }
+
 extern "C" size_t wl_workspace_bytes(const wl_config* cfg)
 {
     if (!config_ok(cfg)) return 0;
+    if (is_generic(cfg)) return wl_gen_bytes(cfg);
     return layout(nullptr, cfg, nullptr);
 }
 
@@ -340,12 +345,21 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
     if (!out) return WL_EINVAL;
     *out = nullptr;
     if (!config_ok(cfg)) return WL_EINVAL;
-    size_t need = layout(nullptr, cfg, nullptr);
+    size_t need = is_generic(cfg) ? wl_gen_bytes(cfg) : layout(nullptr, cfg, nullptr);
     if (!dev_ws || ws_bytes < need || ((uintptr_t)dev_ws & 255u)) return WL_ENOMEM;
     wl_sim* s = new (std::nothrow) wl_sim();     // value-initialised: every POD member zero
     if (!s) return WL_ENOMEM;
     s->cfg = *cfg;
     s->st = (cudaStream_t)cuda_stream;
+    if (is_generic(cfg)) {                       // fp64 / tangent: the generic engine owns the workspace
+        if (cudaMallocHost((void**)&s->hs, sizeof(DevScal)) != cudaSuccess) { delete s; return WL_ECUDA; }
+        memset(s->hs, 0, sizeof(DevScal));
+        int rc = wl_gen_create(s, dev_ws);
+        if (rc != WL_OK) { cudaFreeHost(s->hs); delete s; return rc; }
+        s->gen_dt_next = cfg->dt0;
+        *out = s;
+        return WL_OK;
+    }
     layout(s, cfg, dev_ws);
     s->u = s->ubuf[0]; s->u0 = s->ubuf[1]; s->ut = s->ubuf[2];
     solver_scratch(s, s->u);
@@ -407,6 +421,7 @@ extern "C" int wl_sim_destroy(wl_sim* s)
 {
     if (!s) return WL_EINVAL;
     cudaStreamSynchronize(s->st);
+    wl_gen_destroy(s);
     if (s->hs) cudaFreeHost(s->hs);
     for (ProfRec& r : s->prof_recs) s->prof_pool.push_back(r);
     for (ProfRec& r : s->prof_pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -453,6 +468,7 @@ static int copy_in(wl_sim* s, const Grid& g, float* padded, int ncomp, const flo
 
 extern "C" int wl_set_fields(wl_sim* s, const float* u, const float* p, int on_device)
 {
+    if (s && s->gen) return wl_gen_set_fields(s, u, p, on_device);
     if (!s) return WL_EINVAL;
     const Grid& g = s->lev[0].g;
     int rc;
@@ -466,6 +482,7 @@ extern "C" int wl_set_fields(wl_sim* s, const float* u, const float* p, int on_d
 
 extern "C" int wl_get_fields(wl_sim* s, float* u, float* p, float* mu0, int on_device)
 {
+    if (s && s->gen) return wl_gen_get_fields(s, u, p, mu0, on_device);
     if (!s) return WL_EINVAL;
     const Grid& g = s->lev[0].g;
     int rc;
@@ -477,6 +494,7 @@ extern "C" int wl_get_fields(wl_sim* s, float* u, float* p, float* mu0, int on_d
 
 extern "C" int wl_init_tgv(wl_sim* s, int sign)
 {
+    if (s && s->gen) return wl_gen_init_tgv(s, sign >= 0 ? 1 : -1);
     if (!s) return WL_EINVAL;
     wl_k_init_tgv(s, sign >= 0 ? 1 : -1);
     bc_all(s, s->u);
@@ -485,6 +503,7 @@ extern "C" int wl_init_tgv(wl_sim* s, int sign)
 
 extern "C" int wl_measure(wl_sim* s, double t)
 {
+    if (s && s->gen) { s->gen_tbody = t; return wl_gen_measure(s, t); }
     if (!s) return WL_EINVAL;
     NvtxRange r("measure!");
     wl_k_set_time(s, t, 0.0f, 1, -1);
@@ -494,6 +513,7 @@ extern "C" int wl_measure(wl_sim* s, double t)
 
 extern "C" int wl_mom_step(wl_sim* s, float dt)
 {
+    if (s && s->gen) return dt > 0.0f ? wl_gen_mom_step(s, (double)dt) : WL_EINVAL;
     if (!s || !(dt > 0.0f)) return WL_EINVAL;
     wl_k_set_time(s, 0.0, dt, -1, 1);
     int rc = mom_step_body(s);
@@ -503,6 +523,22 @@ extern "C" int wl_mom_step(wl_sim* s, float dt)
 
 extern "C" int wl_step(wl_sim* s, double t, float dt, int adaptive)
 {
+    if (s && s->gen) {                           // generic engine: the CFL result makes a host round trip
+        const int dev = adaptive && s->primed;
+        if (!dev && !(dt > 0.0f)) return WL_EINVAL;
+        const float dtu = dev ? s->gen_dt_next : dt;
+        const double tu = dev ? s->gen_t + (double)dtu : t;
+        int rc = WL_OK;
+        if (s->cfg.body.kind != WL_BODY_NONE && (s->cfg.body.motion != WL_MOTION_STATIC || s->cfg.nextra > 0 || s->cfg.body.scale_freq != 0.0f)) {
+            s->gen_tbody = tu;
+            rc = wl_gen_measure(s, tu);
+        }
+        if (rc == WL_OK) rc = wl_gen_mom_step(s, (double)dtu);
+        if (rc == WL_OK) rc = wl_gen_cfl(s, &s->gen_dt_next);
+        s->gen_t = tu;
+        s->primed = adaptive ? 1 : 0;
+        return rc;
+    }
     if (!s) return WL_EINVAL;
     int dev = adaptive && s->primed;   // device-resident t and dt are valid
     if (!dev && !(dt > 0.0f)) return WL_EINVAL;
@@ -517,6 +553,11 @@ extern "C" int wl_step(wl_sim* s, double t, float dt, int adaptive)
 
 extern "C" int wl_cfl(wl_sim* s, float* dt_out)
 {
+    if (s && s->gen && dt_out) {
+        int rc = wl_gen_cfl(s, dt_out);
+        if (rc == WL_OK && s->noconv) { s->noconv = 0; return WL_ENOCONV; }
+        return rc;
+    }
     if (!s || !dt_out) return WL_EINVAL;
     wl_k_cfl(s, s->u);
     WL_CUDA_CHECK(s, cudaMemcpyAsync(&s->hs->dt_next, &s->ds->dt_next, sizeof(float), cudaMemcpyDeviceToHost, s->st));
@@ -530,6 +571,12 @@ extern "C" int wl_cfl(wl_sim* s, float* dt_out)
 
 extern "C" int wl_pressure_force(wl_sim* s, double t, float F_out[3])
 {
+    if (s && s->gen && F_out) {
+        double F[3];
+        int rc = wl_gen_force(s, t == t ? t : s->gen_tbody, F, nullptr);
+        for (int k = 0; k < 3; ++k) F_out[k] = (float)F[k];
+        return rc;
+    }
     if (!s || !F_out) return WL_EINVAL;
     wl_k_force(s, t);                                // NaN: the body where measure! last placed it
     WL_CUDA_CHECK(s, cudaMemcpyAsync(s->hs->force, s->ds->force, 3 * sizeof(double), cudaMemcpyDeviceToHost, s->st));
@@ -541,6 +588,7 @@ extern "C" int wl_pressure_force(wl_sim* s, double t, float F_out[3])
 
 extern "C" int wl_energy(wl_sim* s, double out[2])
 {
+    if (s && s->gen && out) return wl_gen_energy(s, out, nullptr);
     if (!s || !out) return WL_EINVAL;
     wl_k_energy(s, s->u);
     WL_CUDA_CHECK(s, cudaMemcpyAsync(s->hs->energy, s->ds->energy, 2 * sizeof(double), cudaMemcpyDeviceToHost, s->st));
@@ -548,6 +596,33 @@ extern "C" int wl_energy(wl_sim* s, double out[2])
     if (rc != WL_OK) return rc;
     out[0] = s->hs->energy[0]; out[1] = s->hs->energy[1];
     return WL_OK;
+}
+
+// ---- fp64 / tangent views (generic engine)
+extern "C" int wl_get_fields_f64(wl_sim* s, double* u, double* p, int tangent, int on_device)
+{
+    if (!s || !s->gen) return WL_EINVAL;
+    return wl_gen_get_fields_f64(s, u, p, tangent ? 1 : 0, on_device);
+}
+extern "C" int wl_set_fields_f64(wl_sim* s, const double* u, const double* p, int on_device)
+{
+    if (!s || !s->gen) return WL_EINVAL;
+    return wl_gen_set_fields_f64(s, u, p, on_device);
+}
+extern "C" int wl_pressure_force_f64(wl_sim* s, double t, double F[3], double dF[3])
+{
+    if (!s || !s->gen || !F) return WL_EINVAL;
+    return wl_gen_force(s, t == t ? t : s->gen_tbody, F, dF);
+}
+extern "C" int wl_energy_f64(wl_sim* s, double out[2], double dout[2])
+{
+    if (!s || !s->gen || !out) return WL_EINVAL;
+    return wl_gen_energy(s, out, dout);
+}
+extern "C" int wl_dbg_get_f64(wl_sim* s, const char* name, int level, int tangent, double* out, size_t out_doubles)
+{
+    if (!s || !s->gen || !name || !out) return WL_EINVAL;
+    return wl_gen_dbg_get(s, name, level, tangent ? 1 : 0, out, out_doubles);
 }
 
 extern "C" int wl_stats(wl_sim* s, wl_stats_t* out)
@@ -565,6 +640,7 @@ extern "C" int wl_stats(wl_sim* s, wl_stats_t* out)
 extern "C" int wl_level_dims(const wl_sim* s, int level, int dims_out[3])
 {
     if (!s || level < 0 || level >= s->nlev) return WL_EINVAL;
+    if (s->gen) { for (int d = 0; d < 3; ++d) dims_out[d] = d < s->nd ? s->cfg.dims[d] >> level : 1; return WL_OK; }
     for (int d = 0; d < 3; ++d) dims_out[d] = s->lev[level].g.n[d];
     return WL_OK;
 }
@@ -578,6 +654,7 @@ static const char* const kern_names[WLK_COUNT] = {
 
 extern "C" int wl_prof_enable(wl_sim* s, int enable)
 {
+    if (s && s->gen) return WL_EINVAL;      // stage hooks belong to the tuned kernels
     if (!s) return WL_EINVAL;
     int rc = sync(s);
     if (rc != WL_OK) return rc;
@@ -589,6 +666,7 @@ extern "C" int wl_prof_enable(wl_sim* s, int enable)
 
 extern "C" int wl_prof_read(wl_sim* s, int cls, char* name_out, size_t name_bytes, double* ms_total, int* launches)
 {
+    if (s && s->gen) return WL_EINVAL;      // stage hooks belong to the tuned kernels
     if (!s || cls < 0) return WL_EINVAL;
     if (cls >= 2 * WLK_COUNT) return 1;
     int rc = sync(s);
@@ -611,6 +689,7 @@ extern "C" int wl_prof_read(wl_sim* s, int cls, char* name_out, size_t name_byte
 // ---- stage hooks
 extern "C" int wl_dbg_save_u0(wl_sim* s)
 {
+    if (s && s->gen) return WL_EINVAL;      // stage hooks belong to the tuned kernels
     if (!s) return WL_EINVAL;
     const Grid& g = s->lev[0].g;
     WL_CUDA_CHECK(s, cudaMemcpyAsync(s->u0, s->u, sizeof(float) * g.nalloc * s->nd, cudaMemcpyDeviceToDevice, s->st));
@@ -618,15 +697,17 @@ extern "C" int wl_dbg_save_u0(wl_sim* s)
 }
 extern "C" int wl_dbg_conv_diff_bdim(wl_sim* s, float dt, int corrector)
 {
+    if (s && s->gen) return WL_EINVAL;      // stage hooks belong to the tuned kernels
     if (!s) return WL_EINVAL;
     wl_k_set_time(s, 0.0, dt, -1, 1);
     wl_k_conv_diff_bdim(s, s->u, s->u0, s->ut, corrector);
     float* t = s->u; s->u = s->ut; s->ut = t;
     return check(s);
 }
-extern "C" int wl_dbg_bc(wl_sim* s) { if (!s) return WL_EINVAL; bc_all(s, s->u); return check(s); }
+extern "C" int wl_dbg_bc(wl_sim* s) { if (!s || s->gen) return WL_EINVAL; bc_all(s, s->u); return check(s); }
 extern "C" int wl_dbg_exit_bc(wl_sim* s, float dt)
 {
+    if (s && s->gen) return WL_EINVAL;      // stage hooks belong to the tuned kernels
     if (!s) return WL_EINVAL;
     wl_k_set_time(s, 0.0, dt, -1, 1);
     wl_k_exit_bc(s, s->u, s->u0);
@@ -634,6 +715,7 @@ extern "C" int wl_dbg_exit_bc(wl_sim* s, float dt)
 }
 extern "C" int wl_dbg_project(wl_sim* s, float w, float dt)
 {
+    if (s && s->gen) return WL_EINVAL;      // stage hooks belong to the tuned kernels
     if (!s) return WL_EINVAL;
     wl_k_set_time(s, 0.0, dt, -1, 1);
     s->solve_slot = 0;
@@ -642,6 +724,7 @@ extern "C" int wl_dbg_project(wl_sim* s, float w, float dt)
 }
 extern "C" int wl_dbg_residual(wl_sim* s)
 {
+    if (s && s->gen) return WL_EINVAL;      // stage hooks belong to the tuned kernels
     // r = div u - A x with the CURRENT x: expressed through k_residual by p := x, w dt := 1
     if (!s) return WL_EINVAL;
     const Grid& g = s->lev[0].g;
@@ -652,21 +735,23 @@ extern "C" int wl_dbg_residual(wl_sim* s)
     WL_CUDA_CHECK(s, cudaMemcpyAsync(s->p, s->lev[0].q, sizeof(float) * g.nalloc, cudaMemcpyDeviceToDevice, s->st));
     return check(s);
 }
-extern "C" int wl_dbg_apply_gradient(wl_sim* s) { if (!s) return WL_EINVAL; wl_k_apply_gradient(s, s->u); return check(s); }
-extern "C" int wl_dbg_restrict(wl_sim* s, int l) { if (!s || l < 0 || l + 1 >= s->nlev) return WL_EINVAL; wl_k_restrict(s, l); return check(s); }
-extern "C" int wl_dbg_prolong(wl_sim* s, int l) { if (!s || l < 0 || l + 1 >= s->nlev) return WL_EINVAL; wl_k_prolong(s, l); return check(s); }
+extern "C" int wl_dbg_apply_gradient(wl_sim* s) { if (!s || s->gen) return WL_EINVAL; wl_k_apply_gradient(s, s->u); return check(s); }
+extern "C" int wl_dbg_restrict(wl_sim* s, int l) { if (!s || s->gen || l < 0 || l + 1 >= s->nlev) return WL_EINVAL; wl_k_restrict(s, l); return check(s); }
+extern "C" int wl_dbg_prolong(wl_sim* s, int l) { if (!s || s->gen || l < 0 || l + 1 >= s->nlev) return WL_EINVAL; wl_k_prolong(s, l); return check(s); }
 extern "C" int wl_dbg_smooth(wl_sim* s, int l, int iters)
 {
+    if (s && s->gen) return WL_EINVAL;      // stage hooks belong to the tuned kernels
     if (!s || l < 0 || l >= s->nlev || iters < 1) return WL_EINVAL;
     wl_k_rsum(s, l);          // in a solve the kernel that wrote r leaves this sum
     wl_k_smooth(s, l, iters);
     return check(s);
 }
-extern "C" int wl_dbg_vcycle(wl_sim* s, int l) { if (!s || l < 0 || l >= s->nlev) return WL_EINVAL; wl_k_vcycle(s, l); return check(s); }
+extern "C" int wl_dbg_vcycle(wl_sim* s, int l) { if (!s || s->gen || l < 0 || l >= s->nlev) return WL_EINVAL; wl_k_vcycle(s, l); return check(s); }
 
 // runs n coarse-level passes (kind: 0 restrict level->level+1, 1 smooth, 2 prolong level+1->level) as ONE k_coarse launch
 extern "C" int wl_dbg_coarse_prog(wl_sim* s, int n, const int* kinds, const int* levels, const int* iters)
 {
+    if (s && s->gen) return WL_EINVAL;      // stage hooks belong to the tuned kernels
     if (!s || n < 1 || n > 3 * WL_MAXLEV || !kinds || !levels || !iters) return WL_EINVAL;
     CoarseProg P; P.n = n;
     for (int k = 0; k < n; ++k) {
@@ -681,6 +766,7 @@ extern "C" int wl_dbg_coarse_prog(wl_sim* s, int n, const int* kinds, const int*
 // PCG scalars of a level: rho, gamma, alpha, beta, rho0, rsum, nlive, live
 extern "C" int wl_dbg_pcg_scalars(wl_sim* s, int level, double out[8])
 {
+    if (s && s->gen) return WL_EINVAL;      // stage hooks belong to the tuned kernels
     if (!s || level < 0 || level >= s->nlev || !out) return WL_EINVAL;
     PcgScal h;
     WL_CUDA_CHECK(s, cudaMemcpyAsync(&h, &s->ds->pcg[level], sizeof(PcgScal), cudaMemcpyDeviceToHost, s->st));
@@ -712,7 +798,7 @@ static int find_array(wl_sim* s, const char* name, int level, float** arr, int* 
 }
 static int dbg_get(wl_sim* s, const char* name, int level, float* out, size_t out_floats, int whole)
 {
-    if (!s || !name || !out) return WL_EINVAL;
+    if (!s || !name || !out || s->gen) return WL_EINVAL;
     float* arr; int nc; const Grid* g;
     int rc = find_array(s, name, level, &arr, &nc, &g);
     if (rc != WL_OK) return rc;
@@ -735,6 +821,7 @@ extern "C" int wl_dbg_get_padded(wl_sim* s, const char* name, int level, float* 
 }
 extern "C" int wl_dbg_set(wl_sim* s, const char* name, int level, const float* in, size_t in_floats)
 {
+    if (s && s->gen) return WL_EINVAL;      // stage hooks belong to the tuned kernels
     if (!s || !name || !in) return WL_EINVAL;
     float* arr; int nc; const Grid* g;
     int rc = find_array(s, name, level, &arr, &nc, &g);

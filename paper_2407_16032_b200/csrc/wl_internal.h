@@ -86,6 +86,10 @@ struct wl_sim {
     int noconv_total;        // ... since create (wl_stats)
     int primed;              // device-resident t and dt are valid (adaptive wl_step)
     int sm_count;
+    void* gen;               // the generic engine (wl_generic.cu) when cfg.precision = 1 or a tangent is asked for, else null
+    int gen_kind;            // 1: double, 2: dual
+    double gen_t, gen_tbody; // simulation time / time the body was last placed (generic engine: host-side)
+    float gen_dt_next;
     char err[256];
     // profiling (off by default): every launch bracketed by two events on the stream
     int prof_on;
@@ -152,6 +156,21 @@ void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout)
 // wl_pcgfused.cu
 int wl_pcg_fused_shape(int nd, const Grid& g, const VT& vt);    // the one-sweep form can take a level of this shape
 int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r);              // 0: not taken (the caller runs the two-pass form)
+// wl_generic.cu
+size_t wl_gen_bytes(const wl_config* c);
+int wl_gen_create(wl_sim* s, void* ws);
+void wl_gen_destroy(wl_sim* s);
+int wl_gen_measure(wl_sim* s, double t);
+int wl_gen_mom_step(wl_sim* s, double dt);
+int wl_gen_cfl(wl_sim* s, float* dt_out);
+int wl_gen_force(wl_sim* s, double t, double* F, double* dF);
+int wl_gen_energy(wl_sim* s, double* out, double* dout);
+int wl_gen_init_tgv(wl_sim* s, int sign);
+int wl_gen_set_fields(wl_sim* s, const float* u, const float* p, int on_device);
+int wl_gen_set_fields_f64(wl_sim* s, const double* u, const double* p, int on_device);
+int wl_gen_get_fields(wl_sim* s, float* u, float* p, float* mu0, int on_device);
+int wl_gen_get_fields_f64(wl_sim* s, double* u, double* p, int lane, int on_device);
+int wl_gen_dbg_get(wl_sim* s, const char* name, int level, int lane, double* out, size_t n);
 // wl_small.cu
 int wl_small_max_cluster(wl_sim* s);
 int wl_small_blocks(const Grid& g);

@@ -18,10 +18,12 @@ from . import build as _build
 BODY_NONE, BODY_SPHERE, BODY_TORUS, BODY_CYLINDER, BODY_PLANE = 0, 1, 2, 3, 4
 MOTION_STATIC, MOTION_SIN = 0, 1
 WL_OK, WL_EINVAL, WL_ENOMEM, WL_ECUDA, WL_ENOCONV = 0, -1, -2, -3, -4
+SEEDS = {"nu": 1, "U": 2, "R": 3, "spin": 4, "amp": 5, "centre": 6}       # WL_SEED_*: the parameter a tangent is taken with respect to
 
 EXPORTS = [
     "wl_workspace_bytes", "wl_sim_create", "wl_sim_destroy", "wl_set_fields", "wl_init_tgv", "wl_measure",
     "wl_mom_step", "wl_cfl", "wl_pressure_force", "wl_energy", "wl_get_fields", "wl_step",
+    "wl_get_fields_f64", "wl_set_fields_f64", "wl_pressure_force_f64", "wl_energy_f64", "wl_dbg_get_f64",
     "wl_dbg_conv_diff_bdim", "wl_dbg_save_u0", "wl_dbg_bc", "wl_dbg_exit_bc", "wl_dbg_project",
     "wl_dbg_residual", "wl_dbg_apply_gradient", "wl_dbg_restrict", "wl_dbg_prolong", "wl_dbg_smooth", "wl_dbg_vcycle",
     "wl_dbg_coarse_prog", "wl_dbg_pcg_scalars",
@@ -53,7 +55,8 @@ class Config(C.Structure):
                 ("nu", C.c_float), ("periodic", C.c_int * 3), ("exit_bc", C.c_int), ("eps", C.c_float),
                 ("dt0", C.c_float), ("dt_max", C.c_float), ("cfl_c", C.c_float), ("cfl_cnu", C.c_float),
                 ("body", Body), ("mg", MG), ("tune", Tuning),
-                ("nextra", C.c_int), ("extra", Body * 3), ("extra_op", C.c_int * 3)]
+                ("nextra", C.c_int), ("extra", Body * 3), ("extra_op", C.c_int * 3),
+                ("precision", C.c_int), ("tangent_param", C.c_int), ("tangent_index", C.c_int)]
 
 
 class Stats(C.Structure):
@@ -90,6 +93,12 @@ def load(build_if_missing: bool = True):
     L.wl_cfl.argtypes = [vp, fp]
     L.wl_pressure_force.argtypes = [vp, C.c_double, fp]
     L.wl_energy.argtypes = [vp, C.POINTER(C.c_double)]
+    dp = C.POINTER(C.c_double)
+    L.wl_get_fields_f64.argtypes = [vp, vp, vp, ip, ip]
+    L.wl_set_fields_f64.argtypes = [vp, vp, vp, ip]
+    L.wl_pressure_force_f64.argtypes = [vp, C.c_double, dp, dp]
+    L.wl_energy_f64.argtypes = [vp, dp, dp]
+    L.wl_dbg_get_f64.argtypes = [vp, C.c_char_p, ip, ip, vp, C.c_size_t]
     L.wl_get_fields.argtypes = [vp, vp, vp, vp, ip]
     L.wl_dbg_conv_diff_bdim.argtypes = [vp, C.c_float, ip]
     L.wl_dbg_save_u0.argtypes = [vp]
@@ -158,6 +167,10 @@ def make_config(cfg: dict) -> Config:
     for k in ("max_levels", "smooth_iters", "max_vcycles", "fixed_vcycles"):
         setattr(c.mg, k, int(cfg[k]))
     c.mg.tol = float(cfg["tol"])
+    c.precision = int(cfg.get("precision", 0))
+    if cfg.get("tangent"):                                 # ("nu" | "U" | "R" | "spin" | "amp" | "centre", index)
+        name, idx = cfg["tangent"]
+        c.tangent_param, c.tangent_index = SEEDS[name], int(idx)
     for k, v in (cfg.get("tune") or {}).items():          # wl_tuning: implementation switches, all zero by default
         if not hasattr(c.tune, k):
             raise KeyError(f"wl_tuning has no field {k}")
@@ -271,6 +284,37 @@ class Sim:
         out = (C.c_double * 2)()
         self._chk(self._L.wl_energy(self._h, out))
         return np.array([out[0], out[1]])
+
+    # -- fp64 / tangent modes (cfg["precision"] = 1 or cfg["tangent"] = (parameter, index)): the generic engine
+    def fields_f64(self, tangent: bool = False):
+        """(u, p) as float64 numpy arrays: the values, or (tangent mode) their derivatives d/d(theta)"""
+        u = np.empty((self.nd,) + self.shape, dtype=np.float64)
+        p = np.empty(self.shape, dtype=np.float64)
+        self._chk(self._L.wl_get_fields_f64(self._h, C.c_void_p(u.ctypes.data), C.c_void_p(p.ctypes.data), int(tangent), 0))
+        return u, p
+
+    def set_fields_f64(self, u=None, p=None):
+        u = None if u is None else np.ascontiguousarray(u, dtype=np.float64)
+        p = None if p is None else np.ascontiguousarray(p, dtype=np.float64)
+        self._chk(self._L.wl_set_fields_f64(self._h, None if u is None else C.c_void_p(u.ctypes.data),
+                                            None if p is None else C.c_void_p(p.ctypes.data), 0))
+
+    def pressure_force_f64(self, t: float = math.nan):
+        F, dF = (C.c_double * 3)(), (C.c_double * 3)()
+        self._chk(self._L.wl_pressure_force_f64(self._h, float(t), F, dF))
+        return np.array(list(F)), np.array(list(dF))
+
+    def energy_f64(self):
+        e, de = (C.c_double * 2)(), (C.c_double * 2)()
+        self._chk(self._L.wl_energy_f64(self._h, e, de))
+        return np.array(list(e)), np.array(list(de))
+
+    def dbg_get_f64(self, name: str, level: int = 0, tangent: bool = False) -> np.ndarray:
+        ld = self.level_dims(level if name in ("L", "iD", "x", "r") else 0)
+        ncomp = {"u": self.nd, "mu0": self.nd, "L": self.nd, "V": self.nd, "mu1": self.nd * self.nd}.get(name, 1)
+        out = np.empty((ncomp,) + tuple(reversed(ld)), dtype=np.float64)
+        self._chk(self._L.wl_dbg_get_f64(self._h, name.encode(), int(level), int(tangent), C.c_void_p(out.ctypes.data), C.c_size_t(out.size)))
+        return out
 
     def get_fields(self, u=None, p=None, mu0=None):
         """Copy into the given buffers (torch cuda / torch cpu / numpy); all on the same side."""

@@ -37,7 +37,7 @@ def test_config_struct_layout_matches_header():
     assert C.sizeof(wl.Tuning) == 4 * 6 + 8 + 8              # six ints, one long long (8-aligned), one int + tail padding
     head = 4 * (1 + 3 + 1 + 3 + 1 + 3 + 1 + 1 + 4) + C.sizeof(wl.Body) + C.sizeof(wl.MG)
     assert wl.Config.tune.offset == (head + 7) // 8 * 8
-    tail = 4 + 3 * C.sizeof(wl.Body) + 4 * 3                  # nextra, extra[3], extra_op[3]
+    tail = 4 + 3 * C.sizeof(wl.Body) + 4 * 3 + 4 * 3          # nextra, extra[3], extra_op[3]; precision, tangent_param, tangent_index
     assert wl.Config.nextra.offset == wl.Config.tune.offset + C.sizeof(wl.Tuning)
     assert C.sizeof(wl.Config) == (wl.Config.nextra.offset + tail + 7) // 8 * 8
 

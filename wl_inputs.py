@@ -31,6 +31,9 @@ CONFIG_DEFAULTS = dict(
     # s_d = 1 + scale_amp[d] cos(2 pi scale_freq t + scale_phase), spin about the axis, and further primitives combined by
     # SDF arithmetic: parts = [dict(kind=..., centre=..., ..., op="+" | "-"), ...] (same keys as the first primitive)
     shell=0.0, scale_amp=(0.0, 0.0, 0.0), scale_freq=0.0, scale_phase=0.0, spin=0.0, parts=None,
+    # scalar type of the CUDA library: precision 1 = fp64; tangent = (parameter name, index): the
+    # forward-mode derivative of the whole step with respect to "nu" | "U" | "R" | "spin" | "amp" | "centre"
+    precision=0, tangent=None,
     max_levels=0, smooth_iters=6, max_vcycles=32, fixed_vcycles=2, tol=1e-4,
 )
 
