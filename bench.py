@@ -510,6 +510,22 @@ def run_gpu(args) -> None:
                 also[NAMES[kk]] = {"skipped": str(e)[:120]}
             torch.cuda.empty_cache()
 
+    # ---- scalar types: the tuned fp32 kernels against the generic engine in fp64 and in fp64
+    # dual numbers (value + d/d nu through every kernel) on C3 at 1/2 scale; the paper quotes +80 % for Dual over plain
+    modes = None
+    if world == 1 and not args.no_also:
+        modes = {}
+        cm = workload_config(2, scale=2)
+        for name, extra in (("fp32_tuned", {}), ("fp64_generic", {"precision": 1}), ("tangent_fp64_dual", {"tangent": ("nu", 0)})):
+            s2, d0 = make_sim(dict(cm, **extra), device)
+            nst = 10
+            ms = time_steps(torch, s2, d0, nst, 3, None)
+            modes[name] = {"ns_per_cell_step": ms * 1e6 / (ncells(cm) * nst), "ms_per_step": ms / nst}
+            s2.close()
+            torch.cuda.empty_cache()
+        modes["workload"] = "C3 at 1/2 scale (128x64x64)"
+        modes["tangent_over_fp64"] = modes["tangent_fp64_dual"]["ms_per_step"] / modes["fp64_generic"]["ms_per_step"]
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -524,7 +540,7 @@ def run_gpu(args) -> None:
             "cells_steps_per_s": agg["cells_steps_per_s"], "force_every_step": force,
             "clocks": clocks, "e2e": e2e, "gpu_launches": l2 - l1, "gpu_launches_per_step": (l2 - l1) / (args.steps * args.repeats),
             "vcycles_per_solve": st["vcycles"], "nan_flag": st["nan_flag"], "dt_last": dt_now,
-            "roofline": roofline, "cpu_baseline": cpu, "tolerance_mode": tol_mode, "also": also,
+            "roofline": roofline, "cpu_baseline": cpu, "tolerance_mode": tol_mode, "also": also, "scalar_types": modes,
             "context": "paper: 1.57 ns/DOF/step on H100 64GB, fp32, half-domain TGV 512^3 (PAPER.md:143); another machine, not a target"}
     print(json.dumps(line), flush=True)
     if dist is not None:
