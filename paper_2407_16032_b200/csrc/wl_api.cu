@@ -7,6 +7,7 @@
 #include <new>
 #include <nvtx3/nvToolsExt.h>
 #include "wl_internal.h"
+#include "wl_tma.cuh"
 
 // NVTX range per routine of the paper's step (P:139 names them; the paper profiles with NVTX ranges under Nsight
 // Systems): visible in nsys / ncu --nvtx, a no-op (one predicted branch) when no tool is attached.
@@ -371,6 +372,9 @@ extern "C" int wl_sim_create(const wl_config* cfg, void* dev_ws, size_t ws_bytes
             if ((long long)g.n[0] * g.n[1] * g.n[2] <= maxc) s->pk_level = l; else break;
         }
     }
+    s->tmc = new (std::nothrow) TmCache();
+    if (!s->tmc) { delete s; return WL_ENOMEM; }
+    s->tmc->n = 0;
     s->fast_A = !cfg->tune.no_fast_a;
     s->fused = !cfg->tune.no_fused;
     s->tiny_on = !cfg->tune.no_block_levels;
@@ -422,6 +426,7 @@ extern "C" int wl_sim_destroy(wl_sim* s)
     if (!s) return WL_EINVAL;
     cudaStreamSynchronize(s->st);
     wl_gen_destroy(s);
+    delete s->tmc;
     if (s->hs) cudaFreeHost(s->hs);
     for (ProfRec& r : s->prof_recs) s->prof_pool.push_back(r);
     for (ProfRec& r : s->prof_pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }

@@ -673,7 +673,11 @@ void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out,
     int cd3 = s->tma_cd && s->nd == 3 && !P.g.per[0] && !P.g.per[1];
     CUtensorMap tm[3];
     if (cd3)
-        for (int c = 0; c < 3 && cd3; ++c) cd3 = wl_tensor_map3(&tm[c], w + c * P.g.nalloc, P.g, CD_W, CD_R);
+        for (int c = 0; c < 3 && cd3; ++c) {
+            const CUtensorMap* pm = wl_tensor_map_cached(s->tmc, w + c * P.g.nalloc, P.g, CD_W, CD_R);
+            cd3 = pm != nullptr;
+            if (pm) tm[c] = *pm;
+        }
     if (cd3) {
         const size_t smem3 = sizeof(float) * CD3_NP * 3 * CD_PLANE + sizeof(float4) * 2 * 3 * CD_NT + 8 * CD3_NP + 16;
         if (!(s->cd_attr_set & 4)) {

@@ -86,6 +86,7 @@ struct wl_sim {
     int noconv_total;        // ... since create (wl_stats)
     int primed;              // device-resident t and dt are valid (adaptive wl_step)
     int sm_count;
+    struct TmCache* tmc;     // encoded tensor maps of the solver and velocity arrays (wl_tma.cuh)
     void* gen;               // the generic engine (wl_generic.cu) when cfg.precision = 1 or a tangent is asked for, else null
     int gen_kind;            // 1: double, 2: dual
     double gen_t, gen_tbody; // simulation time / time the body was last placed (generic engine: host-side)

@@ -377,7 +377,12 @@ void wl_k_pcg_A_fast(wl_sim* s, int l, int first, const float* ein, float* eout)
     int bulk = s->bulk_A && lv.vt.lxl == 5 && !lv.g.per[0] && !lv.g.per[1] && lv.vt.ngx % 32 == 0;
     CUtensorMap tm_r, tm_e;
     memset(&tm_r, 0, sizeof(tm_r)); memset(&tm_e, 0, sizeof(tm_e));
-    if (bulk) bulk = wl_tensor_map3(&tm_r, lv.r, lv.g, 4 * 32 + 8, 8 + 2) && (first || wl_tensor_map3(&tm_e, ein, lv.g, 4 * 32 + 8, 8 + 2));
+    if (bulk) {
+        const CUtensorMap* pr = wl_tensor_map_cached(s->tmc, lv.r, lv.g, 4 * 32 + 8, 8 + 2);
+        const CUtensorMap* pe = first ? pr : wl_tensor_map_cached(s->tmc, ein, lv.g, 4 * 32 + 8, 8 + 2);
+        bulk = pr && pe;
+        if (bulk) { tm_r = *pr; if (!first) tm_e = *pe; }
+    }
     const size_t smem = wl_pcg_fast_smem(lv.vt, first, bulk);
     switch (lv.vt.lxl) {
     case 5:

@@ -413,9 +413,15 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
     float *ra = lv.r, *rb = lv.r2;            // ra: the residual as it stands
     float *ea = lv.e2, *eb = lv.e;            // ea: the direction of the previous iteration, eb: the one being written
     float *qa = lv.q2, *qb = lv.q;
-    CUtensorMap tm_r, tm_e, tm_q, tm_x;
+    // every map this call needs, encoded once per handle (cached) and checked BEFORE the first launch: a failed encode sends
+    // the caller to the two-pass form instead of launching a sweep with a stale map
+    const float* halo_arrays[6] = { lv.r, lv.r2, lv.e, lv.e2, lv.q, lv.q2 };
+    for (int k = 0; k < 6; ++k)
+        if (!wl_tensor_map_cached(s->tmc, halo_arrays[k], lv.g, FF_RW, 10)) return 0;
+    const CUtensorMap* ptm_x = wl_tensor_map_cached(s->tmc, lv.x, lv.g, 128, 8);
+    if (!ptm_x) return 0;
+    CUtensorMap tm_r = *wl_tensor_map_cached(s->tmc, ra, lv.g, FF_RW, 10), tm_e, tm_q, tm_x = *ptm_x;
     memset(&tm_e, 0, sizeof(tm_e)); memset(&tm_q, 0, sizeof(tm_q));
-    if (!wl_tensor_map3(&tm_r, ra, lv.g, FF_RW, 10) || !wl_tensor_map3(&tm_x, lv.x, lv.g, 128, 8)) return 0;
     {
         ProfScope ps_(s, WLK_PCG_MATVEC, l > 0);
         k_pcg_fused<1><<<grid, WL_VB, ff_smem(1), s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, 0, lv.L, lv.iD, lv.x, ra, rb, ea, eb, qa, qb, sc, s->rb,
@@ -424,7 +430,9 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
     for (int k = 2; k <= iters; ++k) {
         float* t = ea; ea = eb; eb = t;
         t = qa; qa = qb; qb = t;
-        wl_tensor_map3(&tm_r, ra, lv.g, FF_RW, 10); wl_tensor_map3(&tm_e, ea, lv.g, FF_RW, 10); wl_tensor_map3(&tm_q, qa, lv.g, FF_RW, 10);
+        tm_r = *wl_tensor_map_cached(s->tmc, ra, lv.g, FF_RW, 10);       // cache hits: encoded and checked above
+        tm_e = *wl_tensor_map_cached(s->tmc, ea, lv.g, FF_RW, 10);
+        tm_q = *wl_tensor_map_cached(s->tmc, qa, lv.g, FF_RW, 10);
         {
             ProfScope ps_(s, WLK_PCG_FUSED, l > 0);
             k_pcg_fused<0><<<grid, WL_VB, ff_smem(0), s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, k - 1, lv.L, lv.iD, lv.x, ra, rb, ea, eb, qa, qb, sc,

@@ -1019,8 +1019,22 @@ static void coarse_launch_one(wl_sim* s, const CoarseProg& prog)
     DevScal* ds = s->ds;
     double* part = s->pk_part;
     void* args[] = { (void*)&levs, (void*)&prog, (void*)&ds, (void*)&part };
-    if (s->nd == 3) cudaLaunchCooperativeKernel((const void*)k_coarse<3>, dim3(s->pk_blocks), dim3(WL_VB), args, 0, s->st);
-    else            cudaLaunchCooperativeKernel((const void*)k_coarse<2>, dim3(s->pk_blocks), dim3(WL_VB), args, 0, s->st);
+    cudaError_t e;
+    if (s->nd == 3) e = cudaLaunchCooperativeKernel((const void*)k_coarse<3>, dim3(s->pk_blocks), dim3(WL_VB), args, 0, s->st);
+    else            e = cudaLaunchCooperativeKernel((const void*)k_coarse<2>, dim3(s->pk_blocks), dim3(WL_VB), args, 0, s->st);
+    if (e != cudaSuccess) {
+        // the grid cannot be co-scheduled on this device (a partitioned GPU: MIG, an MPS SM limit): from now on every level runs its
+        // passes as stand-alone kernels, starting with this chain
+        cudaGetLastError();
+        s->pk_level = s->nlev;
+        s->tiny_on = 0;
+        for (int o = 0; o < prog.n; ++o) {
+            const CoarseOp& op = prog.op[o];
+            if (op.kind == COP_RESTRICT) wl_k_restrict(s, op.level);
+            else if (op.kind == COP_PROLONG) wl_k_prolong(s, op.level);
+            else { wl_k_rsum(s, op.level); wl_k_smooth(s, op.level, op.iters, 1); }
+        }
+    }
 }
 
 // blocks of the k_small cluster a pass needs (the level whose cells it walks), or 0 when the pass belongs to k_coarse

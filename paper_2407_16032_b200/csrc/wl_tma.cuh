@@ -53,3 +53,26 @@ static inline int wl_tensor_map3(CUtensorMap* tm, const float* base, const Grid&
     return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
+
+// Per-handle cache of encoded tensor maps, keyed by (base pointer, row pitch, box): the solver arrays never move, so every
+// map is encoded once (a smoother call used to re-encode ~15 of them) and an encode failure is seen by the caller, which
+// then takes the path without TMA.
+struct TmCache {
+    struct Entry { const float* base; int P, S1, S2, bx, by; CUtensorMap tm; };
+    Entry e[64];
+    int n;
+};
+static inline const CUtensorMap* wl_tensor_map_cached(TmCache* c, const float* base, const Grid& g, int box_x, int box_y)
+{
+    for (int k = 0; k < c->n; ++k) {
+        const TmCache::Entry& q = c->e[k];
+        if (q.base == base && q.P == g.P && q.S1 == g.S[1] && q.S2 == g.S[2] && q.bx == box_x && q.by == box_y) return &q.tm;
+    }
+    TmCache::Entry q;
+    q.base = base; q.P = g.P; q.S1 = g.S[1]; q.S2 = g.S[2]; q.bx = box_x; q.by = box_y;
+    if (!wl_tensor_map3(&q.tm, base, g, box_x, box_y)) return nullptr;
+    const int slot = c->n < 64 ? c->n++ : 63;          // a full cache recycles its last slot
+    c->e[slot] = q;
+    return &c->e[slot].tm;
+}
+
