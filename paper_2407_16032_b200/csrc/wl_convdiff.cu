@@ -182,11 +182,23 @@ __device__ __forceinline__ float4 cd_fetch(const Grid& g, const float* __restric
 // values for phi > 0 / phi <= 0, fbp / fbn the boundary fallbacks of R-H
 __device__ __forceinline__ float face_flux(float phi, float wup, float wm, float wc, float wun, bool fbp, bool fbn, float nu)
 {
+    // phi psi - nu (wc - wm) with the limited value psi = q(U, C, D) of the upwind triple, written WITHOUT selecting U, C, D: with
+    // d1 = wc - wm, tt = the difference on the upwind side (wm - wup if phi > 0, else wun - wc), s1 = sign(d1) and avg = (wm + wc)/2,
+    //     m = max(0, min((2 |d1| + s1 tt)/6, 9 s1 tt, |d1|)),   psi = avg +- (s1 m - d1/2)   (+ for phi > 0),
+    // (the quick() above in differences from C, and C = avg -+ d1/2), so phi psi = phi avg + |phi| (s1 m - d1/2): one select, two sign
+    // transfers, and the three differences of a row of faces are shared between neighbouring faces.  The R-H fallback drops the
+    // correction.
     const bool pos = phi > 0.0f;
     const bool fb = pos ? fbp : fbn;
-    const float U = pos ? wup : wun, C = pos ? wm : wc, D = pos ? wc : wm;
-    const float psi = fb ? 0.5f * (wm + wc) : quick(U, C, D);
-    return phi * psi - nu * (wc - wm);
+    const float d1 = wc - wm;
+    const float tt = pos ? wm - wup : wun - wc;
+    const unsigned sgn = __float_as_uint(d1) & 0x80000000u;
+    const float stt = __uint_as_float(__float_as_uint(tt) ^ sgn);
+    const float ad = fabsf(d1);
+    const float m = fmaxf(0.0f, fminf(fminf(fmaf(stt, 1.0f / 6.0f, ad * (1.0f / 3.0f)), 9.0f * stt), ad));
+    float corr = fmaf(-0.5f, d1, __uint_as_float(__float_as_uint(m) ^ sgn));
+    corr = fb ? 0.0f : corr;
+    return fmaf(0.5f * phi, wm + wc, fmaf(fabsf(phi), corr, -nu * d1));
 }
 
 struct CdT { int ntx, nty, ntz, ntiles, zc; };
@@ -366,32 +378,40 @@ __device__ __forceinline__ void cd2_fluxes(const FlowP& P, const CdView2& v, int
     }
 }
 
+// what the output phase needs from global memory: issued BEFORE the flux phase of the plane, so that the L2 latency of these
+// loads (they were the largest stall of the kernel: 1.8 warps per issue on the long scoreboard) hides behind the arithmetic
+struct Cd2Pre { float mm[4], uu[4], vv[4]; };
+template <int ND, int I>
+__device__ __forceinline__ void cd2_preload(const FlowP& P, int gx, int gy, int gz, int nv, const float* __restrict__ u0,
+                                            const float* __restrict__ mu0, float Vi, int corrector, Cd2Pre& o)
+{
+    const Grid& g = P.g;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { o.mm[k] = 0.0f; o.uu[k] = 0.0f; o.vv[k] = Vi; }
+    if (nv <= 0) return;
+    const int64_t id = gidx(g, gx, gy, gz);
+    unpack4(ld4(mu0 + I * g.nalloc, id), o.mm);
+    if (corrector) unpack4(ld4(u0 + I * g.nalloc, id), o.uu);
+    if (P.Vf) unpack4(ld4(P.Vf + I * g.nalloc, id), o.vv);      // a general body: V is a field
+}
+
 // output phase: r = rx + (fyl - fyu) + fzd; f = u0 + dt r - V; B = V + mu0 f; predictor u = B, corrector u = (u' + B)/2
 template <int ND, int I>
 __device__ __forceinline__ void cd2_output(const FlowP& P, int gx, int gy, int gz, int nv, const Cd2Part& q, const float (&fyu)[4],
-                                           const float* __restrict__ u0, const float* __restrict__ mu0, float* __restrict__ out,
-                                           float dt, float Vi, int corrector)
+                                           const Cd2Pre& pre, float* __restrict__ out, float dt, int corrector)
 {
     const Grid& g = P.g;
     if (nv <= 0) return;
-    float o[4], uu[4], mm[4];
+    float o[4];
     const int64_t id = gidx(g, gx, gy, gz);
-    unpack4(ld4(mu0 + I * g.nalloc, id), mm);
-    if (corrector) unpack4(ld4(u0 + I * g.nalloc, id), uu);
-    else {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) uu[k] = q.wc[k];
-    }
-#pragma unroll
-    float vv[4] = { Vi, Vi, Vi, Vi };
-    if (P.Vf) unpack4(ld4(P.Vf + I * g.nalloc, id), vv);      // a general body: V is a field
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         float r = q.rx[k];
         r += q.fyl[k] - fyu[k];
         if (ND == 3) r += q.fzd[k];
-        const float f = uu[k] + dt * r - vv[k];
-        const float B = vv[k] + mm[k] * f;
+        const float uu = corrector ? pre.uu[k] : q.wc[k];
+        const float f = uu + dt * r - pre.vv[k];
+        const float B = pre.vv[k] + pre.mm[k] * f;
         o[k] = corrector ? 0.5f * (q.wc[k] + B) : B;
     }
     st4(out + I * g.nalloc, id, o, nv);
@@ -455,10 +475,11 @@ __global__ void __launch_bounds__(CD2_NT(ND), 1) k_cd_tile2(FlowP P, CdT T, cons
                 v.b[ND == 3 ? d : 2] = ring + s * SLOT + tofs;
             }
             Cd2Part q;
+            Cd2Pre pre;
             const bool first = z == z0;
-            if (comp == 0)      cd2_fluxes<ND, 0>(P, v, gx, gy, z, top, first, fz, q);
-            else if (comp == 1) cd2_fluxes<ND, 1>(P, v, gx, gy, z, top, first, fz, q);
-            else if (ND == 3)   cd2_fluxes<ND, 2>(P, v, gx, gy, z, top, first, fz, q);
+            if (comp == 0)      { cd2_preload<ND, 0>(P, gx, gy, z, nv, u0, mu0, Vi, corrector, pre); cd2_fluxes<ND, 0>(P, v, gx, gy, z, top, first, fz, q); }
+            else if (comp == 1) { cd2_preload<ND, 1>(P, gx, gy, z, nv, u0, mu0, Vi, corrector, pre); cd2_fluxes<ND, 1>(P, v, gx, gy, z, top, first, fz, q); }
+            else if (ND == 3)   { cd2_preload<ND, 2>(P, gx, gy, z, nv, u0, mu0, Vi, corrector, pre); cd2_fluxes<ND, 2>(P, v, gx, gy, z, top, first, fz, q); }
             ex[(comp * CD_TY + ty) * CD_TX + tx] = make_float4(q.fyl[0], q.fyl[1], q.fyl[2], q.fyl[3]);
             __syncthreads();                       // every lower-y-face flux of the plane is in shared memory
             float fyu[4];
@@ -468,9 +489,9 @@ __global__ void __launch_bounds__(CD2_NT(ND), 1) k_cd_tile2(FlowP P, CdT T, cons
             } else {
                 unpack4(ex[(comp * CD_TY + ty + 1) * CD_TX + tx], fyu);
             }
-            if (comp == 0)      cd2_output<ND, 0>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
-            else if (comp == 1) cd2_output<ND, 1>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
-            else if (ND == 3)   cd2_output<ND, 2>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
+            if (comp == 0)      cd2_output<ND, 0>(P, gx, gy, z, nv, q, fyu, pre, out, dt, corrector);
+            else if (comp == 1) cd2_output<ND, 1>(P, gx, gy, z, nv, q, fyu, pre, out, dt, corrector);
+            else if (ND == 3)   cd2_output<ND, 2>(P, gx, gy, z, nv, q, fyu, pre, out, dt, corrector);
             if (more) {
                 __syncthreads();
                 cd2_store_regs<ND>(ring + s0 * SLOT, st);
@@ -556,10 +577,11 @@ __global__ void __launch_bounds__(CD2_NT(3), 1) k_cd_tile3(FlowP P, CdT T, const
                 v.b[d] = ring + s * SLOT + tofs;
             }
             Cd2Part q;
+            Cd2Pre pre;
             const bool first = z == z0;
-            if (comp == 0)      cd2_fluxes<ND, 0>(P, v, gx, gy, z, top, first, fz, q);
-            else if (comp == 1) cd2_fluxes<ND, 1>(P, v, gx, gy, z, top, first, fz, q);
-            else                cd2_fluxes<ND, 2>(P, v, gx, gy, z, top, first, fz, q);
+            if (comp == 0)      { cd2_preload<ND, 0>(P, gx, gy, z, nv, u0, mu0, Vi, corrector, pre); cd2_fluxes<ND, 0>(P, v, gx, gy, z, top, first, fz, q); }
+            else if (comp == 1) { cd2_preload<ND, 1>(P, gx, gy, z, nv, u0, mu0, Vi, corrector, pre); cd2_fluxes<ND, 1>(P, v, gx, gy, z, top, first, fz, q); }
+            else                { cd2_preload<ND, 2>(P, gx, gy, z, nv, u0, mu0, Vi, corrector, pre); cd2_fluxes<ND, 2>(P, v, gx, gy, z, top, first, fz, q); }
             float4* exz = ex + (z & 1) * ND * CD_NT;
             exz[(comp * CD_TY + ty) * CD_TX + tx] = make_float4(q.fyl[0], q.fyl[1], q.fyl[2], q.fyl[3]);
             __syncthreads();                       // the lower-y-face fluxes of the plane are in shared memory; the ring reads of the plane are done
@@ -571,9 +593,9 @@ __global__ void __launch_bounds__(CD2_NT(3), 1) k_cd_tile3(FlowP P, CdT T, const
             } else {
                 unpack4(exz[(comp * CD_TY + ty + 1) * CD_TX + tx], fyu);
             }
-            if (comp == 0)      cd2_output<ND, 0>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
-            else if (comp == 1) cd2_output<ND, 1>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
-            else                cd2_output<ND, 2>(P, gx, gy, z, nv, q, fyu, u0, mu0, out, dt, Vi, corrector);
+            if (comp == 0)      cd2_output<ND, 0>(P, gx, gy, z, nv, q, fyu, pre, out, dt, corrector);
+            else if (comp == 1) cd2_output<ND, 1>(P, gx, gy, z, nv, q, fyu, pre, out, dt, corrector);
+            else                cd2_output<ND, 2>(P, gx, gy, z, nv, q, fyu, pre, out, dt, corrector);
             s0 = s0 + 1 == CD3_NP ? 0 : s0 + 1;
         }
     }
