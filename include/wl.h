@@ -92,6 +92,7 @@ typedef struct {
     int zc;              /* planes per tile of the vector kernels (0: 8) */
     long long pk_max_cells; /* levels >= 1 with at most this many cells run inside the persistent kernels (0: 1 M; < 0: none) */
     int pk_blocks_per_sm;   /* co-resident blocks per SM of the cooperative kernel (0: 2) */
+    int pk_fail;            /* test hook: treat the first cooperative / cluster launch as refused by the device (exercises the fallback) */
 } wl_tuning;
 
 /* Problem statement (grid size, boundary velocity, length scale, viscosity, BC type,

@@ -1019,9 +1019,10 @@ static void coarse_launch_one(wl_sim* s, const CoarseProg& prog)
     DevScal* ds = s->ds;
     double* part = s->pk_part;
     void* args[] = { (void*)&levs, (void*)&prog, (void*)&ds, (void*)&part };
-    cudaError_t e;
-    if (s->nd == 3) e = cudaLaunchCooperativeKernel((const void*)k_coarse<3>, dim3(s->pk_blocks), dim3(WL_VB), args, 0, s->st);
-    else            e = cudaLaunchCooperativeKernel((const void*)k_coarse<2>, dim3(s->pk_blocks), dim3(WL_VB), args, 0, s->st);
+    cudaError_t e = cudaErrorCooperativeLaunchTooLarge;
+    if (s->cfg.tune.pk_fail) { }                  // test hook: the device "refuses" the launch
+    else if (s->nd == 3) e = cudaLaunchCooperativeKernel((const void*)k_coarse<3>, dim3(s->pk_blocks), dim3(WL_VB), args, 0, s->st);
+    else                 e = cudaLaunchCooperativeKernel((const void*)k_coarse<2>, dim3(s->pk_blocks), dim3(WL_VB), args, 0, s->st);
     if (e != cudaSuccess) {
         // the grid cannot be co-scheduled on this device (a partitioned GPU: MIG, an MPS SM limit): from now on every level runs its
         // passes as stand-alone kernels, starting with this chain
@@ -1062,7 +1063,7 @@ static void coarse_launch(wl_sim* s, const CoarseProg& prog)
             P.op[P.n++] = prog.op[i++];
         }
         if (small) {
-            if (!wl_k_small_prog(s, P, C)) {        // the cluster could not be launched after all: the cooperative kernel from now on
+            if (s->cfg.tune.pk_fail || !wl_k_small_prog(s, P, C)) {        // the cluster could not be launched after all: the cooperative kernel from now on
                 cudaGetLastError();
                 s->small_cmax = 0;
                 coarse_launch_one(s, P);

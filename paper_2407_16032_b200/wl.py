@@ -47,7 +47,8 @@ class MG(C.Structure):
 
 class Tuning(C.Structure):
     _fields_ = [("no_fused", C.c_int), ("no_fast_a", C.c_int), ("no_bulk", C.c_int), ("no_block_levels", C.c_int),
-                ("no_tma_cd", C.c_int), ("zc", C.c_int), ("pk_max_cells", C.c_longlong), ("pk_blocks_per_sm", C.c_int)]
+                ("no_tma_cd", C.c_int), ("zc", C.c_int), ("pk_max_cells", C.c_longlong), ("pk_blocks_per_sm", C.c_int),
+                ("pk_fail", C.c_int)]
 
 
 class Config(C.Structure):

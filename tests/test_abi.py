@@ -34,7 +34,7 @@ def test_config_struct_layout_matches_header():
     from paper_2407_16032_b200 import wl
     assert C.sizeof(wl.Body) == 4 * (1 + 3 + 2 + 1 + 1 + 9 + 1 + 5 + 1)
     assert C.sizeof(wl.MG) == 4 * 5
-    assert C.sizeof(wl.Tuning) == 4 * 6 + 8 + 8              # six ints, one long long (8-aligned), one int + tail padding
+    assert C.sizeof(wl.Tuning) == 4 * 6 + 8 + 8              # six ints, one long long (8-aligned), two ints
     head = 4 * (1 + 3 + 1 + 3 + 1 + 3 + 1 + 1 + 4) + C.sizeof(wl.Body) + C.sizeof(wl.MG)
     assert wl.Config.tune.offset == (head + 7) // 8 * 8
     tail = 4 + 3 * C.sizeof(wl.Body) + 4 * 3 + 4 * 3          # nextra, extra[3], extra_op[3]; precision, tangent_param, tangent_index

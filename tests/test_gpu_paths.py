@@ -20,6 +20,7 @@ SWITCHES = [
     {"pk_max_cells": -1},                   # every level by stand-alone kernels
     {"no_bulk": 1},                         # pass A copies its planes with per-thread cp.async instead of TMA boxes
     {"no_tma_cd": 1},                       # conv_diff from the register-staged ring (k_cd_tile2) instead of the TMA-fed one
+    {"pk_fail": 1},                         # the device refuses the cluster and the cooperative launch: fallback to stand-alone passes
 ]
 
 
