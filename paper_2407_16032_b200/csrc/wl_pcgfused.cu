@@ -13,7 +13,11 @@
 // between two buffers (a block reads the OLD r and q of its neighbours' cells); the last sweep writes r back to where it
 // was, and a sweep that finds the smoother stopped applies the update still owed or copies r across, so after the call r
 // is where it was.  The planes of r, e, q (with halos) and x (own cells) arrive as TMA boxes, three planes ahead of use.
-// Levels this form does not take (periodic x or y, fewer than 68 cells along x, 2-D) keep the two-pass form.
+// A TMA box cannot wrap, so on a level that is periodic in x or y the arrays read with halos (r, e, q) carry periodic GHOST cells:
+// whoever writes cell 1 / n of a periodic direction also writes the ghost n+1 / 0 (the sweeps do it for r', e', q'; a small kernel
+// does it for r before the first sweep, since r comes from the residual / restriction / prolongation kernels, which wrap at load
+// time and keep no ghosts).  z wraps through the plane coordinate of the box.
+// Levels this form does not take (fewer than 68 cells along x, 2-D) keep the two-pass form.
 #include <cstdio>
 #include <cstring>
 #include "wl_internal.h"
@@ -69,13 +73,17 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
     const bool own = gx < vt.ngx, valid = own && c1 <= g.n[1];
     const int sy = (int)g.sy, sz = (int)g.sz;
     const int off_own = WL_OFF + c0 + ff_src(c1, g.n[1], 0) * sy;
+    // 1/D keeps no ghosts: where a thread's group stands on a periodic ghost (the first group past a ragged row end in x, the row
+    // past the last one in y) it takes 1/D of the cells the ghosts mirror
+    const bool wrapx = g.per[0] && c0 == g.n[0] + 1;
+    const int off_d = WL_OFF + (wrapx ? 1 : c0) + ff_src(c1, g.n[1], g.per[1]) * sy;
     const int idx_own = (ty + 1) * RW + 4 + 4 * tx;
     bool hrow = false, hrow_ld = false; int off_h = 0, idx_h = 0, hc0 = 0, hc1 = 0;
     if (tid < 2 * LX) {
         const int hr = tid >> 5, hx = tid & (LX - 1);
         hrow = true; hrow_ld = tix * LX + hx < vt.ngx;
         hc0 = 1 + 4 * (tix * LX + hx); hc1 = hr ? y0 + LY : y0 - 1;
-        off_h = WL_OFF + hc0 + ff_src(hc1, g.n[1], 0) * sy;
+        off_h = WL_OFF + hc0 + ff_src(hc1, g.n[1], g.per[1]) * sy;        // 1/D keeps no ghosts: the wrapped row
         idx_h = (hr ? LY + 1 : 0) * RW + 4 + 4 * hx;
     }
     bool hcol = false; int off_x = 0, idx_x = 0, xc0 = 0, xc1 = 0;
@@ -83,9 +91,18 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
         const int rr = (tid - 64) >> 1, side = tid & 1;
         hcol = true;
         xc0 = side ? x0 + 4 * LX : x0 - 1; xc1 = y0 + rr;
-        off_x = WL_OFF + ff_src(xc0, g.n[0], 0) + ff_src(xc1, g.n[1], 0) * sy;
+        off_x = WL_OFF + ff_src(xc0, g.n[0], g.per[0]) + ff_src(xc1, g.n[1], 0) * sy;
         idx_x = (rr + 1) * RW + (side ? 4 + 4 * LX : 3);
     }
+    // periodic ghosts of the arrays written here (see the head of the file): cell 1 -> ghost n+1, cell n -> ghost 0, per direction
+    const bool gx_lo = g.per[0] && c0 == 1, gx_hi = g.per[0] && c0 + 3 == g.n[0];
+    const bool gy_lo = g.per[1] && c1 == 1, gy_hi = g.per[1] && c1 == g.n[1];
+    auto ghosts = [&](float* __restrict__ a, int i, const float4& v) {
+        if (gx_lo) a[i + g.n[0]] = v.x;
+        if (gx_hi) a[i - c0] = v.w;
+        if (gy_lo) *reinterpret_cast<float4*>(a + i + g.n[1] * sy) = v;
+        if (gy_hi) *reinterpret_cast<float4*>(a + i - g.n[1] * sy) = v;
+    };
     const unsigned sraw = (unsigned)__cvta_generic_to_shared(raw);
     auto issue = [&](int p, int slot) {
         if (p >= z0 - 1 && p <= z1 + 1 && tid == 0) {
@@ -112,23 +129,24 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
 #pragma unroll
     for (int k = 0; k < 4; ++k) { cxl[k] = Lc; cxh[k] = Lc; d_in[k] = iDc; d_bz[k] = iDc; dh_in[k] = iDc; dh_bz[k] = iDc; }
     if (PLB) {
-        const int byo = ff_bnd(c1, g.n[1], 0), byh = ff_bnd(hc1, g.n[1], 0);
+        const int px = g.per[0], py = g.per[1];
+        const int byo = ff_bnd(c1, g.n[1], py), byh = ff_bnd(hc1, g.n[1], py);
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-            if (c0 + k == 1) cxl[k] = 0.0f;
-            if (c0 + k == g.n[0]) cxh[k] = 0.0f;
-            const int bo = byo + ff_bnd(c0 + k, g.n[0], 0), bh = byh + ff_bnd(hc0 + k, g.n[0], 0);
+            if (!px && c0 + k == 1) cxl[k] = 0.0f;
+            if (!px && c0 + k == g.n[0]) cxh[k] = 0.0f;
+            const int bo = byo + ff_bnd(c0 + k, g.n[0], px), bh = byh + ff_bnd(hc0 + k, g.n[0], px);
             d_in[k] = ff_pick(T, bo); d_bz[k] = ff_pick(T, bo + 1);
             dh_in[k] = ff_pick(T, bh); dh_bz[k] = ff_pick(T, bh + 1);
         }
-        if (c1 == 1) cyl = 0.0f;
-        if (c1 == g.n[1]) cyh = 0.0f;
-        const int bx = ff_bnd(xc0, g.n[0], 0) + ff_bnd(xc1, g.n[1], 0);
+        if (!py && c1 == 1) cyl = 0.0f;
+        if (!py && c1 == g.n[1]) cyh = 0.0f;
+        const int bx = ff_bnd(xc0, g.n[0], px) + ff_bnd(xc1, g.n[1], py);
         dx_in = ff_pick(T, bx); dx_bz = ff_pick(T, bx + 1);
     }
     auto load_iD = [&](int p, bool full) {    // GEN: 1/D of plane p at the positions the operands come from
         const int zo = ff_src(p, g.n[2], g.per[2]) * sz;
-        if (own) unpack4(ld4(iD, off_own + zo), d_in);
+        if (own || wrapx) unpack4(ld4(iD, off_d + zo), d_in);
         if (full && hrow_ld) unpack4(ld4(iD, off_h + zo), dh_in);
         if (full && hcol) dx_in = ld1(iD, off_x + zo);
     };
@@ -158,7 +176,9 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
                     const int i = off_own + p * sz;
                     float xv[4];
                     unpack4(*reinterpret_cast<const float4*>(st + 3 * PLR + 128 * ty + 4 * tx), xv);
-                    *reinterpret_cast<float4*>(rout + i) = make_float4(rn[0], rn[1], rn[2], rn[3]);
+                    const float4 rv = make_float4(rn[0], rn[1], rn[2], rn[3]);
+                    *reinterpret_cast<float4*>(rout + i) = rv;
+                    ghosts(rout, i, rv);
                     *reinterpret_cast<float4*>(x + i) = make_float4(xv[0] + alpha * ee[0], xv[1] + alpha * ee[1], xv[2] + alpha * ee[2], xv[3] + alpha * ee[3]);
                 }
             }
@@ -249,8 +269,11 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
         }
         if (valid) {
             const int i = off_own + z * sz;
-            *reinterpret_cast<float4*>(eout + i) = make_float4(zc[0], zc[1], zc[2], zc[3]);
-            *reinterpret_cast<float4*>(qout + i) = make_float4(qq[0], qq[1], qq[2], qq[3]);
+            const float4 ev = make_float4(zc[0], zc[1], zc[2], zc[3]), qv = make_float4(qq[0], qq[1], qq[2], qq[3]);
+            *reinterpret_cast<float4*>(eout + i) = ev;
+            *reinterpret_cast<float4*>(qout + i) = qv;
+            ghosts(eout, i, ev);
+            ghosts(qout, i, qv);
             // fp32 products summed over the thread's four cells, accumulated in fp64 once per plane
             float sg = qq[0] * zc[0], s2 = qq[0] * zrc[0], s3 = qq[0] * __fmul_rn(dc[0], qq[0]);
 #pragma unroll
@@ -391,10 +414,29 @@ __global__ void __launch_bounds__(WL_VB, 4) k_pcg_last(Grid g, VT vt, const int*
 
 static size_t ff_smem(int first) { return sizeof(float) * ((size_t)FF_S * (first ? FF_PLR : 3 * FF_PLR + FF_XB) + 2 * FF_PL) + 8 * FF_S + 8; }
 
-// 3-D, no wrap in x or y (a TMA box cannot wrap), whole float4 groups and at least 17 of them per row (32 threads along x), 32-bit offsets
+// 3-D, whole float4 groups and at least 17 of them per row (32 threads along x), 32-bit offsets
 int wl_pcg_fused_shape(int nd, const Grid& g, const VT& vt)
 {
-    return nd == 3 && !g.per[0] && !g.per[1] && g.n[0] % 4 == 0 && vt.lxl == 5 && g.nalloc < ((int64_t)1 << 31);
+    return nd == 3 && g.n[0] % 4 == 0 && vt.lxl == 5 && g.nalloc < ((int64_t)1 << 31);
+}
+
+// periodic ghost cells of one scalar array in x and y (interior rows / columns only: the stencil needs no corners)
+__global__ void k_wrap_ghosts(Grid g, float* __restrict__ a)
+{
+    const int64_t nx = g.per[0] ? (int64_t)g.n[1] * g.n[2] : 0, ny = g.per[1] ? (int64_t)g.n[0] * g.n[2] : 0;
+    for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < nx + ny; t += (int64_t)gridDim.x * blockDim.x) {
+        if (t < nx) {
+            const int c1 = 1 + (int)(t % g.n[1]), c2 = 1 + (int)(t / g.n[1]);
+            const int64_t row = gidx(g, 0, c1, c2);
+            a[row] = a[row + g.n[0]];
+            a[row + g.n[0] + 1] = a[row + 1];
+        } else {
+            const int64_t u = t - nx;
+            const int c0 = 1 + (int)(u % g.n[0]), c2 = 1 + (int)(u / g.n[0]);
+            a[gidx(g, c0, 0, c2)] = a[gidx(g, c0, g.n[1], c2)];
+            a[gidx(g, c0, g.n[1] + 1, c2)] = a[gidx(g, c0, 1, c2)];
+        }
+    }
 }
 
 // The smoother on level l as iters + 1 sweeps (see the head of this file).  Returns 0 when the level does not take this form.
@@ -422,6 +464,13 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
     if (!ptm_x) return 0;
     CUtensorMap tm_r = *wl_tensor_map_cached(s->tmc, ra, lv.g, FF_RW, 10), tm_e, tm_q, tm_x = *ptm_x;
     memset(&tm_e, 0, sizeof(tm_e)); memset(&tm_q, 0, sizeof(tm_q));
+    if (lv.g.per[0] || lv.g.per[1]) {          // r comes from kernels that keep no ghosts
+        ProfScope ps_(s, WLK_MISC, l > 0);
+        const int64_t n = (int64_t)lv.g.n[2] * (lv.g.n[0] + lv.g.n[1]);
+        int nb = (int)((n + 255) / 256);
+        if (nb > s->sm_count * 4) nb = s->sm_count * 4;
+        k_wrap_ghosts<<<nb, 256, 0, s->st>>>(lv.g, ra);
+    }
     {
         ProfScope ps_(s, WLK_PCG_MATVEC, l > 0);
         k_pcg_fused<1><<<grid, WL_VB, ff_smem(1), s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, 0, lv.L, lv.iD, lv.x, ra, rb, ea, eb, qa, qb, sc, s->rb,

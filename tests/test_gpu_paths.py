@@ -160,10 +160,14 @@ def test_smoother_removes_residual_mean_on_the_gpu():
     o.close(); g.close()
 
 
-# levels the one-sweep smoother (wl_pcgfused.cu) takes: 3-D, at least 68 cells along x, no wrap in x and y; with
+# levels the one-sweep smoother (wl_pcgfused.cu) takes: 3-D, at least 68 cells along x; with
 # pk_max_cells = -1 level 1 of the second case (128 x 16 x 12) is a stand-alone level too and takes it as well
 FUSED = [((128, 40, 24), (0, 0, 0), 1, "sphere", False), ((256, 32, 24), (0, 0, 1), 1, "torus", False),
-         ((160, 44, 24), (0, 0, 0), 1, "sphere", False)]          # the last: rows of 1.25 tiles, 5.5 tiles along y
+         ((160, 44, 24), (0, 0, 0), 1, "sphere", False),          # rows of 1.25 tiles, 5.5 tiles along y
+         # levels that wrap in x and / or y: the arrays read with halos carry periodic ghost cells (a TMA box cannot wrap)
+         ((136, 40, 24), (1, 1, 1), 0, "torus", False),           # ragged row end on a periodic x
+         ((256, 32, 24), (1, 1, 0), 0, "sphere", False),          # levels 0 and 1
+         ((160, 44, 24), (0, 1, 0), 1, "sphere", False)]          # ragged last row of tiles on a periodic y
 
 
 def _fused_levels(case):
