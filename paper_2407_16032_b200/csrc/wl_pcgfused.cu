@@ -24,6 +24,7 @@
 #include "wl_tma.cuh"
 
 #define FF_S 3                    // raw stages
+#define FF_BPS 2                  // resident blocks per SM of a fused sweep (the first sweep, with a third of the shared memory, runs 3)
 #define FF_RW 136                 // floats per shared row: cells x0-4 .. x0+131
 #define FF_PL (FF_RW * 10)        // floats per shared plane: rows y0-1 .. y0+8
 #define FF_PLR ((FF_PL + 31) / 32 * 32)
@@ -51,7 +52,7 @@ __device__ __forceinline__ float ff_dir(float ee, float rn, float d, float beta)
 // previous iteration are staged (one TMA box each per plane, halos included), r' and e' are formed at every position of
 // the plane, r' and x are stored for the tile's own cells, and the stencil runs on e' as in wl_pcgfast.cu.
 // acc: gamma = q'.e', q'.(iD r'), q'.(iD q'), and (FIRST) rho = e'.(r - m).
-template <int FIRST, int MODE>
+template <int FIRST, int MODE, int PER>
 __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, float Lc, float iDc, const FfTab& T, float alpha, float beta, float m,
                                         const float* __restrict__ L, const float* __restrict__ iD, float* __restrict__ x, float* __restrict__ rout,
                                         float* __restrict__ eout, float* __restrict__ qout, float* raw, float* ebuf, double (&acc)[4],
@@ -75,15 +76,16 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
     const int off_own = WL_OFF + c0 + ff_src(c1, g.n[1], 0) * sy;
     // 1/D keeps no ghosts: where a thread's group stands on a periodic ghost (the first group past a ragged row end in x, the row
     // past the last one in y) it takes 1/D of the cells the ghosts mirror
-    const bool wrapx = g.per[0] && c0 == g.n[0] + 1;
-    const int off_d = WL_OFF + (wrapx ? 1 : c0) + ff_src(c1, g.n[1], g.per[1]) * sy;
+    const int px = PER ? g.per[0] : 0, py = PER ? g.per[1] : 0;       // PER == 0: the level wraps in neither x nor y
+    const bool wrapx = px && c0 == g.n[0] + 1;
+    const int off_d = WL_OFF + (wrapx ? 1 : c0) + ff_src(c1, g.n[1], py) * sy;
     const int idx_own = (ty + 1) * RW + 4 + 4 * tx;
     bool hrow = false, hrow_ld = false; int off_h = 0, idx_h = 0, hc0 = 0, hc1 = 0;
     if (tid < 2 * LX) {
         const int hr = tid >> 5, hx = tid & (LX - 1);
         hrow = true; hrow_ld = tix * LX + hx < vt.ngx;
         hc0 = 1 + 4 * (tix * LX + hx); hc1 = hr ? y0 + LY : y0 - 1;
-        off_h = WL_OFF + hc0 + ff_src(hc1, g.n[1], g.per[1]) * sy;        // 1/D keeps no ghosts: the wrapped row
+        off_h = WL_OFF + hc0 + ff_src(hc1, g.n[1], py) * sy;        // 1/D keeps no ghosts: the wrapped row
         idx_h = (hr ? LY + 1 : 0) * RW + 4 + 4 * hx;
     }
     bool hcol = false; int off_x = 0, idx_x = 0, xc0 = 0, xc1 = 0;
@@ -91,13 +93,14 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
         const int rr = (tid - 64) >> 1, side = tid & 1;
         hcol = true;
         xc0 = side ? x0 + 4 * LX : x0 - 1; xc1 = y0 + rr;
-        off_x = WL_OFF + ff_src(xc0, g.n[0], g.per[0]) + ff_src(xc1, g.n[1], 0) * sy;
+        off_x = WL_OFF + ff_src(xc0, g.n[0], px) + ff_src(xc1, g.n[1], 0) * sy;
         idx_x = (rr + 1) * RW + (side ? 4 + 4 * LX : 3);
     }
     // periodic ghosts of the arrays written here (see the head of the file): cell 1 -> ghost n+1, cell n -> ghost 0, per direction
-    const bool gx_lo = g.per[0] && c0 == 1, gx_hi = g.per[0] && c0 + 3 == g.n[0];
-    const bool gy_lo = g.per[1] && c1 == 1, gy_hi = g.per[1] && c1 == g.n[1];
+    const bool gx_lo = px && c0 == 1, gx_hi = px && c0 + 3 == g.n[0];
+    const bool gy_lo = py && c1 == 1, gy_hi = py && c1 == g.n[1];
     auto ghosts = [&](float* __restrict__ a, int i, const float4& v) {
+        if (!PER) return;
         if (gx_lo) a[i + g.n[0]] = v.x;
         if (gx_hi) a[i - c0] = v.w;
         if (gy_lo) *reinterpret_cast<float4*>(a + i + g.n[1] * sy) = v;
@@ -129,7 +132,6 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
 #pragma unroll
     for (int k = 0; k < 4; ++k) { cxl[k] = Lc; cxh[k] = Lc; d_in[k] = iDc; d_bz[k] = iDc; dh_in[k] = iDc; dh_bz[k] = iDc; }
     if (PLB) {
-        const int px = g.per[0], py = g.per[1];
         const int byo = ff_bnd(c1, g.n[1], py), byh = ff_bnd(hc1, g.n[1], py);
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
@@ -210,6 +212,7 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
     float zm[4], zc[4], zp[4], zrc[4], zrp[4], dc[4], dp[4], dummy[4], dummy2[4];
     issue(zs - dir, FF_S - 1);
     issue(zs, 0);
+    issue(zs + dir, 1);
     if (GEN) load_iD(zs - dir, false);
     arrived(FF_S - 1);
     form(zs - dir, FF_S - 1, zm, dummy, dummy2, false);
@@ -218,7 +221,7 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
     form(zs, 0, zc, zrc, dc, true);
     __syncthreads();                          // slot FF_S-1 is free again
 #pragma unroll
-    for (int d = 1; d < FF_S; ++d) issue(zs + d * dir, d);
+    for (int d = 2; d < FF_S; ++d) issue(zs + d * dir, d);
     int sl = 0;                               // slot of plane z
     for (int n = z1 - z0, z = zs; n >= 0; --n, z += dir) {
         const int sn = sl + 1 == FF_S ? 0 : sl + 1;       // slot of the plane after z
@@ -326,8 +329,9 @@ __device__ __forceinline__ void ff_pointwise(const Grid& g, const VT& vt, int ti
 }
 
 // kprev: the iteration whose update (alpha, and the mean m when kprev == 1) this sweep applies; 0 in the first sweep
-template <int FIRST>
-__global__ void __launch_bounds__(WL_VB, 3) k_pcg_fused(Grid g, VT vt, const int* __restrict__ plain, float Lc, float iDc, int kprev,
+// PER: the level wraps in x or y (ghost cells maintained, 1/D taken from the mirrored cells); 0 keeps all of that out of the code
+template <int FIRST, int PER>
+__global__ void __launch_bounds__(WL_VB, FIRST ? 3 : FF_BPS) k_pcg_fused(Grid g, VT vt, const int* __restrict__ plain, float Lc, float iDc, int kprev,
                                                          const float* __restrict__ L, const float* __restrict__ iD, float* __restrict__ x,
                                                          const float* __restrict__ rin, float* __restrict__ rout, const float* __restrict__ ein,
                                                          float* __restrict__ eout, const float* __restrict__ qin, float* __restrict__ qout,
@@ -364,9 +368,11 @@ __global__ void __launch_bounds__(WL_VB, 3) k_pcg_fused(Grid g, VT vt, const int
     FfTab T;
     T.t0 = 1.0f / (-6.0f * Lc); T.t1 = 1.0f / (-5.0f * Lc); T.t2 = 1.0f / (-4.0f * Lc); T.t3 = 1.0f / (-3.0f * Lc);
     double acc[4] = { 0.0, 0.0, 0.0, 0.0 };
+    int mode_next = blockIdx.x < vt.ntiles ? plain[blockIdx.x] : 0;
     for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
-        const int mode = plain[tile];         // block-uniform
-#define FF_CALL(M) ff_tile<FIRST, M>(g, vt, tile, Lc, iDc, T, alpha, beta, m, L, iD, x, rout, eout, qout, raw, ebuf, acc, mbar, phases, &tm_r, &tm_e, &tm_q, &tm_x)
+        const int mode = mode_next;           // block-uniform; the next tile's is fetched a tile ahead of its use
+        mode_next = tile + gridDim.x < vt.ntiles ? plain[tile + gridDim.x] : 0;
+#define FF_CALL(M) ff_tile<FIRST, M, PER>(g, vt, tile, Lc, iDc, T, alpha, beta, m, L, iD, x, rout, eout, qout, raw, ebuf, acc, mbar, phases, &tm_r, &tm_e, &tm_q, &tm_x)
         if (mode == TM_PLI) FF_CALL(TM_PLI);
         else if (mode == TM_PLB) FF_CALL(TM_PLB);
         else FF_CALL(TM_GEN);
@@ -445,13 +451,19 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
     Level& lv = s->lev[l];
     if (!lv.r2 || !lv.q2 || iters < 1) return 0;
     PcgScal* sc = &s->ds->pcg[l];
-    int grid = lv.vt.ntiles < s->sm_count * 3 ? lv.vt.ntiles : s->sm_count * 3;
+    // persistent grids: FF_BPS blocks per SM for the fused sweeps (registers: no spills at 128), 3 for the first sweep
+    int grid = lv.vt.ntiles < s->sm_count * FF_BPS ? lv.vt.ntiles : s->sm_count * FF_BPS;
+    int grid1 = lv.vt.ntiles < s->sm_count * 3 ? lv.vt.ntiles : s->sm_count * 3;
     if (grid > WL_MAX_PARTIALS) grid = WL_MAX_PARTIALS;
+    if (grid1 > WL_MAX_PARTIALS) grid1 = WL_MAX_PARTIALS;
     if (!(s->cd_attr_set & 16)) {         // per handle: a process may hold handles on several devices
-        cudaFuncSetAttribute(k_pcg_fused<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ff_smem(1));
-        cudaFuncSetAttribute(k_pcg_fused<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ff_smem(0));
+        cudaFuncSetAttribute(k_pcg_fused<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ff_smem(1));
+        cudaFuncSetAttribute(k_pcg_fused<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ff_smem(1));
+        cudaFuncSetAttribute(k_pcg_fused<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ff_smem(0));
+        cudaFuncSetAttribute(k_pcg_fused<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ff_smem(0));
         s->cd_attr_set |= 16;
     }
+    const bool per = lv.g.per[0] || lv.g.per[1];
     float *ra = lv.r, *rb = lv.r2;            // ra: the residual as it stands
     float *ea = lv.e2, *eb = lv.e;            // ea: the direction of the previous iteration, eb: the one being written
     float *qa = lv.q2, *qb = lv.q;
@@ -464,7 +476,7 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
     if (!ptm_x) return 0;
     CUtensorMap tm_r = *wl_tensor_map_cached(s->tmc, ra, lv.g, FF_RW, 10), tm_e, tm_q, tm_x = *ptm_x;
     memset(&tm_e, 0, sizeof(tm_e)); memset(&tm_q, 0, sizeof(tm_q));
-    if (lv.g.per[0] || lv.g.per[1]) {          // r comes from kernels that keep no ghosts
+    if (per) {                                 // r comes from kernels that keep no ghosts
         ProfScope ps_(s, WLK_MISC, l > 0);
         const int64_t n = (int64_t)lv.g.n[2] * (lv.g.n[0] + lv.g.n[1]);
         int nb = (int)((n + 255) / 256);
@@ -473,8 +485,8 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
     }
     {
         ProfScope ps_(s, WLK_PCG_MATVEC, l > 0);
-        k_pcg_fused<1><<<grid, WL_VB, ff_smem(1), s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, 0, lv.L, lv.iD, lv.x, ra, rb, ea, eb, qa, qb, sc, s->rb,
-                                                         tm_r, tm_e, tm_q, tm_x);
+        auto kern = per ? k_pcg_fused<1, 1> : k_pcg_fused<1, 0>;
+        kern<<<grid1, WL_VB, ff_smem(1), s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, 0, lv.L, lv.iD, lv.x, ra, rb, ea, eb, qa, qb, sc, s->rb, tm_r, tm_e, tm_q, tm_x);
     }
     for (int k = 2; k <= iters; ++k) {
         float* t = ea; ea = eb; eb = t;
@@ -484,8 +496,8 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
         tm_q = *wl_tensor_map_cached(s->tmc, qa, lv.g, FF_RW, 10);
         {
             ProfScope ps_(s, WLK_PCG_FUSED, l > 0);
-            k_pcg_fused<0><<<grid, WL_VB, ff_smem(0), s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, k - 1, lv.L, lv.iD, lv.x, ra, rb, ea, eb, qa, qb, sc,
-                                                             s->rb, tm_r, tm_e, tm_q, tm_x);
+            auto kern = per ? k_pcg_fused<0, 1> : k_pcg_fused<0, 0>;
+            kern<<<grid, WL_VB, ff_smem(0), s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, k - 1, lv.L, lv.iD, lv.x, ra, rb, ea, eb, qa, qb, sc, s->rb, tm_r, tm_e, tm_q, tm_x);
         }
         t = ra; ra = rb; rb = t;
     }
