@@ -224,10 +224,11 @@ static size_t layout(wl_sim* s, const wl_config* c, void* base)
         int* plain = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
         int* uniform = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
         int* tile_live = (int*)cv.take(sizeof(int) * (size_t)vt.ntiles);
+        int* sched = fused ? (int*)cv.take(sizeof(int) * (size_t)vt.ntiles) : nullptr;
         if (s) {
             Level& lv = s->lev[l];
             lv.g = g; lv.L = L; lv.iD = iD; lv.x = x; lv.r = r; lv.e = e; lv.e2 = e2; lv.q = q; lv.r2 = r2; lv.q2 = q2;
-            lv.vt = vt; lv.plain = plain; lv.uniform = uniform; lv.tile_live = tile_live;
+            lv.vt = vt; lv.plain = plain; lv.uniform = uniform; lv.tile_live = tile_live; lv.sched = sched;
             lv.Lc = nd == 3 ? (float)(1 << l) : 1.0f;
             lv.iDc = 1.0f / (-(2.0f * nd) * lv.Lc);
         }

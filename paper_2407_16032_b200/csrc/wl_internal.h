@@ -27,6 +27,7 @@ struct Level {
     float* r2;   // second residual and A e buffers of the one-sweep PCG form (wl_pcgfused.cu); null on levels that do not take it
     float* q2;
     VT vt;       // vector tiling of this level
+    int* sched;     // levels of the one-sweep smoother: the order its blocks take the tiles in (tile | mode << 24), TM_GEN tiles first (k_tile_sched)
     int* tile_live; // per tile: number of coupled cells (iD != 0) in it, kept so that k_diag_flags can skip tiles the body cannot reach
     int* uniform; // per-tile flag: every face coefficient of every cell of the tile equals Lc
     int* plain;  // per-tile flag: the tile and its face-neighbour tiles are uniform (kernels skip L and iD loads)

@@ -152,6 +152,21 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
         if (full && hrow_ld) unpack4(ld4(iD, off_h + zo), dh_in);
         if (full && hcol) dx_in = ld1(iD, off_x + zo);
     };
+    // GEN: L and 1/D are plain loads, consumed in the iteration that issues them; what the next iterations will load is pulled into
+    // L2 a plane (L) or two (1/D) ahead, so that those loads wait for L2 and not for DRAM
+    auto pf = [](const float* a) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a)); };
+    auto prefetch_gen = [&](int pd, int pl) {
+        const int zo = ff_src(pd, g.n[2], g.per[2]) * sz;
+        if (own || wrapx) pf(iD + off_d + zo);
+        if (hrow_ld) pf(iD + off_h + zo);
+        if (hcol) pf(iD + off_x + zo);
+        if (valid && pl >= z0 && pl <= z1) {
+            const int i = off_own + pl * sz;
+            pf(L + i); if (tx == LX - 1) pf(L + i + 4);
+            pf(L + g.nalloc + i); if (ty == LY - 1) pf(L + g.nalloc + i + sy);
+            pf(L + 2 * g.nalloc + i + (dir > 0 ? sz : 0));
+        }
+    };
     // plane p from stage slot `slot`: r' and x stored for the own cells, e' -> registers and shared, iD r' and iD -> registers
     auto form = [&](int p, int slot, float (&ep)[4], float (&zr)[4], float (&dd)[4], bool full) {
         const float* st = raw + slot * SP;
@@ -213,7 +228,7 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
     issue(zs - dir, FF_S - 1);
     issue(zs, 0);
     issue(zs + dir, 1);
-    if (GEN) load_iD(zs - dir, false);
+    if (GEN) { load_iD(zs - dir, false); prefetch_gen(zs, zs); prefetch_gen(zs + dir, zs); }
     arrived(FF_S - 1);
     form(zs - dir, FF_S - 1, zm, dummy, dummy2, false);
     if (GEN) load_iD(zs, true);
@@ -228,6 +243,7 @@ __device__ __forceinline__ void ff_tile(const Grid& g, const VT& vt, int tile, f
         float lx[5] = { 0.f, 0.f, 0.f, 0.f, 0.f }, ly[4] = { 0.f, 0.f, 0.f, 0.f }, lyp[4] = { 0.f, 0.f, 0.f, 0.f };
         float lz[4] = { 0.f, 0.f, 0.f, 0.f }, lzp[4] = { 0.f, 0.f, 0.f, 0.f };
         if (GEN) {                            // 1/D of the next plane and the face coefficients of the own cells of plane z
+            prefetch_gen(z + 2 * dir, z + dir);
             load_iD(z + dir, true);
             if (valid) {
                 const int i = off_own + z * sz;
@@ -331,7 +347,7 @@ __device__ __forceinline__ void ff_pointwise(const Grid& g, const VT& vt, int ti
 // kprev: the iteration whose update (alpha, and the mean m when kprev == 1) this sweep applies; 0 in the first sweep
 // PER: the level wraps in x or y (ghost cells maintained, 1/D taken from the mirrored cells); 0 keeps all of that out of the code
 template <int FIRST, int PER>
-__global__ void __launch_bounds__(WL_VB, FIRST ? 3 : FF_BPS) k_pcg_fused(Grid g, VT vt, const int* __restrict__ plain, float Lc, float iDc, int kprev,
+__global__ void __launch_bounds__(WL_VB, FIRST ? 3 : FF_BPS) k_pcg_fused(Grid g, VT vt, const int* __restrict__ plain, const int* __restrict__ sched, float Lc, float iDc, int kprev,
                                                          const float* __restrict__ L, const float* __restrict__ iD, float* __restrict__ x,
                                                          const float* __restrict__ rin, float* __restrict__ rout, const float* __restrict__ ein,
                                                          float* __restrict__ eout, const float* __restrict__ qin, float* __restrict__ qout,
@@ -368,10 +384,11 @@ __global__ void __launch_bounds__(WL_VB, FIRST ? 3 : FF_BPS) k_pcg_fused(Grid g,
     FfTab T;
     T.t0 = 1.0f / (-6.0f * Lc); T.t1 = 1.0f / (-5.0f * Lc); T.t2 = 1.0f / (-4.0f * Lc); T.t3 = 1.0f / (-3.0f * Lc);
     double acc[4] = { 0.0, 0.0, 0.0, 0.0 };
-    int mode_next = blockIdx.x < vt.ntiles ? plain[blockIdx.x] : 0;
-    for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
-        const int mode = mode_next;           // block-uniform; the next tile's is fetched a tile ahead of its use
-        mode_next = tile + gridDim.x < vt.ntiles ? plain[tile + gridDim.x] : 0;
+    // tiles in the order of k_tile_sched (wl_poisson.cu): entry = tile | mode << 24, fetched a tile ahead of its use
+    int next = blockIdx.x < vt.ntiles ? sched[blockIdx.x] : 0;
+    for (int k = blockIdx.x; k < vt.ntiles; k += gridDim.x) {
+        const int tile = next & 0xffffff, mode = next >> 24;          // block-uniform
+        next = k + gridDim.x < vt.ntiles ? sched[k + gridDim.x] : 0;
 #define FF_CALL(M) ff_tile<FIRST, M, PER>(g, vt, tile, Lc, iDc, T, alpha, beta, m, L, iD, x, rout, eout, qout, raw, ebuf, acc, mbar, phases, &tm_r, &tm_e, &tm_q, &tm_x)
         if (mode == TM_PLI) FF_CALL(TM_PLI);
         else if (mode == TM_PLB) FF_CALL(TM_PLB);
@@ -449,7 +466,7 @@ __global__ void k_wrap_ghosts(Grid g, float* __restrict__ a)
 int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
 {
     Level& lv = s->lev[l];
-    if (!lv.r2 || !lv.q2 || iters < 1) return 0;
+    if (!lv.r2 || !lv.q2 || !lv.sched || iters < 1) return 0;
     PcgScal* sc = &s->ds->pcg[l];
     // persistent grids: FF_BPS blocks per SM for the fused sweeps (registers: no spills at 128), 3 for the first sweep
     int grid = lv.vt.ntiles < s->sm_count * FF_BPS ? lv.vt.ntiles : s->sm_count * FF_BPS;
@@ -486,7 +503,7 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
     {
         ProfScope ps_(s, WLK_PCG_MATVEC, l > 0);
         auto kern = per ? k_pcg_fused<1, 1> : k_pcg_fused<1, 0>;
-        kern<<<grid1, WL_VB, ff_smem(1), s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, 0, lv.L, lv.iD, lv.x, ra, rb, ea, eb, qa, qb, sc, s->rb, tm_r, tm_e, tm_q, tm_x);
+        kern<<<grid1, WL_VB, ff_smem(1), s->st>>>(lv.g, lv.vt, lv.plain, lv.sched, lv.Lc, lv.iDc, 0, lv.L, lv.iD, lv.x, ra, rb, ea, eb, qa, qb, sc, s->rb, tm_r, tm_e, tm_q, tm_x);
     }
     for (int k = 2; k <= iters; ++k) {
         float* t = ea; ea = eb; eb = t;
@@ -497,7 +514,7 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
         {
             ProfScope ps_(s, WLK_PCG_FUSED, l > 0);
             auto kern = per ? k_pcg_fused<0, 1> : k_pcg_fused<0, 0>;
-            kern<<<grid, WL_VB, ff_smem(0), s->st>>>(lv.g, lv.vt, lv.plain, lv.Lc, lv.iDc, k - 1, lv.L, lv.iD, lv.x, ra, rb, ea, eb, qa, qb, sc, s->rb, tm_r, tm_e, tm_q, tm_x);
+            kern<<<grid, WL_VB, ff_smem(0), s->st>>>(lv.g, lv.vt, lv.plain, lv.sched, lv.Lc, lv.iDc, k - 1, lv.L, lv.iD, lv.x, ra, rb, ea, eb, qa, qb, sc, s->rb, tm_r, tm_e, tm_q, tm_x);
         }
         t = ra; ra = rb; rb = t;
     }

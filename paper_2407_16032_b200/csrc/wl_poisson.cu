@@ -937,6 +937,36 @@ __global__ void __launch_bounds__(WL_VB, WL_PK_MINB) k_coarse(const LevDev* levs
     coarse_body<ND>(levs, prog, ds, part);
 }
 
+// The order in which the one-sweep smoother (wl_pcgfused.cu) hands out the tiles of a level: block b of G takes entries b, b + G, ...
+// A TM_GEN tile costs about two uniform ones (L and 1/D are loaded), and with the tiles dealt in index order the blocks that met two
+// or three of them finished last (C4: 219 us per sweep against 205 without a body).  So the TM_GEN tiles go first, one per block
+// as far as they reach, and the uniform tiles follow in index order (neighbouring blocks keep working on neighbouring memory): the
+// deal stays static, so the per-block partial sums and with them the results stay the same from run to run.
+__global__ void __launch_bounds__(1024) k_tile_sched(int ntiles, const int* __restrict__ plain, int* __restrict__ sched)
+{
+    __shared__ int cnt[1024];
+    const int tid = threadIdx.x, per = (ntiles + 1023) / 1024;
+    const int t0 = tid * per < ntiles ? tid * per : ntiles, t1 = t0 + per < ntiles ? t0 + per : ntiles;
+    int c = 0;
+    for (int t = t0; t < t1; ++t) c += plain[t] == TM_GEN ? 1 : 0;
+    cnt[tid] = c;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {       // inclusive scan
+        const int v = tid >= o ? cnt[tid - o] : 0;
+        __syncthreads();
+        cnt[tid] += v;
+        __syncthreads();
+    }
+    const int ngen = cnt[1023];
+    int ig = cnt[tid] - c;                     // TM_GEN tiles before t0
+    int ip = ngen + (t0 - ig);                 // uniform tiles before t0 come after all the TM_GEN tiles
+    for (int t = t0; t < t1; ++t) {
+        const int mode = plain[t];
+        if (mode == TM_GEN) sched[ig++] = t | (mode << 24);
+        else                sched[ip++] = t | (mode << 24);
+    }
+}
+
 // ================================================================== host launchers
 #define DISPATCH(s, cls, coarse, kern, T, ...)                                               \
     do {                                                                                     \
@@ -983,6 +1013,7 @@ void wl_k_poisson_update(wl_sim* s)
             ProfScope ps_(s, WLK_POISSON_UPDATE, l > 0);
             int nb = (lv.vt.ntiles + 255) / 256;
             k_plain_mode<<<nb < 64 ? nb : 64, 256, 0, s->st>>>(lv.g, lv.vt, lv.uniform, lv.plain);
+            if (lv.sched) k_tile_sched<<<1, 1024, 0, s->st>>>(lv.vt.ntiles, lv.plain, lv.sched);
         }
     }
 }

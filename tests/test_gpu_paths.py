@@ -209,7 +209,13 @@ def test_one_sweep_smoother_matches_the_oracle_and_the_two_pass_form(case, iters
         res = []
         for l in _fused_levels(case):
             r0 = _smoother_inputs(o, g, l)
+            g.prof_enable(True)
             xg, rg = _run_smoother(o, g, l, r0, iters)
+            prof = g.prof_read()
+            g.prof_enable(False)
+            # no silent change of path: the one-sweep form is iters - 1 fused sweeps, the two-pass form none
+            nfused = sum(n for k, (_ms, n) in prof.items() if k.startswith("pcg_fused"))
+            assert nfused == (0 if "no_fused" in sw else iters - 1), (sw, l, prof)
             tol = TOL if iters == 1 else 1e-4
             assert relerr(xg, O(o, "x", l)) <= tol, (sw, l)
             assert np.abs(rg - O(o, "r", l)).max() <= tol * np.abs(r0).max(), (sw, l)
