@@ -239,12 +239,14 @@ __device__ __forceinline__ void march(const Grid& g, const VPos& p, const Src& S
 
 // ---------------------------------------------------------------- diagonal + uniform flags
 // D = -sum_i (L[c,i] + L[c+d_i,i]); iD = 1/D if |D| > 2n*1e-6 else 0 (R-O).  A tile is uniform
-// when every face coefficient of every cell in it has its body-free value.
+// when every face coefficient of every cell in it has its body-free value.  flags[tile]: bit 0 = uniform; bits 1..6 = the
+// layer of cells along the tile's -x, +x, -y, +y, -z, +z face holds a cell that is not (what the tile beyond that face has to
+// know, k_plain_mode).
 template <int ND>
 __global__ void __launch_bounds__(WL_VB) k_diag_flags(Grid g, VT vt, const float* __restrict__ L, float Lc, float* __restrict__ iD, int* __restrict__ uniform,
                                                       int* __restrict__ tile_live, CellBox B, PcgScal* sc, RedBuf rb)
 {
-    __shared__ int live_s;
+    __shared__ int live_s, bad_s;
     double v[1] = { 0.0 };
     for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
         VPos p = vt_pos(g, vt, tile);
@@ -258,10 +260,13 @@ __global__ void __launch_bounds__(WL_VB) k_diag_flags(Grid g, VT vt, const float
                 continue;
             }
         }
-        if (threadIdx.x == 0) live_s = 0;
+        if (threadIdx.x == 0) { live_s = 0; bad_s = 0; }
         __syncthreads();
-        int ok = 1, cnt = 0;
+        int bad = 0, cnt = 0;
         if (p.nv > 0) {
+            const int lx4 = 4 << vt.lxl, ly = WL_VB >> vt.lxl;
+            const int xlo = 1 + lx4 * (tile % vt.ntx), xhi = min(xlo + lx4 - 1, g.n[0]);
+            const int ylo = 1 + ly * ((tile / vt.ntx) % vt.nty), yhi = min(ylo + ly - 1, g.n[1]);
             const int64_t rc = (int64_t)WL_OFF + (int64_t)p.c1 * g.sy;
             Coef C, R;
             for (int z = p.z0; z <= p.z1; ++z) {
@@ -280,7 +285,15 @@ __global__ void __launch_bounds__(WL_VB) k_diag_flags(Grid g, VT vt, const float
                     if (k < p.nv) {
                         bool same = C.x[k] == R.x[k] && C.x[k + 1] == R.x[k + 1] && C.y[k] == R.y[k] && C.yp[k] == R.yp[k];
                         if (ND == 3) same = same && C.z[k] == R.z[k] && C.zp[k] == R.zp[k];
-                        if (!same) ok = 0;
+                        if (!same) {
+                            bad |= 1;
+                            if (p.c0 + k == xlo) bad |= 2;
+                            if (p.c0 + k == xhi) bad |= 4;
+                            if (p.c1 == ylo) bad |= 8;
+                            if (p.c1 == yhi) bad |= 16;
+                            if (ND == 3 && z == p.z0) bad |= 32;
+                            if (ND == 3 && z == p.z1) bad |= 64;
+                        }
                     }
                 }
                 st4(iD, i, d, p.nv);
@@ -288,8 +301,9 @@ __global__ void __launch_bounds__(WL_VB) k_diag_flags(Grid g, VT vt, const float
         }
         v[0] += (double)cnt;
         if (cnt) atomicAdd(&live_s, cnt);
-        ok = __syncthreads_and(ok);
-        if (threadIdx.x == 0) { uniform[tile] = ok; tile_live[tile] = live_s; }
+        if (bad) atomicOr(&bad_s, bad);
+        __syncthreads();
+        if (threadIdx.x == 0) { uniform[tile] = bad_s ^ 1; tile_live[tile] = live_s; }
         __syncthreads();
     }
     if (grid_reduce<1, OpSum>(v, rb)) {
@@ -299,14 +313,15 @@ __global__ void __launch_bounds__(WL_VB) k_diag_flags(Grid g, VT vt, const float
 
 // The PCG passes recompute e' = beta e + iD r at the six neighbours of every cell, so a tile may
 // only use analytic coefficients if the cells one step outside it are body-free too: its mode is
-// TM_GEN unless it and its face-neighbour tiles (periodic wrap) are uniform.  A missing neighbour
-// is a non-periodic domain boundary, whose faces carry L = 0 (R-O) and need no values beyond.
+// TM_GEN unless it is uniform and so is the layer of cells that each face-neighbour tile (periodic wrap) turns
+// towards it.  A missing neighbour is a non-periodic domain boundary, whose faces carry L = 0 (R-O) and need no
+// values beyond.
 __global__ void k_plain_mode(Grid g, VT vt, const int* __restrict__ self, int* __restrict__ plain)
 {
     for (int tile = blockIdx.x * blockDim.x + threadIdx.x; tile < vt.ntiles; tile += gridDim.x * blockDim.x) {
         int t[3] = { tile % vt.ntx, (tile / vt.ntx) % vt.nty, tile / (vt.ntx * vt.nty) };
         const int nt[3] = { vt.ntx, vt.nty, vt.ntz };
-        int ok = self[tile];
+        int ok = self[tile] & 1;
         for (int d = 0; d < 3 && ok; ++d)
             for (int s = -1; s <= 1; s += 2) {
                 int q[3] = { t[0], t[1], t[2] };
@@ -315,7 +330,8 @@ __global__ void k_plain_mode(Grid g, VT vt, const int* __restrict__ self, int* _
                     if (!g.per[d]) continue;
                     q[d] = q[d] < 0 ? nt[d] - 1 : 0;
                 }
-                ok = ok && self[q[0] + vt.ntx * (q[1] + vt.nty * q[2])];
+                // the neighbour beyond my +d face shows me its -d layer (bit 1 + 2d), the one beyond my -d face its +d layer
+                ok = ok && !((self[q[0] + vt.ntx * (q[1] + vt.nty * q[2])] >> (s > 0 ? 1 + 2 * d : 2 + 2 * d)) & 1);
             }
         int mode = TM_GEN;
         if (ok) {
