@@ -175,7 +175,7 @@ int wl_gen_get_fields_f64(wl_sim* s, double* u, double* p, int lane, int on_devi
 int wl_gen_dbg_get(wl_sim* s, const char* name, int level, int lane, double* out, size_t n);
 // wl_small.cu
 int wl_small_max_cluster(wl_sim* s);
-int wl_small_blocks(const Grid& g);
+int wl_small_blocks(const Grid& g, int cmax);
 int wl_k_small_prog(wl_sim* s, const CoarseProg& P, int C);
 // wl_poisson.cu
 void wl_k_poisson_update(wl_sim* s);                 // iD on level 0, coarse L and iD

@@ -1091,8 +1091,7 @@ static int op_small_blocks(wl_sim* s, const CoarseOp& op)
     if (!s->tiny_on) return 0;
     if (s->small_cmax < 0) s->small_cmax = wl_small_max_cluster(s);      // once per handle
     const int walked = op.kind == COP_RESTRICT ? op.level + 1 : op.level;
-    const int C = wl_small_blocks(s->lev[walked].g);
-    return C <= s->small_cmax ? C : 0;
+    return wl_small_blocks(s->lev[walked].g, s->small_cmax);
 }
 
 // runs a chain of coarse-level passes: consecutive passes of the same kind (whole-GPU cooperative kernel / one on-chip cluster)

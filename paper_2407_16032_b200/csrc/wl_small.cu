@@ -22,9 +22,9 @@
 namespace cg = cooperative_groups;
 
 #define SM_NT 1024                     // threads per block
-#define SM_K 4                         // cells per thread
-#define SM_CHUNK (SM_NT * SM_K)        // cells per block
-#define SM_SHIFT 12                    // log2(SM_CHUNK)
+#define SM_K 4                         // cells per thread, at most
+#define SM_CHUNK (SM_NT * SM_K)        // cells per block, at most
+#define SM_ONE 2048                    // a level of at most this many cells is smoothed by ONE block (block barriers only)
 
 struct SmShared {
     float e[SM_CHUNK];                 // CG direction of the block's cells (read by the other blocks of the cluster)
@@ -41,11 +41,30 @@ struct SmCtx {
     int C;                             // blocks in the cluster
     int rank;
     int phase;
+    int nt;                            // C == 1: the first nt threads of the block (whole warps) take part in barriers and sums
 };
+
+// How a level of N cells is spread over a cluster of C blocks: Cl blocks own 2^shift cells each (1024, 2048 or 4096: one, two or
+// four per thread).  A sum over the cluster costs ~1900 cycles, over one block ~900, a stencil sweep ~1100 per cell of a thread:
+// up to SM_ONE cells one block does it all; above, as many blocks as give every thread one cell.
+__host__ __device__ inline void sm_spread(int N, int C, int& Cl, int& shift)
+{
+    Cl = 1;
+    if (N > SM_ONE) while (Cl * 1024 < N && Cl < C) Cl <<= 1;
+    shift = 10;
+    while ((Cl << shift) < N && shift < 12) ++shift;
+}
+
+__device__ __forceinline__ void sm_bar(int nt)
+{
+    if (nt >= SM_NT) __syncthreads();
+    else if (nt > 32) asm volatile("bar.sync 1, %0;" ::"r"(nt) : "memory");
+    else __syncwarp();
+}
 
 __device__ __forceinline__ void sm_sync(const SmCtx& c)
 {
-    if (c.C == 1) __syncthreads();
+    if (c.C == 1) sm_bar(c.nt);
     else cg::this_cluster().sync();    // barrier.cluster arrive.release / wait.acquire: orders shared AND global memory in the cluster
 }
 
@@ -64,13 +83,15 @@ __device__ __forceinline__ void sm_reduce(SmCtx& c, double (&v)[NV])
         const double w = warp_red<OpSum>(v[k]);
         if (lane == 0) sh.warp[k][wid] = w;
     }
-    __syncthreads();
     if (c.C == 1) {
+        const int nw = c.nt >> 5;
+        sm_bar(c.nt);
 #pragma unroll
-        for (int k = 0; k < NV; ++k) v[k] = warp_red<OpSum>(sh.warp[k][lane]);      // 32 warps: one value per lane; every warp redundantly
-        __syncthreads();                                                        // warp[] may be rewritten by the next reduction
+        for (int k = 0; k < NV; ++k) v[k] = warp_red<OpSum>(lane < nw ? sh.warp[k][lane] : 0.0);   // one value per lane; every warp redundantly
+        sm_bar(c.nt);                                                           // warp[] may be rewritten by the next reduction
         return;
     }
+    __syncthreads();
     cg::cluster_group cl = cg::this_cluster();
     double (*slots)[16] = sh.slots[c.phase & 1];
     if (wid == 0) {
@@ -109,12 +130,23 @@ __device__ __forceinline__ int64_t sm_gidx(const Grid& g, int c0, int c1, int c2
 // cell are looked up by cell number (tables in shared memory) and read from this block's shared memory or, for the few owned
 // by another block, through the cluster window.
 template <int ND>
-__device__ __forceinline__ void sm_smooth(SmCtx& c, const LevDev& lv, PcgScal* sc, int iters)
+__device__ __forceinline__ void sm_smooth(SmCtx& cl, const LevDev& lv, PcgScal* sc, int iters)
 {
-    SmShared& sh = *c.sh;
+    SmShared& sh = *cl.sh;
     const Grid& g = lv.g;
     const int N = g.n[0] * g.n[1] * g.n[2];
     const int tid = threadIdx.x;
+    int Cl, shift;
+    sm_spread(N, cl.C, Cl, shift);
+    const int K = 1 << (shift - 10), cmask = (1 << shift) - 1;        // cells per thread, chunk - 1
+    SmCtx c = cl;
+    if (Cl == 1) {
+        // one block, and of it only the warps that own cells: block-local barriers and sums; everybody else goes straight to the
+        // barrier that ends the pass (the caller's)
+        c.C = 1;
+        c.nt = N >= SM_NT ? SM_NT : (N + 31) & ~31;
+        if (cl.rank != 0 || tid >= c.nt) return;
+    }
     const int st[3] = { 1, g.n[0], g.n[0] * g.n[1] };
     float x[SM_K], r[SM_K], q[SM_K], d[SM_K];
     bool ok[SM_K];
@@ -125,10 +157,10 @@ __device__ __forceinline__ void sm_smooth(SmCtx& c, const LevDev& lv, PcgScal* s
     };
 #pragma unroll
     for (int j = 0; j < SM_K; ++j) {
-        const int k = c.rank * SM_CHUNK + j * SM_NT + tid, loc = j * SM_NT + tid;
-        ok[j] = k < N;
+        const int k = (c.rank << shift) + j * SM_NT + tid, loc = j * SM_NT + tid;
+        ok[j] = j < K && k < N;
         x[j] = r[j] = q[j] = d[j] = 0.0f;
-        if (!ok[j]) { sh.e[loc] = 0.0f; continue; }
+        if (!ok[j]) { if (j < K) sh.e[loc] = 0.0f; continue; }
         int cc[3];
         sm_coords(g, k, cc[0], cc[1], cc[2]);
         const int gi = (int)sm_gidx<ND>(g, cc[0], cc[1], cc[2]);
@@ -145,7 +177,7 @@ __device__ __forceinline__ void sm_smooth(SmCtx& c, const LevDev& lv, PcgScal* s
     }
     // operand of the stencil at cell kk: this block's shared memory, or another block's through the cluster window
     auto E = [&](int kk) -> float {
-        const int rr = kk >> SM_SHIFT, off = kk & (SM_CHUNK - 1);
+        const int rr = kk >> shift, off = kk & cmask;
         if (rr == c.rank) return sh.e[off];
         return *cg::this_cluster().map_shared_rank(&sh.e[off], rr);
     };
@@ -161,7 +193,7 @@ __device__ __forceinline__ void sm_smooth(SmCtx& c, const LevDev& lv, PcgScal* s
     for (int j = 0; j < SM_K; ++j) {
         if (d[j] != 0.0f) r[j] -= m;
         const float z = __fmul_rn(d[j], r[j]);
-        sh.e[j * SM_NT + tid] = z;
+        if (j < K) sh.e[j * SM_NT + tid] = z;
         if (ok[j]) w1[0] += (double)z * (double)r[j];
     }
     sm_reduce<1>(c, w1);                              // (its barrier also publishes e)
@@ -189,7 +221,7 @@ __device__ __forceinline__ void sm_smooth(SmCtx& c, const LevDev& lv, PcgScal* s
         double r2[1] = { 0.0 };
 #pragma unroll
         for (int j = 0; j < SM_K; ++j) {
-            x[j] += alpha * sh.e[j * SM_NT + tid];
+            if (j < K) x[j] += alpha * sh.e[j * SM_NT + tid];
             r[j] -= alpha * q[j];
             if (ok[j]) r2[0] += (double)__fmul_rn(d[j], r[j]) * (double)r[j];
         }
@@ -202,16 +234,17 @@ __device__ __forceinline__ void sm_smooth(SmCtx& c, const LevDev& lv, PcgScal* s
 #pragma unroll
         for (int j = 0; j < SM_K; ++j) {
             const int loc = j * SM_NT + tid;
-            sh.e[loc] = __fmaf_rn(beta, sh.e[loc], __fmul_rn(d[j], r[j]));
+            if (j < K) sh.e[loc] = __fmaf_rn(beta, sh.e[loc], __fmul_rn(d[j], r[j]));
         }
         sm_sync(c);                                   // the new direction is visible to the whole cluster
     }
 #pragma unroll
     for (int j = 0; j < SM_K; ++j)
-        if (ok[j]) { const int gi = offset(c.rank * SM_CHUNK + j * SM_NT + tid); lv.x[gi] = x[j]; lv.r[gi] = r[j]; }
+        if (ok[j]) { const int gi = offset((c.rank << shift) + j * SM_NT + tid); lv.x[gi] = x[j]; lv.r[gi] = r[j]; }
     if (c.rank == 0 && tid == 0) {
         sc->rsum = 0.0; sc->nlive = v[1]; sc->rho = rho; sc->rho0 = rho0; sc->live = live; sc->stop_k = done;
     }
+    cl.phase = c.phase;
 }
 
 // ---------------------------------------------------------------- residual restriction (R-S): r_c = sum of the 2^n children; x_c = 0
@@ -274,6 +307,7 @@ __global__ void __launch_bounds__(SM_NT, 1) k_small(const LevDev* levs, const __
     c.C = (int)gridDim.x;                               // the launch is one cluster
     c.rank = (int)blockIdx.x;
     c.phase = 0;
+    c.nt = SM_NT;
     for (int o = 0; o < prog.n; ++o) {
         const CoarseOp op = prog.op[o];
         if (threadIdx.x == 0) {
@@ -316,13 +350,14 @@ int wl_small_max_cluster(wl_sim* s)
     return 0;
 }
 
-// blocks a level needs in k_small
-int wl_small_blocks(const Grid& g)
+// blocks of a cluster of at most cmax that k_small spreads a level over (sm_spread); 0: the level is too large for such a cluster
+int wl_small_blocks(const Grid& g, int cmax)
 {
     const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
-    int C = 1;
-    while ((long long)C * SM_CHUNK < N && C < 1024) C <<= 1;
-    return C;
+    if (cmax < 1 || N > (long long)cmax * SM_CHUNK) return 0;
+    int Cl, shift;
+    sm_spread((int)N, cmax, Cl, shift);
+    return Cl;
 }
 
 // one launch: the chain `prog` over small levels, as one cluster of `C` blocks.  Returns 0 if the launch failed.
