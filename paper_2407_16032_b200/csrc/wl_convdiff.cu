@@ -139,12 +139,17 @@ __device__ float f_at(const FlowP& P, const float* __restrict__ w, const float* 
 
 // ====================================================================== the tile kernel
 #define CD_TX 32                       // threads along x, four cells each
-#define CD_TY 8                        // rows per block
+#define CD2_TY 8                       // rows per block of k_cd_tile2 (one block of 256 x ND threads per SM)
+#define CD3_TY 4                       // rows per block of k_cd_tile3: two resident blocks of 128 x 3 threads beat one of 256 x 3 (630 -> 587 us on C4)
+#define CD_TY CD2_TY                   // the register-staged loaders below belong to k_cd_tile2
 #define CD_NT (CD_TX * CD_TY)
 #define CD_G (CD_TX + 2)               // float4 groups per shared row: cells bx-4 .. bx+4*CD_TX+3
 #define CD_W (4 * CD_G)                // floats per shared row
 #define CD_R (CD_TY + 4)               // shared rows: by-2 .. by+CD_TY+1
 #define CD_PLANE (CD_W * CD_R)         // floats per component per plane
+#define CD3_NT (CD_TX * CD3_TY)        // the same for k_cd_tile3
+#define CD3_R (CD3_TY + 4)
+#define CD3_PLANE (CD_W * CD3_R)
 #define CD_NP 5                        // ring of planes z-2 .. z+2
 
 __device__ __forceinline__ int wrap_any(int c, int N)      // 1..N for any c
@@ -210,15 +215,19 @@ struct CdT { int ntx, nty, ntz, ntiles, zc; };
 // cells of the three components (a flux is the same expression of the same operands whichever thread evaluates it).
 // view of the ring for one thread: b[dz + 2] points at the thread's own float4 of component 0 in plane z+dz, so that
 // every stencil read is one shared load at a compile-time offset (component, row and group offsets are immediates)
+// (TY: rows per block, which fixes the distance between the components of a plane)
+template <int TY>
 struct CdView2 { const float* b[CD_NP]; };
-__device__ __forceinline__ void v4(const CdView2& v, int comp, int dz, int dy, int dg, float* o)
+template <int TY>
+__device__ __forceinline__ void v4(const CdView2<TY>& v, int comp, int dz, int dy, int dg, float* o)
 {
-    const float4 t = *reinterpret_cast<const float4*>(v.b[dz + 2] + comp * CD_PLANE + dy * CD_W + 4 * dg);
+    const float4 t = *reinterpret_cast<const float4*>(v.b[dz + 2] + comp * (CD_W * (TY + 4)) + dy * CD_W + 4 * dg);
     o[0] = t.x; o[1] = t.y; o[2] = t.z; o[3] = t.w;
 }
-__device__ __forceinline__ float v1(const CdView2& v, int comp, int dz, int dy, int col)
+template <int TY>
+__device__ __forceinline__ float v1(const CdView2<TY>& v, int comp, int dz, int dy, int col)
 {
-    return v.b[dz + 2][comp * CD_PLANE + dy * CD_W + col];
+    return v.b[dz + 2][comp * (CD_W * (TY + 4)) + dy * CD_W + col];
 }
 #define CD2_NT(ND) (CD_NT * (ND))
 #define CD2_STAGE(ND) ((CD_ITEMS(ND) + CD2_NT(ND) - 1) / CD2_NT(ND))
@@ -253,8 +262,8 @@ struct Cd2Part {
 
 // fluxes of component I at the thread's four cells of plane gz.  fz: in (unless `first`) the flux through the lower z
 // face left by the previous plane; out the flux through the upper z face.
-template <int ND, int I>
-__device__ __forceinline__ void cd2_fluxes(const FlowP& P, const CdView2& v, int gx, int gy, int gz, bool top, bool first, float (&fz)[4], Cd2Part& o)
+template <int ND, int I, int TY>
+__device__ __forceinline__ void cd2_fluxes(const FlowP& P, const CdView2<TY>& v, int gx, int gy, int gz, bool top, bool first, float (&fz)[4], Cd2Part& o)
 {
     const Grid& g = P.g;
     const float nu = P.nu;
@@ -436,7 +445,7 @@ __global__ void __launch_bounds__(CD2_NT(ND), 1) k_cd_tile2(FlowP P, CdT T, cons
     float4* ex = reinterpret_cast<float4*>(ring + NP * SLOT);      // [ND][CD_TY][CD_TX] lower-y-face fluxes of the plane
     const int comp = threadIdx.x / CD_NT, t2 = threadIdx.x - comp * CD_NT;
     const float Vi = ds->vel[comp];
-    CdView2 v;
+    CdView2<CD2_TY> v;
     const int tx = t2 & (CD_TX - 1), ty = t2 / CD_TX;
     const int tofs = (ty + 2) * CD_W + 4 * (tx + 1);          // the thread's own group inside a plane
     const bool top = ty == CD_TY - 1;
@@ -509,7 +518,7 @@ __global__ void __launch_bounds__(CD2_NT(ND), 1) k_cd_tile2(FlowP P, CdT T, cons
 // No thread touches a global load for the ring, no register staging, and ONE block barrier per plane (the hand-over
 // of the y-face fluxes, double-buffered) instead of three.
 #define CD3_NP 6
-__global__ void __launch_bounds__(CD2_NT(3), 1) k_cd_tile3(FlowP P, CdT T, const float* __restrict__ u0, const float* __restrict__ mu0,
+__global__ void __launch_bounds__(3 * CD3_NT, 2) k_cd_tile3(FlowP P, CdT T, const float* __restrict__ u0, const float* __restrict__ mu0,
                                                            float* __restrict__ out, const DevScal* __restrict__ ds, int corrector,
                                                            const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1,
                                                            const __grid_constant__ CUtensorMap tm2)
@@ -519,16 +528,16 @@ __global__ void __launch_bounds__(CD2_NT(3), 1) k_cd_tile3(FlowP P, CdT T, const
     float* ring = reinterpret_cast<float*>(cd_smem);
     const Grid& g = P.g;
     const float dt = ds->dt;
-    constexpr int SLOT = ND * CD_PLANE;            // floats per ring slot (a multiple of 32: slots stay 128-byte aligned)
-    float4* ex = reinterpret_cast<float4*>(ring + CD3_NP * SLOT);          // [2][ND][CD_TY][CD_TX] lower-y-face fluxes
+    constexpr int SLOT = ND * CD3_PLANE;            // floats per ring slot (a multiple of 32: slots stay 128-byte aligned)
+    float4* ex = reinterpret_cast<float4*>(ring + CD3_NP * SLOT);          // [2][ND][CD3_TY][CD_TX] lower-y-face fluxes
     const unsigned sring = (unsigned)__cvta_generic_to_shared(ring);
-    const unsigned mbar = (unsigned)__cvta_generic_to_shared(ex + 2 * ND * CD_NT);     // [CD3_NP] slot barriers
-    const int comp = threadIdx.x / CD_NT, t2 = threadIdx.x - comp * CD_NT;
+    const unsigned mbar = (unsigned)__cvta_generic_to_shared(ex + 2 * ND * CD3_NT);     // [CD3_NP] slot barriers
+    const int comp = threadIdx.x / CD3_NT, t2 = threadIdx.x - comp * CD3_NT;
     const float Vi = ds->vel[comp];
-    CdView2 v;
+    CdView2<CD3_TY> v;
     const int tx = t2 & (CD_TX - 1), ty = t2 / CD_TX;
     const int tofs = (ty + 2) * CD_W + 4 * (tx + 1);          // the thread's own group inside a plane
-    const bool top = ty == CD_TY - 1;
+    const bool top = ty == CD3_TY - 1;
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int k = 0; k < CD3_NP; ++k) mbar_init(mbar + 8u * k, 1);
@@ -538,7 +547,7 @@ __global__ void __launch_bounds__(CD2_NT(3), 1) k_cd_tile3(FlowP P, CdT T, const
     for (int tile = blockIdx.x; tile < T.ntiles; tile += gridDim.x) {
         const int tix = tile % T.ntx, rem = tile / T.ntx;
         const int tiy = rem % T.nty, tiz = rem / T.nty;
-        const int bx = 1 + 4 * CD_TX * tix, by = 1 + CD_TY * tiy;
+        const int bx = 1 + 4 * CD_TX * tix, by = 1 + CD3_TY * tiy;
         const int z0 = 1 + T.zc * tiz, z1 = min(z0 + T.zc - 1, g.n[2]);
         const int gx = bx + 4 * tx, gy = by + ty;
         int nv = g.n[0] - gx + 1;
@@ -550,8 +559,8 @@ __global__ void __launch_bounds__(CD2_NT(3), 1) k_cd_tile3(FlowP P, CdT T, const
             const int cz = src_coord(p, g.n[2], g.per[2]);
             mbar_expect_tx(bar, (unsigned)(SLOT * 4));
             tma_box3(dst, &tm0, WL_OFF + bx - 4, by - 2, cz, bar);
-            tma_box3(dst + 4u * CD_PLANE, &tm1, WL_OFF + bx - 4, by - 2, cz, bar);
-            tma_box3(dst + 8u * CD_PLANE, &tm2, WL_OFF + bx - 4, by - 2, cz, bar);
+            tma_box3(dst + 4u * CD3_PLANE, &tm1, WL_OFF + bx - 4, by - 2, cz, bar);
+            tma_box3(dst + 8u * CD3_PLANE, &tm2, WL_OFF + bx - 4, by - 2, cz, bar);
         };
         auto arrived = [&](int slot) {
             mbar_wait(mbar + 8u * (unsigned)slot, (phases >> slot) & 1u);
@@ -582,8 +591,8 @@ __global__ void __launch_bounds__(CD2_NT(3), 1) k_cd_tile3(FlowP P, CdT T, const
             if (comp == 0)      { cd2_preload<ND, 0>(P, gx, gy, z, nv, u0, mu0, Vi, corrector, pre); cd2_fluxes<ND, 0>(P, v, gx, gy, z, top, first, fz, q); }
             else if (comp == 1) { cd2_preload<ND, 1>(P, gx, gy, z, nv, u0, mu0, Vi, corrector, pre); cd2_fluxes<ND, 1>(P, v, gx, gy, z, top, first, fz, q); }
             else                { cd2_preload<ND, 2>(P, gx, gy, z, nv, u0, mu0, Vi, corrector, pre); cd2_fluxes<ND, 2>(P, v, gx, gy, z, top, first, fz, q); }
-            float4* exz = ex + (z & 1) * ND * CD_NT;
-            exz[(comp * CD_TY + ty) * CD_TX + tx] = make_float4(q.fyl[0], q.fyl[1], q.fyl[2], q.fyl[3]);
+            float4* exz = ex + (z & 1) * ND * CD3_NT;
+            exz[(comp * CD3_TY + ty) * CD_TX + tx] = make_float4(q.fyl[0], q.fyl[1], q.fyl[2], q.fyl[3]);
             __syncthreads();                       // the lower-y-face fluxes of the plane are in shared memory; the ring reads of the plane are done
             if (threadIdx.x == 0 && z + 4 <= z1 + 2) issue(z + 4, s0);     // into the slot plane z-2 occupied; needed two steps from now
             float fyu[4];
@@ -591,7 +600,7 @@ __global__ void __launch_bounds__(CD2_NT(3), 1) k_cd_tile3(FlowP P, CdT T, const
 #pragma unroll
                 for (int k = 0; k < 4; ++k) fyu[k] = q.fyu[k];
             } else {
-                unpack4(exz[(comp * CD_TY + ty + 1) * CD_TX + tx], fyu);
+                unpack4(exz[(comp * CD3_TY + ty + 1) * CD_TX + tx], fyu);
             }
             if (comp == 0)      cd2_output<ND, 0>(P, gx, gy, z, nv, q, fyu, pre, out, dt, corrector);
             else if (comp == 1) cd2_output<ND, 1>(P, gx, gy, z, nv, q, fyu, pre, out, dt, corrector);
@@ -663,11 +672,11 @@ __global__ void __launch_bounds__(128) k_cd_band(FlowP P, const float* __restric
 }
 
 // ====================================================================== host launcher
-static CdT cd_tiling(const wl_sim* s, const Grid& g)
+static CdT cd_tiling(const wl_sim* s, const Grid& g, int rows)
 {
     CdT T;
     T.ntx = (g.n[0] + 4 * CD_TX - 1) / (4 * CD_TX);
-    T.nty = (g.n[1] + CD_TY - 1) / CD_TY;
+    T.nty = (g.n[1] + rows - 1) / rows;
     T.zc = 1; T.ntz = 1;
     if (s->nd == 3) {
         // planes per tile: long marches amortise the four halo planes; keep >= ~6 tiles per resident block
@@ -684,7 +693,6 @@ static CdT cd_tiling(const wl_sim* s, const Grid& g)
 void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out, int corrector)
 {
     FlowP P = wl_flowp(s);
-    CdT T = cd_tiling(s, P.g);
     const size_t smem2 = sizeof(float) * (size_t)(s->nd == 3 ? CD_NP : 1) * s->nd * CD_PLANE + sizeof(float4) * (size_t)s->nd * CD_NT;
     if (!(s->cd_attr_set & 2)) {
         cudaFuncSetAttribute(k_cd_tile2<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(float) * CD_NP * 3 * CD_PLANE + sizeof(float4) * 3 * CD_NT));
@@ -696,19 +704,21 @@ void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out,
     CUtensorMap tm[3];
     if (cd3)
         for (int c = 0; c < 3 && cd3; ++c) {
-            const CUtensorMap* pm = wl_tensor_map_cached(s->tmc, w + c * P.g.nalloc, P.g, CD_W, CD_R);
+            const CUtensorMap* pm = wl_tensor_map_cached(s->tmc, w + c * P.g.nalloc, P.g, CD_W, CD3_R);
             cd3 = pm != nullptr;
             if (pm) tm[c] = *pm;
         }
     if (cd3) {
-        const size_t smem3 = sizeof(float) * CD3_NP * 3 * CD_PLANE + sizeof(float4) * 2 * 3 * CD_NT + 8 * CD3_NP + 16;
+        const CdT T = cd_tiling(s, P.g, CD3_TY);
+        const size_t smem3 = sizeof(float) * CD3_NP * 3 * CD3_PLANE + sizeof(float4) * 2 * 3 * CD3_NT + 8 * CD3_NP + 16;
         if (!(s->cd_attr_set & 4)) {
             cudaFuncSetAttribute(k_cd_tile3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3);
             s->cd_attr_set |= 4;
         }
         ProfScope ps(s, WLK_CONVDIFF);
-        k_cd_tile3<<<T.ntiles, CD2_NT(3), smem3, s->st>>>(P, T, u0, s->mu0, out, s->ds, corrector, tm[0], tm[1], tm[2]);
+        k_cd_tile3<<<T.ntiles, 3 * CD3_NT, smem3, s->st>>>(P, T, u0, s->mu0, out, s->ds, corrector, tm[0], tm[1], tm[2]);
     } else {
+        const CdT T = cd_tiling(s, P.g, CD2_TY);
         ProfScope ps(s, WLK_CONVDIFF);
         if (s->nd == 3) k_cd_tile2<3><<<T.ntiles, CD2_NT(3), smem2, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
         else            k_cd_tile2<2><<<T.ntiles, CD2_NT(2), smem2, s->st>>>(P, T, w, u0, s->mu0, out, s->ds, corrector);
