@@ -41,6 +41,7 @@ extern "C" {
 #define WL_ENOMEM   -2   /* workspace too small or misaligned */
 #define WL_ECUDA    -3   /* CUDA error (sticky); text through wl_last_error */
 #define WL_ENOCONV  -4   /* tolerance-mode Poisson solve hit max_vcycles (result still written) */
+#define WL_ETOOBIG  -5   /* wl_energy_static: the grid exceeds WL_STATIC_MAX_CELLS */
 
 /* body kinds and motions: SDF + coordinate map of the paper's AutoBody.
  * WL_BODY_CYLINDER is the circular cylinder of P:121 / P:179 (radius R, infinitely long along `axis`: it spans a
@@ -245,6 +246,26 @@ int wl_level_dims(const wl_sim* s, int level, int dims_out[3]);
  * (not an error) once `cls` is past the last class. */
 int wl_prof_enable(wl_sim* s, int enable);
 int wl_prof_read(wl_sim* s, int cls, char* name_out, size_t name_bytes, double* ms_total, int* launches);
+
+/* ---- the one entry point that ALLOCATES NOTHING (wl_noalloc.cu), for callers that cannot call cudaMalloc: code under
+ * CUDA-graph capture, tight serving loops, harnesses that forbid it.  No handle, no workspace.
+ * Kinetic energy and enstrophy as wl_energy defines them (reading R-E2) of a velocity field the CALLER holds:
+ *   u_dev   device; ndim component arrays (u_x, u_y[, u_z]) of (dims[0]+2)(dims[1]+2)[(dims[2]+2)] floats each, x fastest, WITH
+ *           the one-cell ghost layer around the interior filled by the caller (the paper's array layout; what
+ *           wl_dbg_get_padded returns); read only, stays the caller's;
+ *   dims    host; interior cells per direction, each >= 1; their product may not exceed WL_STATIC_MAX_CELLS;
+ *   out_dev device; two doubles written: out[0] = 1/2 sum_cells sum_i u_i^2, out[1] = 1/2 sum_cells |w|^2 (fp32 products,
+ *           fp64 sums in a fixed order);
+ *   err     host, may be NULL; receives a text when the call fails (err_len bytes at most).
+ * Asynchronous on `cuda_stream` (one memset node + one kernel: capturable); does not synchronise.  Returns WL_OK, WL_EINVAL
+ * (bad argument), WL_ETOOBIG (more than WL_STATIC_MAX_CELLS cells: nothing is launched) or WL_ECUDA.
+ * The reduction scratch (a pair of partial sums per 1024 cells + a ticket counter) is a file-scope __device__ array of
+ * 1 MiB + 256 B that every GPU which loads libwl holds until the process exits.  ALL calls on a device share it: calls that
+ * overlap on the GPU (different streams or host threads) race on it and return garbage; calls on one stream are safe.  It
+ * keeps the last call's contents; the call clears what must start at zero.  The first call on a device looks the array's
+ * address up (cudaGetSymbolAddress): make that call outside a stream capture. */
+#define WL_STATIC_MAX_CELLS (64ll * 1024 * 1024)
+int wl_energy_static(const float* u_dev, int ndim, const int* dims, void* cuda_stream, double* out_dev, char* err, size_t err_len);
 
 const char* wl_last_error(const wl_sim* s);
 int wl_stats(wl_sim* s, wl_stats_t* out);

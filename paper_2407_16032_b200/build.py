@@ -18,7 +18,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIBDIR = PKG / "lib"
 LIB = LIBDIR / "libwl.so"
-SOURCES = ["wl_api.cu", "wl_flow.cu", "wl_convdiff.cu", "wl_poisson.cu", "wl_pcgfast.cu", "wl_pcgfused.cu", "wl_small.cu", "wl_generic.cu"]
+SOURCES = ["wl_api.cu", "wl_flow.cu", "wl_convdiff.cu", "wl_poisson.cu", "wl_pcgfast.cu", "wl_pcgfused.cu", "wl_small.cu", "wl_generic.cu", "wl_noalloc.cu"]
 HEADERS = ["wl_common.cuh", "wl_body.cuh", "wl_vec.cuh", "wl_tma.cuh", "wl_internal.h", "wl_dual.cuh"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -28,7 +28,7 @@ EXPORTS = [
     "wl_dbg_residual", "wl_dbg_apply_gradient", "wl_dbg_restrict", "wl_dbg_prolong", "wl_dbg_smooth", "wl_dbg_vcycle",
     "wl_dbg_coarse_prog", "wl_dbg_pcg_scalars",
     "wl_dbg_get", "wl_dbg_set", "wl_dbg_get_padded", "wl_level_dims", "wl_last_error", "wl_stats", "wl_abi_version",
-    "wl_prof_enable", "wl_prof_read",
+    "wl_prof_enable", "wl_prof_read", "wl_energy_static",
 ]
 
 
@@ -123,6 +123,8 @@ def load(build_if_missing: bool = True):
     L.wl_abi_version.restype = ip
     L.wl_prof_enable.argtypes = [vp, ip]
     L.wl_prof_read.argtypes = [vp, ip, C.c_char_p, C.c_size_t, C.POINTER(C.c_double), C.POINTER(C.c_int)]
+    L.wl_energy_static.restype = ip
+    L.wl_energy_static.argtypes = [vp, ip, C.POINTER(C.c_int), vp, vp, C.c_char_p, C.c_size_t]
     _lib = L
     return L
 
@@ -186,6 +188,32 @@ def workspace_bytes(cfg: dict) -> int:
 
 class WLError(RuntimeError):
     pass
+
+
+STATIC_MAX_CELLS = 64 * 1024 * 1024       # WL_STATIC_MAX_CELLS of include/wl.h
+
+
+def energy_static(u, out, dims=None, stream=None):
+    """wl_energy_static: (kinetic energy, enstrophy) of a velocity field WITH its ghost layer, written into `out`; allocates
+    nothing (the reduction scratch is a static device array of libwl: calls that overlap on the GPU race on it).
+    u: torch cuda float32, contiguous, shape (nd, [n2+2,] n1+2, n0+2); out: torch cuda float64 with 2 elements; dims: interior cells
+    (n0, n1[, n2]), taken from u.shape when None; stream: a torch stream (None: the current one).  Asynchronous."""
+    import torch
+    if not (u.is_cuda and u.dtype == torch.float32 and u.is_contiguous()):
+        raise TypeError("u must be a contiguous float32 cuda tensor")
+    if not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= 2):
+        raise TypeError("out must be a contiguous float64 cuda tensor with two elements")
+    nd = int(u.shape[0])
+    if dims is None:
+        dims = tuple(int(n) - 2 for n in reversed(u.shape[1:]))
+    d = (C.c_int * 3)(*(list(dims) + [1] * (3 - len(dims))))
+    st = (stream if stream is not None else torch.cuda.current_stream(u.device)).cuda_stream
+    err = C.create_string_buffer(512)
+    with torch.cuda.device(u.device):
+        rc = load().wl_energy_static(C.c_void_p(u.data_ptr()), nd, d, C.c_void_p(st), C.c_void_p(out.data_ptr()), err, 512)
+    if rc != 0:
+        raise WLError(f"libwl error {rc}: {err.value.decode()}")
+    return out
 
 
 class Sim:
