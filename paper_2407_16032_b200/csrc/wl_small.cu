@@ -121,6 +121,28 @@ __device__ __forceinline__ int64_t sm_gidx(const Grid& g, int c0, int c1, int c2
     return (int64_t)WL_OFF + (c0 + 1) + (int64_t)(c1 + 1) * g.sy + (ND == 3 ? (int64_t)(c2 + 1) * g.sz : 0);
 }
 
+// prolongation + increment at ONE fine cell (R-S): e = P x_c (piecewise constant) at the cell and its 2 ND neighbours; returns e at the
+// cell and, in `acc`, (A_f e) there.  Used by the stand-alone pass (sm_prolong) and by the smoother that absorbs the pass into its
+// loading phase: the same expression, so the same bits either way.
+template <int ND>
+__device__ __forceinline__ float sm_prolong_cell(const LevDev& lf, const LevDev& lc, const int (&cc)[3], int64_t i, float& acc)
+{
+    const Grid &gf = lf.g, &gc = lc.g;
+    const int64_t gst[3] = { 1, gf.sy, gf.sz };
+    const float ec = lc.x[sm_gidx<ND>(gc, cc[0] >> 1, cc[1] >> 1, cc[2] >> 1)];
+    acc = 0.0f;
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+        int a[3] = { cc[0], cc[1], cc[2] }, b[3] = { cc[0], cc[1], cc[2] };
+        a[d] = cc[d] > 0 ? cc[d] - 1 : (gf.per[d] ? gf.n[d] - 1 : cc[d]);              // across a wall the coefficient is zero
+        b[d] = cc[d] < gf.n[d] - 1 ? cc[d] + 1 : (gf.per[d] ? 0 : cc[d]);
+        const float el = lc.x[sm_gidx<ND>(gc, a[0] >> 1, a[1] >> 1, a[2] >> 1)];
+        const float eh = lc.x[sm_gidx<ND>(gc, b[0] >> 1, b[1] >> 1, b[2] >> 1)];
+        acc += lf.L[d * gf.nalloc + i + gst[d]] * (eh - ec) - lf.L[d * gf.nalloc + i] * (ec - el);
+    }
+    return ec;
+}
+
 // ---------------------------------------------------------------- Jacobi-PCG smoother (R-T, R-T2), on chip
 //   r <- r - mean(r over the coupled cells) on those cells; z = e = iD r; rho0 = rho = r.z; |rho| < tau: return
 //   k = 1..iters: q = A e; gamma = q.e; gamma = 0 or not finite: return; alpha = rho/gamma; x += alpha e; r -= alpha q;
@@ -130,8 +152,10 @@ __device__ __forceinline__ int64_t sm_gidx(const Grid& g, int c0, int c1, int c2
 // cell are looked up by cell number (tables in shared memory) and read from this block's shared memory or, for the few owned
 // by another block, through the cluster window.
 template <int ND>
-__device__ __forceinline__ void sm_smooth(SmCtx& cl, const LevDev& lv, PcgScal* sc, int iters)
+__device__ __forceinline__ void sm_smooth(SmCtx& cl, const LevDev& lv, PcgScal* sc, int iters, const LevDev* coarse)
 {
+    // coarse != null: the prolongation from that level (x += P x_c, r -= A P x_c) has not been run as a pass of its own and is
+    // applied here, while x and r are loaded
     SmShared& sh = *cl.sh;
     const Grid& g = lv.g;
     const int N = g.n[0] * g.n[1] * g.n[2];
@@ -174,6 +198,12 @@ __device__ __forceinline__ void sm_smooth(SmCtx& cl, const LevDev& lv, PcgScal* 
             sh.Lhi[i][loc] = lv.L[i * g.nalloc + gi + gst[i]];
         }
         x[j] = lv.x[gi]; r[j] = lv.r[gi]; d[j] = lv.iD[gi];
+        if (coarse) {
+            float acc;
+            const float ec = sm_prolong_cell<ND>(lv, *coarse, cc, gi, acc);
+            x[j] += ec;
+            r[j] -= acc;
+        }
     }
     // operand of the stencil at cell kk: this block's shared memory, or another block's through the cluster window
     auto E = [&](int kk) -> float {
@@ -274,24 +304,14 @@ __device__ __forceinline__ void sm_restrict(const SmCtx& c, const LevDev& lf, co
 template <int ND>
 __device__ __forceinline__ void sm_prolong(const SmCtx& c, const LevDev& lf, const LevDev& lc)
 {
-    const Grid &gf = lf.g, &gc = lc.g;
+    const Grid& gf = lf.g;
     const int N = gf.n[0] * gf.n[1] * gf.n[2];
-    const int64_t gst[3] = { 1, gf.sy, gf.sz };
     for (int k = c.rank * SM_NT + threadIdx.x; k < N; k += c.C * SM_NT) {
         int cc[3];
         sm_coords(gf, k, cc[0], cc[1], cc[2]);
         const int64_t i = sm_gidx<ND>(gf, cc[0], cc[1], cc[2]);
-        const float ec = lc.x[sm_gidx<ND>(gc, cc[0] >> 1, cc[1] >> 1, cc[2] >> 1)];
-        float acc = 0.0f;
-#pragma unroll
-        for (int d = 0; d < ND; ++d) {
-            int a[3] = { cc[0], cc[1], cc[2] }, b[3] = { cc[0], cc[1], cc[2] };
-            a[d] = cc[d] > 0 ? cc[d] - 1 : (gf.per[d] ? gf.n[d] - 1 : cc[d]);              // across a wall the coefficient is zero
-            b[d] = cc[d] < gf.n[d] - 1 ? cc[d] + 1 : (gf.per[d] ? 0 : cc[d]);
-            const float el = lc.x[sm_gidx<ND>(gc, a[0] >> 1, a[1] >> 1, a[2] >> 1)];
-            const float eh = lc.x[sm_gidx<ND>(gc, b[0] >> 1, b[1] >> 1, b[2] >> 1)];
-            acc += lf.L[d * gf.nalloc + i + gst[d]] * (eh - ec) - lf.L[d * gf.nalloc + i] * (ec - el);
-        }
+        float acc;
+        const float ec = sm_prolong_cell<ND>(lf, lc, cc, i, acc);
         lf.x[i] += ec;
         lf.r[i] -= acc;
     }
@@ -308,14 +328,18 @@ __global__ void __launch_bounds__(SM_NT, 1) k_small(const LevDev* levs, const __
     c.rank = (int)blockIdx.x;
     c.phase = 0;
     c.nt = SM_NT;
+    bool absorbed = false;                              // the previous op was a prolongation left to the smoother that follows it
     for (int o = 0; o < prog.n; ++o) {
         const CoarseOp op = prog.op[o];
+        // prolong(l+1 -> l) followed by smooth(l): the smoother loads x and r of level l anyway and applies the prolongation while it
+        // does (one pass over the level arrays and one cluster barrier less; the same arithmetic)
+        if (op.kind == COP_PROLONG && o + 1 < prog.n && prog.op[o + 1].kind == COP_SMOOTH && prog.op[o + 1].level == op.level) { absorbed = true; continue; }
         if (threadIdx.x == 0) {
             la = levs[op.level];
-            lb = levs[op.level + (op.kind == COP_SMOOTH ? 0 : 1)];
+            lb = levs[op.level + (op.kind == COP_SMOOTH && !absorbed ? 0 : 1)];
         }
         __syncthreads();
-        if (op.kind == COP_SMOOTH) sm_smooth<ND>(c, la, &ds->pcg[op.level], op.iters);
+        if (op.kind == COP_SMOOTH) { sm_smooth<ND>(c, la, &ds->pcg[op.level], op.iters, absorbed ? &lb : nullptr); absorbed = false; }
         else if (op.kind == COP_RESTRICT) sm_restrict<ND>(c, la, lb);
         else sm_prolong<ND>(c, la, lb);
         sm_sync(c);                                     // the pass's global writes are visible to every block; la / lb are free
