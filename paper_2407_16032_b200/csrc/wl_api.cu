@@ -250,12 +250,13 @@ extern "C" int wl_abi_version(void) { return 2; }
 // ------------------------------------------------------------------ the step
 static void bc_all(wl_sim* s, float* u) { wl_k_bc(s, u); }
 
-static int solve(wl_sim* s)
+// defer_x: the caller runs apply_gradient next and nothing else reads x (the last smoother call may leave its final update to it)
+static int solve(wl_sim* s, bool defer_x)
 {
     const wl_mg& mg = s->cfg.mg;
     int nv = 0;
     if (mg.fixed_vcycles > 0) {
-        for (; nv < mg.fixed_vcycles; ++nv) { wl_k_vcycle(s, 0); wl_k_smooth(s, 0, mg.smooth_iters, nv + 1 < mg.fixed_vcycles); }
+        for (; nv < mg.fixed_vcycles; ++nv) { wl_k_vcycle(s, 0); wl_k_smooth(s, 0, mg.smooth_iters, nv + 1 < mg.fixed_vcycles ? 1 : (defer_x ? -1 : 0)); }
         s->res[s->solve_slot] = -1.0;
     } else {
         double res = 0.0;
@@ -294,7 +295,7 @@ static int project(wl_sim* s, float* u, float w)
     NvtxRange nv("project!");
     solver_scratch(s, u);
     wl_k_residual(s, u, w);
-    int rc = solve(s);
+    int rc = solve(s, true);
     wl_k_apply_gradient(s, u);
     return rc;
 }

@@ -518,12 +518,16 @@ int wl_k_smooth_fused(wl_sim* s, int l, int iters, int need_r)
         }
         t = ra; ra = rb; rb = t;
     }
-    {
+    if (need_r < 0 && l == 0) {
+        // nobody but apply_gradient reads x of level 0 now: it adds alpha e on the fly (4 instead of 12 bytes per cell)
+        s->pend_e = eb;
+        s->pend_k = iters;
+    } else {
         // the last update brings r back to lv.r: in place when it is there already
         float* rout = lv.r;
         int g2 = lv.vt.ntiles < s->sm_count * 8 ? lv.vt.ntiles : s->sm_count * 8;
         ProfScope ps_(s, WLK_PCG_UPDATE, l > 0);
-        k_pcg_last<<<g2, WL_VB, 0, s->st>>>(lv.g, lv.vt, lv.plain, iters, lv.iD, lv.x, ra, rout, eb, qb, sc, need_r);
+        k_pcg_last<<<g2, WL_VB, 0, s->st>>>(lv.g, lv.vt, lv.plain, iters, lv.iD, lv.x, ra, rout, eb, qb, sc, need_r > 0 ? 1 : 0);
     }
     cudaMemsetAsync(&sc->rsum, 0, sizeof(double), s->st);    // the mean of r has been removed (R-T2)
     return 1;

@@ -450,21 +450,33 @@ __global__ void __launch_bounds__(WL_VB, WL_R_MINB) k_residual(Grid g, VT vt, co
 
 // ---------------------------------------------------------------- project!, second half
 // (P:88 kernel): u[c,i] -= L[c,i] (x[c] - x[c-d_i]); p = x / pscale
-template <int ND, int MODE>
+// PEND: the smoother left its last update to this kernel (wl_pcgfused.cu): x stands for x + a e wherever it is read (x itself is not
+// rewritten: the next solve starts from p).
+template <int ND, int MODE, int PEND>
 __device__ __forceinline__ void gradient_tile(const Grid& g, const VPos& p, float* u, const float* L, float Lc,
-                                              const float* x, float* pr, float isc)
+                                              const float* xa, float* pr, float isc, const float* e, float a)
 {
+    struct {
+        const float* x; const float* e; float a;
+        __device__ __forceinline__ float4 v(int64_t j) const
+        {
+            float4 t = ld4(x, j);
+            if (PEND) { const float4 s = ld4(e, j); t.x = t.x + a * s.x; t.y = t.y + a * s.y; t.z = t.z + a * s.z; t.w = t.w + a * s.w; }
+            return t;
+        }
+        __device__ __forceinline__ float s(int64_t j) const { float t = ld1(x, j); if (PEND) t = t + a * ld1(e, j); return t; }
+    } X = { xa, e, a };
     const int64_t rc = (int64_t)WL_OFF + (int64_t)p.c1 * g.sy;
     const int64_t rm = (int64_t)WL_OFF + (int64_t)nb_lo(p.c1, g.n[1], g.per[1]) * g.sy;
     float zm[4] = { 0.f, 0.f, 0.f, 0.f };
-    if (ND == 3) unpack4(ld4(x, rc + p.c0 + (int64_t)nb_lo(p.z0, g.n[2], g.per[2]) * g.sz), zm);
+    if (ND == 3) unpack4(X.v(rc + p.c0 + (int64_t)nb_lo(p.z0, g.n[2], g.per[2]) * g.sz), zm);
     Coef C;
     for (int z = p.z0; z <= p.z1; ++z) {
         const int64_t i = rc + (int64_t)z * g.sz + p.c0;
         float xc[4], ym[4], o[4];
-        unpack4(ld4(x, i), xc);
-        const float xm = ld1(x, rc + (int64_t)z * g.sz + ((p.c0 == 1 && g.per[0]) ? g.n[0] : p.c0 - 1));
-        unpack4(ld4(x, rm + (int64_t)z * g.sz + p.c0), ym);
+        unpack4(X.v(i), xc);
+        const float xm = X.s(rc + (int64_t)z * g.sz + ((p.c0 == 1 && g.per[0]) ? g.n[0] : p.c0 - 1));
+        unpack4(X.v(rm + (int64_t)z * g.sz + p.c0), ym);
         float l[4] = { Lc, Lc, Lc, Lc }, uu[4];
         if (MODE == TM_PLB) coef_load<ND, TM_PLB>(g, L, Lc, i, C, z == p.z0, p, z);
         // x component
@@ -503,9 +515,34 @@ __global__ void __launch_bounds__(WL_VB, WL_G_MINB) k_apply_gradient(Grid g, VT 
     for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
         VPos ps = vt_pos(g, vt, tile);
         if (ps.nv == 0) continue;
-#define CALL(M) gradient_tile<ND, M>(g, ps, u, L, Lc, x, p, isc)
+#define CALL(M) gradient_tile<ND, M, 0>(g, ps, u, L, Lc, x, p, isc, nullptr, 0.0f)
         TILE_MODES(plain[tile], CALL);
 #undef CALL
+    }
+}
+
+// the same with the smoother's last update x += alpha e (iteration kprev) applied on the fly; the update is owed under the
+// conditions of k_pcg_last: the smoother is live, or it stopped in that very iteration
+template <int ND>
+__global__ void __launch_bounds__(WL_VB, WL_G_MINB) k_apply_gradient_pend(Grid g, VT vt, const int* __restrict__ plain, float* __restrict__ u, const float* __restrict__ L, float Lc,
+                                                               const float* __restrict__ x, float* __restrict__ p, const DevScal* __restrict__ ds,
+                                                               const float* __restrict__ e, const PcgScal* __restrict__ sc, int kprev)
+{
+    const float isc = 1.0f / ds->pscale;
+    const bool owed = sc->live || sc->stop_k == kprev;
+    const float a = (float)sc->alpha;
+    for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
+        VPos ps = vt_pos(g, vt, tile);
+        if (ps.nv == 0) continue;
+        if (owed) {
+#define CALL(M) gradient_tile<ND, M, 1>(g, ps, u, L, Lc, x, p, isc, e, a)
+            TILE_MODES(plain[tile], CALL);
+#undef CALL
+        } else {
+#define CALL(M) gradient_tile<ND, M, 0>(g, ps, u, L, Lc, x, p, isc, nullptr, 0.0f)
+            TILE_MODES(plain[tile], CALL);
+#undef CALL
+        }
     }
 }
 
@@ -1043,6 +1080,13 @@ void wl_k_residual(wl_sim* s, const float* u, float w)
 void wl_k_apply_gradient(wl_sim* s, float* u)
 {
     Level& lv = s->lev[0];
+    if (s->pend_e) {
+        const float* e = s->pend_e;
+        s->pend_e = nullptr;
+        VDISPATCH(s, WLK_GRADIENT, 0, lv.vt, k_apply_gradient_pend<2>, k_apply_gradient_pend<3>, lv.g, lv.vt, lv.plain, u, lv.L, lv.Lc, lv.x, s->p, s->ds,
+                  e, &s->ds->pcg[0], s->pend_k);
+        return;
+    }
     VDISPATCH(s, WLK_GRADIENT, 0, lv.vt, k_apply_gradient<2>, k_apply_gradient<3>, lv.g, lv.vt, lv.plain, u, lv.L, lv.Lc, lv.x, s->p, s->ds);
 }
 
