@@ -256,7 +256,7 @@ static int solve(wl_sim* s, bool defer_x)
     const wl_mg& mg = s->cfg.mg;
     int nv = 0;
     if (mg.fixed_vcycles > 0) {
-        for (; nv < mg.fixed_vcycles; ++nv) { wl_k_vcycle(s, 0); wl_k_smooth(s, 0, mg.smooth_iters, nv + 1 < mg.fixed_vcycles ? 1 : (defer_x ? -1 : 0)); }
+        for (; nv < mg.fixed_vcycles; ++nv) { wl_k_vcycle(s, 0); wl_k_smooth(s, 0, mg.smooth_iters, nv + 1 < mg.fixed_vcycles ? (s->nlev > 1 ? 2 : 1) : (defer_x ? -1 : 0)); }
         s->res[s->solve_slot] = -1.0;
     } else {
         double res = 0.0;

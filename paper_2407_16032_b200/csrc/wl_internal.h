@@ -76,6 +76,8 @@ struct wl_sim {
     int mbox_lo[3], mbox_hi[3]; // padded coordinates of the box the last measure! rewrote (the whole array the first time)
     const float* pend_e;     // the last smoother call of a solve left its final x += alpha e to apply_gradient (wl_pcgfused.cu): the direction, else null
     int pend_k;              // ... and the iteration whose update that is
+    const float *pr_r, *pr_q, *pr_e;   // between two V-cycles of a solve: the smoother left x += alpha e, r -= alpha q to restrict(0) and prolong(0) (null: nothing pending)
+    int pr_k;
     int fused0;              // level 0 takes the one-sweep PCG form; its r2, q2 live in a dead velocity buffer (wl_api.cu solver_scratch)
     int fused;               // PCG smoother in its one-sweep form where the level allows (wl_tuning.no_fused switches it off)
     int fast_A;              // uniform tiles of PCG pass A go through k_pcg_A_fast (wl_tuning.no_fast_a switches it off)
@@ -186,7 +188,7 @@ void wl_k_restrict(wl_sim* s, int l);                // r_{l+1} = sum children r
 void wl_k_prolong(wl_sim* s, int l);                 // x_l += P x_{l+1}; r_l -= A_l P x_{l+1}
 // need_r = 0: nobody reads the residual of this level before it is rewritten (a coarse level before its prolongation, the
 // last smoother call of a solve with a fixed number of V-cycles): the one-sweep form then leaves r one update behind
-void wl_k_smooth(wl_sim* s, int l, int iters, int need_r = 1);   // need_r: 1 the residual is read afterwards; 0 only x; -1 only x, and by apply_gradient alone (level 0)
+void wl_k_smooth(wl_sim* s, int l, int iters, int need_r = 1);   // need_r: 1 the residual is read afterwards; 0 only x; -1 only x, and by apply_gradient alone (level 0); 2 x and r, and by the restrict(0) / prolong(0) of the next V-cycle alone
 void wl_k_coarse_prog(wl_sim* s, const CoarseProg& P);   // one k_coarse launch
 void wl_k_rsum(wl_sim* s, int l);                    // pcg[l].rsum = sum of r over the coupled cells (stage hooks)
 void wl_k_vcycle(wl_sim* s, int l);

@@ -548,8 +548,10 @@ __global__ void __launch_bounds__(WL_VB, WL_G_MINB) k_apply_gradient_pend(Grid g
 
 // ---------------------------------------------------------------- residual restriction
 // r_c[C] = sum of the 2^n children; x_c = 0 (R-S).  One thread per four coarse cells.
-template <int ND, int MODE>
-__device__ __forceinline__ void restrict_tile(const Grid& gf, const Grid& gc, const VPos& p, const float* rf, const float* iDc_arr, float* rc, float* xc, double& rsum)
+// PEND: the fine level's smoother left its last update to its readers (wl_pcgfused.cu): r stands for r - a q
+template <int ND, int MODE, int PEND = 0>
+__device__ __forceinline__ void restrict_tile(const Grid& gf, const Grid& gc, const VPos& p, const float* rf, const float* iDc_arr, float* rc, float* xc, double& rsum,
+                                              const float* qf = nullptr, float a = 0.0f)
 {
     const int f0 = 2 * p.c0 - 1, f1 = 2 * p.c1 - 1;      // first fine child (f0 = 1 + 8 gx: 32-byte aligned)
     for (int z = p.z0; z <= p.z1; ++z) {
@@ -559,9 +561,11 @@ __device__ __forceinline__ void restrict_tile(const Grid& gf, const Grid& gc, co
             for (int a1 = 0; a1 < 2; ++a1) {
                 const int64_t b = gidx(gf, f0, f1 + a1, ND == 3 ? 2 * z - 1 + a2 : 0);
                 float4 lo = ld4(rf, b);
+                if (PEND) { const float4 t = ld4(qf, b); lo.x = __fmaf_rn(-a, t.x, lo.x); lo.y = __fmaf_rn(-a, t.y, lo.y); lo.z = __fmaf_rn(-a, t.z, lo.z); lo.w = __fmaf_rn(-a, t.w, lo.w); }
                 s[0] += lo.x; s[0] += lo.y; s[1] += lo.z; s[1] += lo.w;
                 if (p.nv > 2) {
                     float4 hi = ld4(rf, b + 4);
+                    if (PEND) { const float4 t = ld4(qf, b + 4); hi.x = __fmaf_rn(-a, t.x, hi.x); hi.y = __fmaf_rn(-a, t.y, hi.y); hi.z = __fmaf_rn(-a, t.z, hi.z); hi.w = __fmaf_rn(-a, t.w, hi.w); }
                     s[2] += hi.x; s[2] += hi.y; s[3] += hi.z; s[3] += hi.w;
                 }
             }
@@ -590,14 +594,43 @@ __global__ void __launch_bounds__(WL_VB) k_restrict_r(Grid gf, Grid gc, VT vt, c
     }
 }
 
+// the same with the fine level's pending update (iteration kprev of its smoother; owed as in k_pcg_last)
+template <int ND>
+__global__ void __launch_bounds__(WL_VB) k_restrict_r_pend(Grid gf, Grid gc, VT vt, const int* __restrict__ plain, const float* __restrict__ rf, const float* __restrict__ iD,
+                                                           float* __restrict__ rc, float* __restrict__ xc, PcgScal* scc, RedBuf rb,
+                                                           const float* __restrict__ qf, const PcgScal* __restrict__ scf, int kprev)
+{
+    double v[1] = { 0.0 };
+    const bool owed = scf->live || scf->stop_k == kprev;
+    const float a = (float)scf->alpha;
+    for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
+        VPos p = vt_pos(gc, vt, tile);
+        if (p.nv == 0) continue;
+        const bool gen = plain[tile] == TM_GEN;
+        if (owed) {
+            if (gen) restrict_tile<ND, TM_GEN, 1>(gf, gc, p, rf, iD, rc, xc, v[0], qf, a);
+            else     restrict_tile<ND, TM_PLI, 1>(gf, gc, p, rf, iD, rc, xc, v[0], qf, a);
+        } else {
+            if (gen) restrict_tile<ND, TM_GEN>(gf, gc, p, rf, iD, rc, xc, v[0]);
+            else     restrict_tile<ND, TM_PLI>(gf, gc, p, rf, iD, rc, xc, v[0]);
+        }
+    }
+    if (grid_reduce<1, OpSum>(v, rb)) {
+        if (threadIdx.x == 0) scc->rsum = v[0];
+    }
+}
+
 // ---------------------------------------------------------------- prolongation + increment
 // e = P x_c (piecewise constant); x_f += e; r_f -= A_f e (R-S)
 __device__ __forceinline__ int par(int c) { return (c + 1) >> 1; }          // parent of a fine index (ghost 0 -> 0, n+1 -> n/2+1)
 __device__ __forceinline__ int wrapC(int C, int n, int per) { if (per) { if (C < 1) C += n; else if (C > n) C -= n; } return C; }
 
-template <int ND, int MODE>
+// PEND: x_f stands for x_f + a e and r_f for rin - a q (the fine smoother's last update, left to its readers); the results go to
+// xf and rf as always
+template <int ND, int MODE, int PEND = 0>
 __device__ __forceinline__ void prolong_tile(const Grid& gf, const Grid& gc, const VPos& p, const float* L, float Lc, const float* iD,
-                                             const float* xc, float* xf, float* rf, double& rsum)
+                                             const float* xc, float* xf, float* rf, double& rsum,
+                                             const float* rin = nullptr, const float* e = nullptr, const float* q = nullptr, float a = 0.0f)
 {
     const int64_t rc = (int64_t)WL_OFF + (int64_t)p.c1 * gf.sy;
     const int Ca = par(p.c0);                       // parents of the group: Ca, Ca, Ca+1, Ca+1
@@ -628,7 +661,14 @@ __device__ __forceinline__ void prolong_tile(const Grid& gf, const Grid& gc, con
         coef_load<ND, MODE>(gf, L, Lc, i, C, z == p.z0, p, z);
         float xo[4], ro[4];
         unpack4(*reinterpret_cast<const float4*>(xf + i), xo);
-        unpack4(*reinterpret_cast<const float4*>(rf + i), ro);
+        if (PEND == 1) {
+            float ee[4], qq[4];
+            unpack4(*reinterpret_cast<const float4*>(rin + i), ro);
+            unpack4(ld4(e, i), ee); unpack4(ld4(q, i), qq);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { xo[k] += a * ee[k]; ro[k] = __fmaf_rn(-a, qq[k], ro[k]); }
+        } else if (PEND == 2) unpack4(*reinterpret_cast<const float4*>(rin + i), ro);      // nothing owed: r only changes buffers
+        else unpack4(*reinterpret_cast<const float4*>(rf + i), ro);
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             xo[k] += w[k + 1];
@@ -651,6 +691,36 @@ __global__ void __launch_bounds__(WL_VB, WL_P_MINB) k_prolong(Grid gf, Grid gc, 
 #define CALL(M) prolong_tile<ND, M>(gf, gc, p, L, Lc, iD, xc, xf, rf, v[0])
         TILE_MODES(plain[tile], CALL);
 #undef CALL
+    }
+    if (grid_reduce<1, OpSum>(v, rb)) {
+        if (threadIdx.x == 0) scf->rsum = v[0];
+    }
+}
+
+template <int ND>
+__global__ void __launch_bounds__(WL_VB, WL_P_MINB) k_prolong_pend(Grid gf, Grid gc, VT vt, const int* __restrict__ plain, const float* __restrict__ L, float Lc, const float* __restrict__ iD,
+                                                        const float* __restrict__ xc, float* __restrict__ xf, float* __restrict__ rf, PcgScal* scf, RedBuf rb,
+                                                        const float* rin, const float* __restrict__ e, const float* __restrict__ q, int kprev)
+{
+    double v[1] = { 0.0 };
+    const bool owed = scf->live || scf->stop_k == kprev;
+    const float a = owed ? (float)scf->alpha : 0.0f;
+    for (int tile = blockIdx.x; tile < vt.ntiles; tile += gridDim.x) {
+        VPos p = vt_pos(gf, vt, tile);
+        if (p.nv == 0) continue;
+        if (owed) {
+#define CALL(M) prolong_tile<ND, M, 1>(gf, gc, p, L, Lc, iD, xc, xf, rf, v[0], rin, e, q, a)
+            TILE_MODES(plain[tile], CALL);
+#undef CALL
+        } else if (rin != rf) {       // nothing owed, but the residual sits in the other buffer
+#define CALL(M) prolong_tile<ND, M, 2>(gf, gc, p, L, Lc, iD, xc, xf, rf, v[0], rin, e, q, a)
+            TILE_MODES(plain[tile], CALL);
+#undef CALL
+        } else {
+#define CALL(M) prolong_tile<ND, M>(gf, gc, p, L, Lc, iD, xc, xf, rf, v[0])
+            TILE_MODES(plain[tile], CALL);
+#undef CALL
+        }
     }
     if (grid_reduce<1, OpSum>(v, rb)) {
         if (threadIdx.x == 0) scf->rsum = v[0];
@@ -1170,6 +1240,11 @@ void wl_k_restrict(wl_sim* s, int l)
 {
     Level &lf = s->lev[l], &lc = s->lev[l + 1];
     if (l >= s->pk_level) { CoarseProg P; P.n = 0; prog_add(P, COP_RESTRICT, l, 0); coarse_launch(s, P); return; }
+    if (l == 0 && s->pr_r) {       // the smoother's last update is still pending (wl_pcgfused.cu): r = pr_r - alpha pr_q
+        VDISPATCH(s, WLK_RESTRICT, 0, lc.vt, k_restrict_r_pend<2>, k_restrict_r_pend<3>, lf.g, lc.g, lc.vt, lc.plain, s->pr_r, lc.iD, lc.r, lc.x, &s->ds->pcg[1], s->rb,
+                  s->pr_q, &s->ds->pcg[0], s->pr_k);
+        return;
+    }
     VDISPATCH(s, WLK_RESTRICT, l > 0, lc.vt, k_restrict_r<2>, k_restrict_r<3>, lf.g, lc.g, lc.vt, lc.plain, lf.r, lc.iD, lc.r, lc.x, &s->ds->pcg[l + 1], s->rb);
 }
 
@@ -1177,6 +1252,13 @@ void wl_k_prolong(wl_sim* s, int l)
 {
     Level &lf = s->lev[l], &lc = s->lev[l + 1];
     if (l >= s->pk_level) { CoarseProg P; P.n = 0; prog_add(P, COP_PROLONG, l, 0); coarse_launch(s, P); return; }
+    if (l == 0 && s->pr_r) {       // ... and is applied here, where x and r are rewritten anyway
+        const float* rin = s->pr_r;
+        s->pr_r = nullptr;
+        VDISPATCH(s, WLK_PROLONG, 0, lf.vt, k_prolong_pend<2>, k_prolong_pend<3>, lf.g, lc.g, lf.vt, lf.plain, lf.L, lf.Lc, lf.iD, lc.x, lf.x, lf.r, &s->ds->pcg[0], s->rb,
+                  rin, s->pr_e, s->pr_q, s->pr_k);
+        return;
+    }
     VDISPATCH(s, WLK_PROLONG, l > 0, lf.vt, k_prolong<2>, k_prolong<3>, lf.g, lc.g, lf.vt, lf.plain, lf.L, lf.Lc, lf.iD, lc.x, lf.x, lf.r, &s->ds->pcg[l], s->rb);
 }
 
