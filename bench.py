@@ -302,8 +302,15 @@ def alg_bytes_table(cfg, prof) -> dict:
     alg["conv_diff_bdim"] = conv_alg_bytes(cfg)
     if "pcg_fused" in prof:                           # one-sweep form: every fine-level pcg_matvec launch is a first sweep, r -> e', q
         alg["pcg_matvec"] = 4 * (1 + 2)
-        # ... and of the two last sweeps of a solve (fixed two V-cycles) the second leaves r alone (x, e' -> x): mean of 24 and 12
-        alg["pcg_update"] = (4 * (4 + 2) + 4 * (2 + 1)) / 2
+        fv = int(cfg.get("fixed_vcycles", 2))
+        if fv > 0 and "pcg_update" not in prof:
+            # fixed V-cycles: no last sweep on level 0.  The final update of a smoother call is applied by its readers on the fly:
+            # between two V-cycles restrict(0) reads q too (+4) and prolong(0) e and q (+8); apply_gradient reads e (+4)
+            alg["restrict"] += 4 * (fv - 1) / fv
+            alg["prolong"] += 8 * (fv - 1) / fv
+            alg["apply_gradient"] += 4
+        else:
+            alg["pcg_update"] = 4 * (4 + 2)           # tolerance mode: every call ends with x, r, e', q -> x, r
     return alg
 
 
