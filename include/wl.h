@@ -91,7 +91,7 @@ typedef struct {
     int no_block_levels; /* small levels by the cooperative kernel instead of the one-block kernel */
     int no_tma_cd;       /* conv_diff from the register-staged ring (k_cd_tile2) instead of the TMA-fed one */
     int zc;              /* planes per tile of the vector kernels (0: 8) */
-    long long pk_max_cells; /* levels >= 1 with at most this many cells run inside the persistent kernels (0: 1 M; < 0: none) */
+    long long pk_max_cells; /* levels >= 1 with at most this many cells run inside the persistent kernels (0: 2^20; < 0: none) */
     int pk_blocks_per_sm;   /* co-resident blocks per SM of the cooperative kernel (0: 2) */
     int pk_fail;            /* test hook: treat the first cooperative / cluster launch as refused by the device (exercises the fallback) */
 } wl_tuning;

@@ -124,7 +124,7 @@ static Grid make_grid(int nd, const int* n, const int* per)
 static long long pk_max_cells(const wl_config* c)
 {
     if (c->tune.pk_max_cells < 0) return 0;
-    return c->tune.pk_max_cells > 0 ? c->tune.pk_max_cells : 1000000;
+    return c->tune.pk_max_cells > 0 ? c->tune.pk_max_cells : (1ll << 20);     // 1 Mi: a 64 x 64 x 256 level (N2) is still one of them
 }
 
 // Vector tiling of a level.  Coarse levels are latency-bound, not bandwidth-bound: they take fewer

@@ -75,7 +75,7 @@ struct DevScal {
     double force[3];
     double resmax;
     int    nan_flag;
-    int    band_count;   // faces with mu1 != 0 found by the last measure! (may exceed the list capacity)
+    int    band_count[4];// faces with mu1 != 0 found by the last measure!, per velocity component (each may exceed its third of the list)
     double energy[2];    // kinetic energy, enstrophy (wl_energy)
 };
 

@@ -643,13 +643,15 @@ __global__ void __launch_bounds__(128) k_cd_band(FlowP P, const float* __restric
     const float dt = ds->dt;
     const float V[3] = { ds->vel[0], ds->vel[1], ds->vel[2] };
     const float scale = corrector ? 0.5f : 1.0f;
-    const int cnt = ds->band_count;
+    // blockIdx.y = velocity component: the list holds one segment of cap / 3 entries per component (k_measure), so that a warp
+    // runs ONE instantiation of band_face instead of up to three one after the other
+    const int i = blockIdx.y, cap3 = cap / 3;
+    const int cnt = ds->band_count[i];
+    const bool fits = ds->band_count[0] <= cap3 && ds->band_count[1] <= cap3 && ds->band_count[2] <= cap3;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x, t0 = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (cnt <= cap) {
+    if (fits) {
         for (int64_t e = t0; e < cnt; e += stride) {
-            const long long code = list[e];
-            const int i = (int)(code & 3);
-            int64_t q = (code >> 2) - WL_OFF;
+            int64_t q = (list[(int64_t)i * cap3 + e] >> 2) - WL_OFF;
             const int c2 = ND == 3 ? (int)(q / g.sz) : 0;
             if (ND == 3) q -= (int64_t)c2 * g.sz;
             const int c1 = (int)(q / g.sy), c0 = (int)(q - (int64_t)c1 * g.sy);
@@ -657,7 +659,7 @@ __global__ void __launch_bounds__(128) k_cd_band(FlowP P, const float* __restric
             else if (i == 1) band_face<ND, 1>(P, w, u0, mu1, out, c0, c1, c2, dt, V[1], scale);
             else if (ND == 3) band_face<ND, 2>(P, w, u0, mu1, out, c0, c1, c2, dt, V[2], scale);
         }
-    } else {
+    } else if (i == 0) {
         // the list overflowed (a body far larger than the capacity heuristic): scan every interior face
         const int64_t n01 = (int64_t)g.n[0] * g.n[1], tot = n01 * g.n[2];
         for (int64_t e = t0; e < tot; e += stride) {
@@ -725,8 +727,8 @@ void wl_k_conv_diff_bdim(wl_sim* s, const float* w, const float* u0, float* out,
     }
     if (s->cfg.body.kind != WL_BODY_NONE) {
         ProfScope ps(s, WLK_CONVDIFF_BAND);
-        const int blocks = s->sm_count * 8;
-        if (s->nd == 3) k_cd_band<3><<<blocks, 128, 0, s->st>>>(P, w, u0, s->mu1, out, s->ds, s->band_list, s->band_cap, corrector);
-        else            k_cd_band<2><<<blocks, 128, 0, s->st>>>(P, w, u0, s->mu1, out, s->ds, s->band_list, s->band_cap, corrector);
+        const int blocks = s->sm_count * 4;          // x the components (grid y)
+        if (s->nd == 3) k_cd_band<3><<<dim3(blocks, 3), 128, 0, s->st>>>(P, w, u0, s->mu1, out, s->ds, s->band_list, s->band_cap, corrector);
+        else            k_cd_band<2><<<dim3(blocks, 2), 128, 0, s->st>>>(P, w, u0, s->mu1, out, s->ds, s->band_list, s->band_cap, corrector);
     }
 }

@@ -99,10 +99,46 @@ __global__ void __launch_bounds__(512) k_measure(Grid g, Tiling T, BodyP b, cons
 #pragma unroll
             for (int k = 0; k < ND; ++k) inner = inner && c[k] >= 1 && c[k] <= g.n[k];
             if (any && inner) {
-                const int slot = atomicAdd(&dsw->band_count, 1);
-                if (slot < band_cap) band[slot] = ((long long)id << 2) | i;
+                // one third of the list per component: the band kernel's warps then work on one component each
+                const int cap3 = band_cap / 3, slot = atomicAdd(&dsw->band_count[i], 1);
+                if (slot < cap3) band[(int64_t)i * cap3 + slot] = ((long long)id << 2) | i;
             }
         }
+    }
+}
+
+// General bodies (V is a per-face field): the boundary-normal faces c_i in {1, N_i + 1} of a non-periodic direction carry mu0 = 0
+// (R-O), so BDIM! puts V there until BC! overwrites it; after the first measure! only the box the body can reach is re-measured, and
+// this kernel keeps V_i on those planes current (V of a non-rigid or spinning map changes everywhere in time).
+template <int ND>
+__global__ void __launch_bounds__(256) k_measure_wallV(Grid g, BodyP b, const DevScal* __restrict__ ds, float* __restrict__ Vf)
+{
+    int64_t A[3];
+    A[0] = (int64_t)g.S[1] * g.S[2]; A[1] = (int64_t)g.S[0] * g.S[2]; A[2] = (int64_t)g.S[0] * g.S[1];
+    int64_t total = 0;
+    for (int j = 0; j < ND; ++j) total += g.per[j] ? 0 : 2 * A[j];
+    for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+        int64_t rem = t;
+        int j = 0;
+        for (;; ++j) {
+            const int64_t cnt = g.per[j] ? 0 : 2 * A[j];
+            if (rem < cnt) break;
+            rem -= cnt;
+        }
+        const int plane = (int)(rem / A[j]);
+        const int64_t ab = rem % A[j];
+        const int d0 = j == 0 ? 1 : 0, d1 = j == 2 ? 1 : 2;
+        int c[3] = { 0, 0, 0 };
+        c[d0] = (int)(ab % g.S[d0]);
+        c[d1] = (int)(ab / g.S[d0]);
+        if (ND == 2) c[2] = 0;
+        c[j] = plane == 0 ? 1 : g.n[j] + 1;
+        double xf[3], nd[3];
+        float vel[3] = { 0.f, 0.f, 0.f };
+#pragma unroll
+        for (int k = 0; k < 3; ++k) xf[k] = k < ND ? (double)((float)wrapc(c[k], g.n[k], g.per[k]) - 0.5f) - (k == j ? 0.5 : 0.0) : 0.0;
+        body_eval<ND, double>(b, ds->part, xf, nd, vel);
+        Vf[j * g.nalloc + gidx(g, c[0], c[1], c[2])] = vel[j];
     }
 }
 
@@ -402,19 +438,40 @@ void wl_k_set_time(wl_sim* s, double t, float dt, int t_mode, int dt_mode)
 
 // The box of padded cells the body can reach, grown by `margin` cells: the supported motion is a sinusoidal translation of
 // known amplitude, so the box is known on the host although t is device-resident.  interior: clip to the interior cells.
+// Box (padded cell coordinates, origin o and extents e) that the body, grown by `margin` cells, can reach at any time: the union over
+// the primitives that ADD material (the first one and every union; a difference only removes) of centre +- (motion amplitude +
+// extent / smallest scale of the map + margin).  A plane, or a map that can scale to nothing, reaches everywhere: the whole grid.
 void wl_body_box(const wl_sim* s, float margin, int interior, int o[3], int e[3])
 {
     const Grid& g = s->lev[0].g;
-    const wl_body& b = s->cfg.body;
+    const wl_config& c = s->cfg;
     for (int d = 0; d < 3; ++d) { o[d] = interior && d < s->nd ? 1 : 0; e[d] = interior ? g.n[d] : g.S[d]; }
+    if (c.body.kind == WL_BODY_NONE) return;
     for (int d = 0; d < s->nd; ++d) {
         const int first = interior ? 1 : 0, last = interior ? g.n[d] : g.n[d] + 1;
-        float ext = b.R;                                          // sphere / circle / cylinder cross-section
-        if (b.kind == WL_BODY_TORUS) ext = d == b.axis ? b.r : b.R + b.r;
-        float reach = ext + margin;
-        if (b.motion == WL_MOTION_SIN) reach += fabsf(b.amp[d]);
-        int lo = (int)floorf(b.centre[d] - reach), hi = (int)ceilf(b.centre[d] + reach) + 1;      // padded coordinates c = x + 1/2
-        if (b.kind == WL_BODY_CYLINDER && d == b.axis) { lo = first; hi = last; }                 // it spans the direction
+        int lo = last + 1, hi = first - 1;
+        bool whole = false;
+        for (int k = 0; k <= c.nextra && !whole; ++k) {
+            const wl_body& b = k == 0 ? c.body : c.extra[k - 1];
+            if (k > 0 && c.extra_op[k - 1] != WL_OP_UNION) continue;
+            if (b.kind == WL_BODY_PLANE || (b.kind == WL_BODY_CYLINDER && d == b.axis)) { whole = true; break; }   // it spans the direction
+            float ext = b.R;                                      // sphere / circle / cylinder cross-section
+            if (b.kind == WL_BODY_TORUS) ext = d == b.axis ? b.r : b.R + b.r;
+            if (b.shell > 0.0f) ext += b.shell;
+            float m = margin;
+            const float smin = 1.0f - fabsf(b.scale_amp[d]);      // xi = s (x - c), s = 1 + scale_amp cos(.): x-extent = extent / s
+            if (b.scale_amp[0] != 0.0f || b.scale_amp[1] != 0.0f || b.scale_amp[2] != 0.0f) {
+                if (smin < 0.25f) { whole = true; break; }
+                ext /= smin;
+                m = 1.5f * margin + 1.0f;                         // the distance of a non-rigid map is first-order (R-E3): a generous band
+            }
+            float reach = ext + m;
+            if (b.motion == WL_MOTION_SIN) reach += fabsf(b.amp[d]);
+            const int l = (int)floorf(b.centre[d] - reach), h = (int)ceilf(b.centre[d] + reach) + 1;      // padded coordinates c = x + 1/2
+            if (l < lo) lo = l;
+            if (h > hi) hi = h;
+        }
+        if (whole) { lo = first; hi = last; }
         if (lo < first) lo = first;
         if (hi > last) hi = last;
         if (g.per[d] && (lo <= 2 || hi >= g.n[d] - 1)) { lo = first; hi = last; }   // ghosts mirror the far side: whole direction
@@ -431,18 +488,23 @@ void wl_k_measure(wl_sim* s)
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_padded(s, g);
     const wl_body& b = s->cfg.body;
-    if (s->measured && b.kind != WL_BODY_NONE && !s->body.general) {      // a general body: the whole grid every time
+    if (s->measured && b.kind != WL_BODY_NONE) {
         int o[3], e[3];
         wl_body_box(s, s->cfg.eps + 2.0f, 0, o, e);                   // the face positions are half a cell off the centres
         T = wl_tiling(s->nd, o, e);
     }
+    const bool whole = !s->measured;
     for (int d = 0; d < 3; ++d) { s->mbox_lo[d] = T.o[d]; s->mbox_hi[d] = T.o[d] + T.e[d] - 1; }
     s->measured = 1;
-    cudaMemsetAsync(&s->ds->band_count, 0, sizeof(int), s->st);
+    cudaMemsetAsync(s->ds->band_count, 0, 4 * sizeof(int), s->st);
     {
         ProfScope ps(s, WLK_MEASURE);
         if (s->nd == 3) k_measure<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1, s->Vf, s->ds, s->band_list, s->band_cap);
         else            k_measure<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1, s->Vf, s->ds, s->band_list, s->band_cap);
+        if (s->Vf && !whole && (!g.per[0] || !g.per[1] || (s->nd == 3 && !g.per[2]))) {
+            if (s->nd == 3) k_measure_wallV<3><<<s->sm_count * 2, 256, 0, s->st>>>(g, s->body, s->ds, s->Vf);
+            else            k_measure_wallV<2><<<s->sm_count * 2, 256, 0, s->st>>>(g, s->body, s->ds, s->Vf);
+        }
     }
     wl_k_poisson_update(s);
 }
@@ -501,7 +563,7 @@ void wl_k_force(wl_sim* s, double t)
 {
     const Grid& g = s->lev[0].g;
     Tiling T = wl_tiles_interior(s, g);
-    if (s->cfg.body.kind != WL_BODY_NONE && !s->body.general) {      // K(d) vanishes further than one cell from the surface: the body's box is enough
+    if (s->cfg.body.kind != WL_BODY_NONE) {      // K(d) vanishes further than one cell from the surface: the body's box is enough
         int o[3], e[3];
         wl_body_box(s, 3.0f, 1, o, e);
         T = wl_tiling(s->nd, o, e);
