@@ -77,9 +77,15 @@ __global__ void __launch_bounds__(512) k_measure(Grid g, Tiling T, BodyP b, cons
                 double xf[3], nd[3];
 #pragma unroll
                 for (int k = 0; k < 3; ++k) xf[k] = k < ND ? (double)xc[k] - (k == i ? 0.5 : 0.0) : 0.0;
-                const float d = (float)body_eval<ND, double>(b, ds->part, xf, nd, vel);
+                // far from the surface (most faces) fp32 decides: further than eps, mu0 is exactly 0 or 1 and mu1 exactly 0 whatever the
+                // last digits of d (its fp32 error is ~1e-4 of a cell: the margin of one cell is ample); only the band pays for fp64
+                float nf[3];
+                float d = body_eval<ND, float>(b, ds->part, xf, nf, vel);
+                if (fabsf(d) <= b.eps + 1.0f) {
+                    d = (float)body_eval<ND, double>(b, ds->part, xf, nd, vel);
 #pragma unroll
-                for (int k = 0; k < 3; ++k) nrm[k] = (float)nd[k];
+                    for (int k = 0; k < 3; ++k) nrm[k] = (float)nd[k];
+                }
                 m0 = bdim_mu0(d, b.eps);
                 m1 = bdim_mu1(d, b.eps);
             }
