@@ -70,6 +70,24 @@ __global__ void __launch_bounds__(512) k_measure(Grid g, Tiling T, BodyP b, cons
         float xc[3];
 #pragma unroll
         for (int k = 0; k < 3; ++k) xc[k] = k < ND ? (float)wrapc(c[k], g.n[k], g.per[k]) - 0.5f : 0.0f;
+        // A cell whose CENTRE is far out in the fluid has all its faces (half a cell away) outside the band: mu0 = 1, mu1 = 0, and V,
+        // which enters only through (1 - mu0) and mu1, is not needed (k_measure_wallV supplies it on the forced boundary faces).  One fp32
+        // evaluation instead of three; the margin of 2.5 cells covers the half cell and the first-order distance of a non-rigid map.
+        if (b.n > 0) {
+            double xd[3];
+            float nf[3], vf[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) xd[k] = (double)xc[k];
+            if (body_eval<ND, float>(b, ds->part, xd, nf, vf) > b.eps + 2.5f) {
+#pragma unroll
+                for (int i = 0; i < ND; ++i) {
+                    mu0[i * g.nalloc + id] = (!g.per[i] && (c[i] == 1 || c[i] == g.n[i] + 1)) ? 0.0f : 1.0f;
+#pragma unroll
+                    for (int j = 0; j < ND; ++j) mu1[(i * ND + j) * g.nalloc + id] = 0.0f;
+                }
+                continue;
+            }
+        }
 #pragma unroll
         for (int i = 0; i < ND; ++i) {
             float m0 = 1.0f, m1 = 0.0f, nrm[3] = { 0.f, 0.f, 0.f }, vel[3] = { 0.f, 0.f, 0.f };
@@ -499,7 +517,6 @@ void wl_k_measure(wl_sim* s)
         wl_body_box(s, s->cfg.eps + 2.0f, 0, o, e);                   // the face positions are half a cell off the centres
         T = wl_tiling(s->nd, o, e);
     }
-    const bool whole = !s->measured;
     for (int d = 0; d < 3; ++d) { s->mbox_lo[d] = T.o[d]; s->mbox_hi[d] = T.o[d] + T.e[d] - 1; }
     s->measured = 1;
     cudaMemsetAsync(s->ds->band_count, 0, 4 * sizeof(int), s->st);
@@ -507,7 +524,7 @@ void wl_k_measure(wl_sim* s)
         ProfScope ps(s, WLK_MEASURE);
         if (s->nd == 3) k_measure<3><<<wl_grid(s, T), wl_block(3), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1, s->Vf, s->ds, s->band_list, s->band_cap);
         else            k_measure<2><<<wl_grid(s, T), wl_block(2), 0, s->st>>>(g, T, s->body, s->ds, s->mu0, s->mu1, s->Vf, s->ds, s->band_list, s->band_cap);
-        if (s->Vf && !whole && (!g.per[0] || !g.per[1] || (s->nd == 3 && !g.per[2]))) {
+        if (s->Vf && (!g.per[0] || !g.per[1] || (s->nd == 3 && !g.per[2]))) {
             if (s->nd == 3) k_measure_wallV<3><<<s->sm_count * 2, 256, 0, s->st>>>(g, s->body, s->ds, s->Vf);
             else            k_measure_wallV<2><<<s->sm_count * 2, 256, 0, s->st>>>(g, s->body, s->ds, s->Vf);
         }
