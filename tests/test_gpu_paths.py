@@ -296,3 +296,28 @@ def test_poisson_update_inside_the_body_box_equals_a_full_update(case):
             assert np.array_equal(g.dbg_get(name, l, padded=True), f.dbg_get(name, l, padded=True)), (name, l)
         assert g.dbg_pcg_scalars(l)["nlive"] == f.dbg_pcg_scalars(l)["nlive"] == float((O(o, "iD", l)[0] != 0).sum())
     o.close(); g.close(); f.close()
+
+
+@pytest.mark.parametrize("amp", [0.0, 1e-19])
+def test_solve_whose_smoother_has_nothing_to_do(amp):
+    """A uniform stream without a body is divergence-free: the residual of both projections is zero (amp = 0) or so small that
+    |rho| < tau stops the smoother in its first sweep (amp = 1e-19), on every level.  The updates that the one-sweep smoother
+    leaves to restrict(0), prolong(0) and apply_gradient are then NOT owed: the stream must come out untouched
+    (amp = 0: bit for bit) and as the oracle's."""
+    from oracle import wl_oracle as wo
+    from paper_2407_16032_b200 import wl
+    cfg = wi.make(ndim=3, dims=(136, 40, 24), U=(1.0, 0.0, 0.0), nu=0.02, exit_bc=1)
+    o, g = wo.OracleSim(cfg), wl.Sim(cfg)
+    u0 = np.zeros((3, 24, 40, 136)); u0[0] = 1.0
+    if amp:
+        u0 += amp * wi.random_velocity((136, 40, 24), seed=3)
+    o.set_fields(u=u0)
+    g.set_fields(u=np.ascontiguousarray(u0, dtype=np.float32))
+    for k in range(2):
+        o.mom_step(0.25); g.mom_step(0.25)
+    u, p = g.fields()
+    assert g.stats()["nan_flag"] == 0 and np.isfinite(u).all() and np.isfinite(p).all()
+    assert np.abs(u - o.interior("u")).max() <= 1e-6
+    if amp == 0.0:
+        assert np.array_equal(u[0], np.ones_like(u[0])) and not u[1:].any() and not p.any()
+    o.close(); g.close()
